@@ -1,0 +1,129 @@
+/* hisq.h -- C ABI of libhisq: the even-odd HISQ staggered Dslash on multiple right-hand sides and the
+ * multi-RHS conjugate gradient on (m^2 - D_eo D_oe) x = b, hand-written CUDA for sm_100a (B200).
+ *
+ * What is computed (arXiv:2306.01098, cited by line of reference/PAPER.md):
+ *
+ *   (D phi)(x) = sum_{mu=0..3} [ X_mu(x) phi(x+mu) - X_mu(x-mu)^+ phi(x-mu)
+ *                              + W_mu(x) phi(x+3mu) - W_mu(x-3mu)^+ phi(x-3mu) ]
+ *
+ * X = fat links, W = Naik links, both complex 3x3 with every constant and the staggered phases
+ * already folded in by the caller; site coordinates periodic, the colour-vector field
+ * periodic in x,y,z and ANTI-periodic in t -- the library applies that sign itself.
+ * D only connects sites of opposite parity pi(x) = (x+y+z+t) mod 2, so it splits into D_eo (even
+ * outputs from odd inputs) and D_oe.  The solver works on A = m^2 - D_eo D_oe, the even-even block
+ * of M^+ M for M = D + m (Eq. (1), :139-141 `applyMdaggM`).
+ *
+ * Conventions common to all calls
+ *   - mu = 0,1,2,3 <-> x,y,z,t; V = Lx*Ly*Lz*Lt; Vh = V/2.  All four extents must be even and >= 4.
+ *   - Site index, Eq. (4):  lex = x + Lx*(y + Ly*(z + Lz*t)),  h = lex / 2 (integer),
+ *     eo = h + pi(x)*Vh: even sites fill [0,Vh), odd sites [Vh,V).
+ *   - CANONICAL link array, Eq. (5): matrix of (x, mu) at slot mu*V + eo(x); each
+ *     matrix 9 complex numbers row-major U[a][b], (re, im) interleaved; (U phi)_a = sum_b U_ab phi_b.
+ *   - CANONICAL half-lattice field of one parity with n right-hand sides: element (k, h, c) at
+ *     ((k*Vh + h)*3 + c) complex, (re, im) interleaved  (k = RHS, c = colour).
+ *   - NATIVE half-lattice field (what hisq_dslash / hisq_cg read and write, so that no per-call
+ *     repack sits inside the operator): element (k, c, h) at ((k*3 + c)*Vh + h) complex.
+ *     hisq_spinor_pack / hisq_spinor_unpack convert.  RHS k is one contiguous block of 3*Vh complex.
+ *   - Element type follows `prec`: HISQ_FP32 -> float, HISQ_FP64 and HISQ_MIXED -> double.
+ *   - Unless a parameter says HOST, every data pointer is a CUDA DEVICE pointer, 16-byte aligned,
+ *     owned by the caller (e.g. a torch tensor's data_ptr()).  The library allocates no device
+ *     memory: the caller gives it one workspace (hisq_workspace_bytes / hisq_set_workspace).
+ *   - All work is enqueued on the stream given to hisq_set_stream (default: the legacy stream).
+ *   - Every function returns 0 on success or a negative HISQ_E* code; nothing throws or aborts.
+ *   - A context is not thread-safe; use one per host thread / per GPU.
+ */
+#ifndef HISQ_H
+#define HISQ_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hisq_ctx hisq_ctx; /* opaque; created by hisq_create, freed by hisq_destroy */
+
+enum { HISQ_FP32 = 4, HISQ_FP64 = 8, HISQ_MIXED = 12 }; /* `prec` */
+enum { HISQ_EVEN = 0, HISQ_ODD = 1 };                   /* parity of the OUTPUT sites */
+enum { HISQ_MAX_NRHS = 16 };
+
+enum {
+    HISQ_OK = 0,
+    HISQ_EINVAL = -1,       /* bad extent (odd or < 4), nrhs < 1 or > HISQ_MAX_NRHS, bad parity/prec, null
+                               or misaligned pointer, in/out aliasing, unknown option                      */
+    HISQ_ENOLINKS = -2,     /* hisq_dslash / hisq_cg before hisq_set_links                                 */
+    HISQ_ENOWORKSPACE = -3, /* no workspace set, or it is smaller than hisq_workspace_bytes(nrhs)          */
+    HISQ_ECUDA = -4,        /* a CUDA call failed; text via hisq_last_error                                */
+    HISQ_ENOCONV = -5,      /* max_iter reached; x holds the last iterate, hisq_get_info the residuals     */
+    HISQ_EBREAKDOWN = -6    /* <p, A p> <= 0 or a non-finite scalar appeared in CG                         */
+};
+
+/* Create a context for an Lx x Ly x Lz x Lt lattice on the current CUDA device.
+ * prec: HISQ_FP32 (fp32 links, fields, arithmetic), HISQ_FP64, or HISQ_MIXED (fp64 interface; CG runs
+ * the fp32 operator inside and an fp64 reliable update outside; hisq_dslash is the fp64 operator). */
+int hisq_create(hisq_ctx **h, int Lx, int Ly, int Lz, int Lt, int prec);
+int hisq_destroy(hisq_ctx *h);
+
+/* cuda_stream: a cudaStream_t passed as void* (e.g. torch.cuda.current_stream().cuda_stream). */
+int hisq_set_stream(hisq_ctx *h, void *cuda_stream);
+
+/* Bytes of device workspace needed for links (internal copy/copies) plus CG temporaries, reduction
+ * buffers and host-call staging for up to `nrhs` right-hand sides.  0 if the arguments are invalid. */
+size_t hisq_workspace_bytes(const hisq_ctx *h, int nrhs);
+/* Hand the library `bytes` of device memory at dev_ptr (256-byte aligned).  The caller keeps ownership
+ * and must keep it alive and untouched until hisq_destroy or the next hisq_set_workspace.  Setting a
+ * workspace invalidates links set earlier. */
+int hisq_set_workspace(hisq_ctx *h, void *dev_ptr, size_t bytes);
+
+/* Copy the two CANONICAL link arrays (each 4*V matrices, Eq. (5)) into the library's own layout
+ * (structure-of-arrays by 16-byte chunk, split by parity and direction; fp32 and fp64 copies for
+ * HISQ_MIXED).  Synchronises the stream before returning: the caller may free fat / naik at once.
+ * Links carry all coefficients and phases; the library applies none. */
+int hisq_set_links(hisq_ctx *h, const void *fat, const void *naik);
+
+/* out = D_eo in (parity = HISQ_EVEN: `out` on even sites, `in` on odd sites) or out = D_oe in
+ * (parity = HISQ_ODD), for nrhs fields at once, each link loaded once and applied to all of them
+ * (PAPER.md:582-586).  in / out: NATIVE half-lattice fields, must not overlap.  Asynchronous. */
+int hisq_dslash(hisq_ctx *h, void *out, const void *in, int parity, int nrhs);
+
+/* Solve (mass^2 - D_eo D_oe) x_k = b_k, k < nrhs, on even sites by conjugate gradient with
+ * independent alpha_k, beta_k per right-hand side and a shared operator application
+ * (PAPER.md:135, :141).  b, x: NATIVE even half-lattice fields; x is overwritten (initial guess 0).
+ * Stops when ||r_k|| <= tol * ||b_k|| (2-norm, not squared) for every k, confirmed on the residual
+ * recomputed as b - A x in fp64; converged right-hand sides are frozen while the rest continue.
+ * HISQ_MIXED: fp32 operator and fp32 r, p, Ap; every `reliable_interval` iterations x is accumulated
+ * in fp64 and r replaced by the fp64 true residual, the search direction kept.
+ * Returns after the solve has finished (synchronises the stream).  HISQ_ENOCONV / HISQ_EBREAKDOWN as above. */
+int hisq_cg(hisq_ctx *h, void *x, const void *b, double mass, double tol, int nrhs);
+
+/* Options: "max_iter" (default 100000), "reliable_interval" (default 100 for HISQ_MIXED, 0 = off for
+ * the others), "check_interval" (iterations enqueued between host polls of the convergence flag,
+ * default 32), "use_graph" (1: replay one CG iteration as a CUDA graph, default 1),
+ * "dslash_block" (threads per CTA of the Dslash kernel, 0 = default), "nrhs_inner" (RHS per thread, 0 = auto),
+ * "tile_y", "tile_z" (CTA sweep order blocking in y,z; 0 = auto). */
+int hisq_set_option(hisq_ctx *h, const char *key, double value);
+
+/* After hisq_cg: iterations done, number of fp64 true-residual recomputations, and per RHS the true
+ * relative residual ||b - A x|| / ||b|| (array of nrhs doubles on the HOST; any pointer may be NULL). */
+int hisq_get_info(const hisq_ctx *h, int *iterations, int *reliable_updates, double *true_rel_resid);
+
+/* CANONICAL <-> NATIVE half-lattice field conversion (device to device, asynchronous). */
+int hisq_spinor_pack(hisq_ctx *h, void *native, const void *canonical, int nrhs);
+int hisq_spinor_unpack(hisq_ctx *h, void *canonical, const void *native, int nrhs);
+
+/* End-to-end variants with HOST buffers (pinned or pageable) in the CANONICAL layout: copy in, pack,
+ * run, unpack, copy out, synchronise.  Staging lives in the workspace. */
+int hisq_dslash_host(hisq_ctx *h, void *out_host, const void *in_host, int parity, int nrhs);
+int hisq_cg_host(hisq_ctx *h, void *x_host, const void *b_host, double mass, double tol, int nrhs);
+
+/* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
+long long hisq_launch_count(const hisq_ctx *h);
+
+const char *hisq_strerror(int code);
+/* Text of the last CUDA error seen by this context ("" if none). */
+const char *hisq_last_error(const hisq_ctx *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HISQ_H */

@@ -1,0 +1,238 @@
+"""ctypes binding of libhisq.so (include/hisq.h).  Argument marshalling only: every step of the hot
+path runs in the library's CUDA kernels.  PyTorch supplies device memory (tensors) and the stream.
+
+There is deliberately no fallback: if the library is missing or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import torch
+
+from . import layout
+
+HISQ_FP32, HISQ_FP64, HISQ_MIXED = 4, 8, 12
+HISQ_EVEN, HISQ_ODD = 0, 1
+HISQ_MAX_NRHS = 16
+HISQ_ENOCONV, HISQ_EBREAKDOWN = -5, -6
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhisq.so")
+
+EXPORTS = [
+    "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
+    "hisq_set_links", "hisq_dslash", "hisq_cg", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
+    "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_launch_count", "hisq_strerror",
+    "hisq_last_error",
+]
+
+_lib = None
+
+
+class HisqError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libhisq error {code}: {msg}")
+        self.code = code
+
+
+def load_library() -> ctypes.CDLL:
+    """Load libhisq.so (must have been built: `python -m paper_2306_01098_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_2306_01098_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i, d, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+    lib.hisq_create.argtypes = [ctypes.POINTER(vp), i, i, i, i, i]
+    lib.hisq_destroy.argtypes = [vp]
+    lib.hisq_set_stream.argtypes = [vp, vp]
+    lib.hisq_workspace_bytes.argtypes = [vp, i]
+    lib.hisq_workspace_bytes.restype = sz
+    lib.hisq_set_workspace.argtypes = [vp, vp, sz]
+    lib.hisq_set_links.argtypes = [vp, vp, vp]
+    lib.hisq_dslash.argtypes = [vp, vp, vp, i, i]
+    lib.hisq_cg.argtypes = [vp, vp, vp, d, d, i]
+    lib.hisq_set_option.argtypes = [vp, ctypes.c_char_p, d]
+    lib.hisq_get_info.argtypes = [vp, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(d)]
+    lib.hisq_spinor_pack.argtypes = [vp, vp, vp, i]
+    lib.hisq_spinor_unpack.argtypes = [vp, vp, vp, i]
+    lib.hisq_dslash_host.argtypes = [vp, vp, vp, i, i]
+    lib.hisq_cg_host.argtypes = [vp, vp, vp, d, d, i]
+    lib.hisq_launch_count.argtypes = [vp]
+    lib.hisq_launch_count.restype = ctypes.c_longlong
+    lib.hisq_strerror.argtypes = [i]
+    lib.hisq_strerror.restype = ctypes.c_char_p
+    lib.hisq_last_error.argtypes = [vp]
+    lib.hisq_last_error.restype = ctypes.c_char_p
+    lib.hisq_debug_dslash_regs.argtypes = [i, i, i]
+    lib.hisq_debug_tiles.argtypes = [vp, i, ctypes.POINTER(i)]
+    _lib = lib
+    return lib
+
+
+_PREC = {"fp32": HISQ_FP32, "fp64": HISQ_FP64, "mixed": HISQ_MIXED}
+
+
+class Hisq:
+    """One lattice + precision on one GPU.  Method names mirror the C ABI.
+
+    Fields passed to dslash / cg are torch CUDA tensors in the NATIVE layout [nrhs, 3, Vh] complex
+    (complex64 for fp32, complex128 otherwise); `pack` / `unpack` convert from / to the canonical
+    [nrhs, Vh, 3].  Links are canonical [4, V, 3, 3] complex (Eq. 5: slot mu*V + eo).
+    """
+
+    def __init__(self, L: Sequence[int], prec: str = "fp64", nrhs_max: int = 1, device: Optional[torch.device] = None):
+        layout.check_extents(L)
+        if not torch.cuda.is_available():
+            raise RuntimeError("libhisq needs a CUDA device (no CPU fallback)")
+        self.lib = load_library()
+        self.L = tuple(int(v) for v in L)
+        self.V = layout.volume(L)
+        self.Vh = self.V // 2
+        self.prec = prec
+        self.device = torch.device(device if device is not None else "cuda:0")
+        self.cdtype = torch.complex64 if prec == "fp32" else torch.complex128
+        self.nrhs_max = int(nrhs_max)
+        self._h = ctypes.c_void_p()
+        with torch.cuda.device(self.device):
+            self._check(self.lib.hisq_create(ctypes.byref(self._h), *self.L, _PREC[prec]))
+            self._check(self.lib.hisq_set_stream(self._h, ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)))
+            nbytes = self.lib.hisq_workspace_bytes(self._h, self.nrhs_max)
+            if nbytes == 0:
+                raise HisqError(-1, "hisq_workspace_bytes rejected the arguments")
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self._check(self.lib.hisq_set_workspace(self._h, ctypes.c_void_p(self.workspace.data_ptr()), nbytes))
+
+    # -- plumbing ---------------------------------------------------------------------------------
+    def _check(self, code: int, allow=()):
+        if code != 0 and code not in allow:
+            msg = self.lib.hisq_strerror(code).decode()
+            if code == -4 and self._h:
+                msg += ": " + self.lib.hisq_last_error(self._h).decode()
+            raise HisqError(code, msg)
+        return code
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self.lib.hisq_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def use_current_stream(self):
+        self._check(self.lib.hisq_set_stream(self._h, ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)))
+
+    def _ptr(self, t: torch.Tensor, shape=None, dtype=None):
+        if not t.is_cuda or not t.is_contiguous():
+            raise ValueError("expected a contiguous CUDA tensor")
+        if dtype is not None and t.dtype != dtype:
+            raise ValueError(f"expected dtype {dtype}, got {t.dtype}")
+        if shape is not None and tuple(t.shape) != tuple(shape):
+            raise ValueError(f"expected shape {tuple(shape)}, got {tuple(t.shape)}")
+        return ctypes.c_void_p(t.data_ptr())
+
+    def new_field(self, nrhs: int, native: bool = True) -> torch.Tensor:
+        shape = (nrhs, 3, self.Vh) if native else (nrhs, self.Vh, 3)
+        return torch.empty(shape, dtype=self.cdtype, device=self.device)
+
+    # -- the C ABI --------------------------------------------------------------------------------
+    def set_option(self, key: str, value: float):
+        self._check(self.lib.hisq_set_option(self._h, key.encode(), float(value)))
+
+    def set_links(self, fat: torch.Tensor, naik: torch.Tensor):
+        shape = (4, self.V, 3, 3)
+        self._check(self.lib.hisq_set_links(self._h, self._ptr(fat, shape, self.cdtype), self._ptr(naik, shape, self.cdtype)))
+
+    def pack(self, canonical: torch.Tensor) -> torch.Tensor:
+        n = canonical.shape[0]
+        out = self.new_field(n, native=True)
+        self._check(self.lib.hisq_spinor_pack(self._h, self._ptr(out), self._ptr(canonical, (n, self.Vh, 3), self.cdtype), n))
+        return out
+
+    def unpack(self, native: torch.Tensor) -> torch.Tensor:
+        n = native.shape[0]
+        out = self.new_field(n, native=False)
+        self._check(self.lib.hisq_spinor_unpack(self._h, self._ptr(out), self._ptr(native, (n, 3, self.Vh), self.cdtype), n))
+        return out
+
+    def dslash(self, inp: torch.Tensor, parity: int, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        n = inp.shape[0]
+        if out is None:
+            out = self.new_field(n)
+        self._check(self.lib.hisq_dslash(self._h, self._ptr(out, (n, 3, self.Vh), self.cdtype),
+                                         self._ptr(inp, (n, 3, self.Vh), self.cdtype), int(parity), n))
+        return out
+
+    def cg(self, b: torch.Tensor, mass: float, tol: float, x: Optional[torch.Tensor] = None, strict: bool = True):
+        """Returns (x, info) with info = dict(iterations, reliable_updates, true_rel_resid, status)."""
+        n = b.shape[0]
+        if x is None:
+            x = self.new_field(n)
+        code = self.lib.hisq_cg(self._h, self._ptr(x, (n, 3, self.Vh), self.cdtype), self._ptr(b, (n, 3, self.Vh), self.cdtype),
+                                float(mass), float(tol), n)
+        self._check(code, allow=() if strict else (HISQ_ENOCONV, HISQ_EBREAKDOWN))
+        return x, self.info(n, code)
+
+    def info(self, nrhs: int, status: int = 0) -> dict:
+        it, rel = ctypes.c_int(0), ctypes.c_int(0)
+        res = (ctypes.c_double * HISQ_MAX_NRHS)()
+        self._check(self.lib.hisq_get_info(self._h, ctypes.byref(it), ctypes.byref(rel), res))
+        return {"iterations": it.value, "reliable_updates": rel.value, "true_rel_resid": [res[k] for k in range(nrhs)],
+                "status": status}
+
+    # host-buffer (end-to-end) entry points: canonical layout, CPU tensors (pinned or not)
+    def dslash_host(self, out_host: torch.Tensor, in_host: torch.Tensor, parity: int):
+        n = in_host.shape[0]
+        for t in (out_host, in_host):
+            if t.is_cuda or not t.is_contiguous() or t.dtype != self.cdtype or tuple(t.shape) != (n, self.Vh, 3):
+                raise ValueError("expected contiguous CPU tensors [nrhs, Vh, 3]")
+        self._check(self.lib.hisq_dslash_host(self._h, ctypes.c_void_p(out_host.data_ptr()), ctypes.c_void_p(in_host.data_ptr()),
+                                              int(parity), n))
+        return out_host
+
+    def cg_host(self, x_host: torch.Tensor, b_host: torch.Tensor, mass: float, tol: float, strict: bool = True):
+        n = b_host.shape[0]
+        for t in (x_host, b_host):
+            if t.is_cuda or not t.is_contiguous() or t.dtype != self.cdtype or tuple(t.shape) != (n, self.Vh, 3):
+                raise ValueError("expected contiguous CPU tensors [nrhs, Vh, 3]")
+        code = self.lib.hisq_cg_host(self._h, ctypes.c_void_p(x_host.data_ptr()), ctypes.c_void_p(b_host.data_ptr()),
+                                     float(mass), float(tol), n)
+        self._check(code, allow=() if strict else (HISQ_ENOCONV, HISQ_EBREAKDOWN))
+        return x_host, self.info(n, code)
+
+    def launch_count(self) -> int:
+        return int(self.lib.hisq_launch_count(self._h))
+
+    def tiles(self, nrhs: int):
+        out = (ctypes.c_int * 2)()
+        self._check(self.lib.hisq_debug_tiles(self._h, nrhs, out))
+        return out[0], out[1]
+
+
+# ---- seeded inputs in the layouts the C ABI takes (wraps inputs.py + layout.py; no method arithmetic) -----
+def make_links(L, seed: int, device, cdtype=torch.complex128, gen_device=None):
+    """(fat, naik) canonical [4, V, 3, 3] on `device`, generated on `gen_device` (default: CPU so the
+    numbers are bit-identical to what the oracle's tests see)."""
+    from . import inputs
+    gdev = torch.device(gen_device) if gen_device is not None else torch.device("cpu")
+    sites = layout.lex_of_eo(L, device=gdev)
+    fat = inputs.fat_links(L, seed, sites).permute(1, 0, 2, 3).to(cdtype).contiguous().to(device)
+    naik = inputs.naik_links(L, seed, sites).permute(1, 0, 2, 3).to(cdtype).contiguous().to(device)
+    return fat, naik
+
+
+def make_sources(L, seed: int, nrhs: int, parity: int, device, cdtype=torch.complex128, gen_device=None):
+    """Gaussian sources on one parity, canonical [nrhs, Vh, 3]."""
+    from . import inputs
+    gdev = torch.device(gen_device) if gen_device is not None else torch.device("cpu")
+    Vh = layout.volume(L) // 2
+    sites = layout.lex_of_eo(L, device=gdev)[parity * Vh:(parity + 1) * Vh]
+    return inputs.sources(L, seed, sites, nrhs).to(cdtype).contiguous().to(device)

@@ -1,0 +1,272 @@
+// blas.cuh -- fused BLAS-1 kernels of the multi-RHS CG (rows a6-a8 of SURVEY.md section 8).
+// Per right-hand side k the scalars alpha_k, beta_k are independent ("solves A x_k = b_k
+// with multiple input vectors b_k"); they live in CgState on the device and are derived in each
+// kernel's prologue, so the host never sits between two kernels of an iteration.
+// Sums are accumulated in fp64 whatever the field precision and reduced in a fixed order.
+//
+// Fields are NATIVE half-lattice arrays: RHS k is the contiguous block [k*nreal, (k+1)*nreal) of reals,
+// nreal = 6*Vh.  Grid: blockIdx.y = k, blockIdx.x over 16-byte vectors of that block.
+#pragma once
+#include "common.cuh"
+
+namespace hisq {
+
+constexpr int kBlasBlock = 256;
+constexpr int kBlasItems = 4;  // 16-byte vectors per thread
+
+template <typename T> struct V16;
+template <> struct V16<double> { using type = double2; static constexpr int n = 2; };
+template <> struct V16<float> { using type = float4; static constexpr int n = 4; };
+
+template <typename T> __device__ __forceinline__ void unpack16(const typename V16<T>::type& w, T* e);
+template <> __device__ __forceinline__ void unpack16<double>(const double2& w, double* e) { e[0] = w.x; e[1] = w.y; }
+template <> __device__ __forceinline__ void unpack16<float>(const float4& w, float* e) { e[0] = w.x; e[1] = w.y; e[2] = w.z; e[3] = w.w; }
+template <typename T> __device__ __forceinline__ typename V16<T>::type pack16(const T* e);
+template <> __device__ __forceinline__ double2 pack16<double>(const double* e) { return make_double2(e[0], e[1]); }
+template <> __device__ __forceinline__ float4 pack16<float>(const float* e) { return make_float4(e[0], e[1], e[2], e[3]); }
+
+inline int blas_grid_x(size_t nreal, int vec_n) {
+    size_t nvec = nreal / vec_n;
+    return (int)((nvec + (size_t)kBlasBlock * kBlasItems - 1) / ((size_t)kBlasBlock * kBlasItems));
+}
+
+// ---- start of a solve: r = b (rounded to T), rho = ||b||^2 in fp64, state reset ---------------------
+template <typename TB, typename T>
+__global__ void __launch_bounds__(kBlasBlock) cg_init_kernel(const TB* __restrict__ b, T* __restrict__ r, size_t nreal,
+                                                             CgState* st, double* partial, double tol, int max_iter)
+{
+    const int k = blockIdx.y;
+    const size_t base = (size_t)k * nreal;
+    double sum[1] = { 0.0 };
+    for (int it = 0; it < kBlasItems * 4; ++it) {
+        size_t i = ((size_t)blockIdx.x * kBlasItems * 4 + it) * kBlasBlock + threadIdx.x;
+        if (i < nreal) {
+            TB v = b[base + i];
+            r[base + i] = (T)v;
+            sum[0] += (double)v * (double)v;
+        }
+    }
+    __shared__ double totals[kMaxNrhs];
+    const int ncols = gridDim.x;
+    if (grid_reduce<1, kBlasBlock>(sum, k, partial, ncols, blockIdx.x, &st->ticket[0], gridDim.x * gridDim.y, gridDim.y, totals)) {
+        const int n = gridDim.y;
+        if (threadIdx.x < n) {
+            const int kk = threadIdx.x;
+            const double bb = totals[kk];
+            st->rho[kk] = bb; st->rho_prev[kk] = bb; st->bnorm2[kk] = bb;
+            st->pq[kk] = 1.0; st->beta[kk] = 0.0; st->sums[kk] = 0.0;
+            st->active[kk] = bb > 0.0 ? 1 : 0;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int any = 0;
+            for (int kk = 0; kk < n; ++kk) any |= st->active[kk];
+            st->tol2 = tol * tol; st->iter = 0; st->max_iter = max_iter; st->breakdown = 0; st->nrhs = n;
+            st->done = any ? 0 : 1;
+        }
+    }
+}
+inline int init_grid_x(size_t nreal) { return (int)((nreal + (size_t)kBlasBlock * kBlasItems * 4 - 1) / ((size_t)kBlasBlock * kBlasItems * 4)); }
+
+// ---- p_k = r_k + beta_k p_k  (first kernel of an iteration; beta = 0 at the start gives p = r) -------
+template <typename T>
+__global__ void __launch_bounds__(kBlasBlock) cg_update_p_kernel(T* __restrict__ p, const T* __restrict__ r, size_t nreal,
+                                                                 const CgState* st)
+{
+    if (st->done) return;
+    using V = typename V16<T>::type;
+    constexpr int N = V16<T>::n;
+    const int k = blockIdx.y;
+    if (!st->active[k]) return;  // frozen RHS keep their search direction (needed if they are resumed)
+    const T beta = (T)st->beta[k];
+    const size_t nvec = nreal / N;
+    V* pv = reinterpret_cast<V*>(p + (size_t)k * nreal);
+    const V* rv = reinterpret_cast<const V*>(r + (size_t)k * nreal);
+    V rr[kBlasItems], pp[kBlasItems];
+#pragma unroll
+    for (int it = 0; it < kBlasItems; ++it) {
+        size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
+        if (i < nvec) { rr[it] = rv[i]; pp[it] = pv[i]; }
+    }
+#pragma unroll
+    for (int it = 0; it < kBlasItems; ++it) {
+        size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
+        if (i < nvec) {
+            T a[N], b[N];
+            unpack16<T>(rr[it], a); unpack16<T>(pp[it], b);
+#pragma unroll
+            for (int e = 0; e < N; ++e) b[e] = fma(beta, b[e], a[e]);
+            pv[i] = pack16<T>(b);
+        }
+    }
+}
+
+// ---- x_k += alpha_k p_k ; r_k -= alpha_k q_k ; rho'_k = ||r_k||^2 ; last block: beta, convergence ----
+template <typename T>
+__global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict__ x, T* __restrict__ r, const T* __restrict__ p,
+                                                                  const T* __restrict__ q, size_t nreal, CgState* st,
+                                                                  double* partial)
+{
+    if (st->done) return;
+    using V = typename V16<T>::type;
+    constexpr int N = V16<T>::n;
+    const int k = blockIdx.y;
+    double alpha_d = 0.0;
+    if (st->active[k]) {
+        const double pq = st->pq[k];
+        alpha_d = (pq > 0.0 && isfinite(pq)) ? st->rho[k] / pq : 0.0;
+    }
+    const T alpha = (T)alpha_d;
+    const size_t nvec = nreal / N;
+    const size_t base = (size_t)k * nreal;
+    V* xv = reinterpret_cast<V*>(x + base);
+    V* rv = reinterpret_cast<V*>(r + base);
+    const V* pv = reinterpret_cast<const V*>(p + base);
+    const V* qv = reinterpret_cast<const V*>(q + base);
+    const bool live = st->active[k] != 0;  // frozen RHS: no traffic, but the block still joins the reduction
+    V xx[kBlasItems], rr[kBlasItems], pp[kBlasItems], qq[kBlasItems];
+#pragma unroll
+    for (int it = 0; it < kBlasItems; ++it) {
+        size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
+        if (live && i < nvec) { xx[it] = xv[i]; rr[it] = rv[i]; pp[it] = pv[i]; qq[it] = qv[i]; }
+    }
+    double sum[1] = { 0.0 };
+#pragma unroll
+    for (int it = 0; it < kBlasItems; ++it) {
+        size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
+        if (live && i < nvec) {
+            T a[N], b[N], c[N], d[N];
+            unpack16<T>(xx[it], a); unpack16<T>(rr[it], b); unpack16<T>(pp[it], c); unpack16<T>(qq[it], d);
+#pragma unroll
+            for (int e = 0; e < N; ++e) {
+                a[e] = fma(alpha, c[e], a[e]);
+                b[e] = fma(-alpha, d[e], b[e]);
+                sum[0] += (double)b[e] * (double)b[e];
+            }
+            xv[i] = pack16<T>(a);
+            rv[i] = pack16<T>(b);
+        }
+    }
+    __shared__ double totals[kMaxNrhs];
+    if (grid_reduce<1, kBlasBlock>(sum, k, partial, gridDim.x, blockIdx.x, &st->ticket[1], gridDim.x * gridDim.y, gridDim.y,
+                                   totals)) {
+        const int n = gridDim.y;
+        if (threadIdx.x < n) {
+            const int kk = threadIdx.x;
+            if (st->active[kk]) {
+                const double rn = totals[kk], pq = st->pq[kk];
+                if (!(pq > 0.0) || !isfinite(pq) || !isfinite(rn)) st->breakdown = 1;
+                st->rho_prev[kk] = st->rho[kk];
+                st->beta[kk] = rn / st->rho[kk];
+                st->rho[kk] = rn;
+                if (rn <= st->tol2 * st->bnorm2[kk]) st->active[kk] = 0;
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int any = 0;
+            for (int kk = 0; kk < n; ++kk) any |= st->active[kk];
+            const int it = st->iter + 1;
+            st->iter = it;
+            if (!any || it >= st->max_iter || st->breakdown) st->done = 1;
+        }
+    }
+}
+
+// ---- after a true-residual recomputation (sums[k] = ||b_k - A x_k||^2): reliable-update bookkeeping ---
+// rho_k = rho_true; beta_k = rho_true / rho_prev (search direction kept; frozen RHS kept
+// theirs too, see cg_update_p_kernel); `done` is re-evaluated.
+__global__ void cg_after_residual_kernel(CgState* st, double* true_rr_out)
+{
+    const int n = st->nrhs;
+    int any = 0;
+    for (int k = 0; k < n; ++k) {
+        const double rt = st->sums[k];
+        true_rr_out[k] = rt;
+        const bool conv = rt <= st->tol2 * st->bnorm2[k];
+        st->beta[k] = (!conv && st->rho_prev[k] > 0.0) ? rt / st->rho_prev[k] : 0.0;
+        st->rho[k] = rt;
+        st->active[k] = (!conv && st->bnorm2[k] > 0.0) ? 1 : 0;
+        any |= st->active[k];
+    }
+    st->done = (!any || st->iter >= st->max_iter || st->breakdown) ? 1 : 0;
+}
+
+// ---- mixed precision helpers ------------------------------------------------------------------------
+// x_hi += x_lo ; x_lo = 0
+__global__ void __launch_bounds__(kBlasBlock) acc_xhi_kernel(double* __restrict__ xhi, float* __restrict__ xlo, size_t n)
+{
+    size_t i = ((size_t)blockIdx.x * kBlasBlock + threadIdx.x) * 4;
+    if (i + 3 < n) {
+        float4 lo = *reinterpret_cast<float4*>(xlo + i);
+        double2 a = *reinterpret_cast<double2*>(xhi + i), b = *reinterpret_cast<double2*>(xhi + i + 2);
+        a.x += (double)lo.x; a.y += (double)lo.y; b.x += (double)lo.z; b.y += (double)lo.w;
+        *reinterpret_cast<double2*>(xhi + i) = a;
+        *reinterpret_cast<double2*>(xhi + i + 2) = b;
+        *reinterpret_cast<float4*>(xlo + i) = make_float4(0.f, 0.f, 0.f, 0.f);
+    } else {
+        for (; i < n; ++i) { xhi[i] += (double)xlo[i]; xlo[i] = 0.f; }
+    }
+}
+
+template <typename TS, typename TD>
+__global__ void __launch_bounds__(kBlasBlock) convert_kernel(const TS* __restrict__ src, TD* __restrict__ dst, size_t n)
+{
+    for (size_t i = (size_t)blockIdx.x * kBlasBlock + threadIdx.x; i < n; i += (size_t)gridDim.x * kBlasBlock)
+        dst[i] = (TD)src[i];
+}
+
+// ---- layout conversion: canonical (k,h,c) <-> native (k,c,h) -----------------------------------------
+template <typename T, bool TO_NATIVE>
+__global__ void __launch_bounds__(256) spinor_layout_kernel(T* __restrict__ dst, const T* __restrict__ src, int Vh, int nrhs)
+{
+    using C = typename Vec<T>::c1;
+    const C* s = reinterpret_cast<const C*>(src);
+    C* d = reinterpret_cast<C*>(dst);
+    const size_t total = (size_t)nrhs * 3 * Vh;
+    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < total; i += (size_t)gridDim.x * 256) {
+        // i enumerates the NATIVE order (k, c, h): coalesced on the native side
+        const int h = (int)(i % Vh);
+        const size_t kc = i / Vh;
+        const int c = (int)(kc % 3);
+        const size_t k = kc / 3;
+        const size_t j = (k * Vh + h) * 3 + c;  // canonical
+        if (TO_NATIVE) d[i] = s[j];
+        else d[j] = s[i];
+    }
+}
+
+// ---- link repack: canonical Eq. (5) [mu][eo][3][3] complex of TS -> internal planes of TD ------------
+// one thread per (mu, eo); dst block (f fixed by caller, parity, mu).
+template <typename TS, typename TD>
+__global__ void __launch_bounds__(256) link_repack_kernel(const TS* __restrict__ src, TD* __restrict__ dst_field, int Vh)
+{
+    const size_t V = (size_t)2 * Vh;
+    const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (idx >= 4 * V) return;
+    const int mu = (int)(idx / V);
+    const size_t eo = idx % V;
+    const int par = eo >= (size_t)Vh ? 1 : 0;
+    const int h = (int)(eo - (size_t)par * Vh);
+    const TS* s = src + idx * 18;
+    TD* blk = dst_field + (size_t)(par * 4 + mu) * ((size_t)Vh * 18);
+    TD e[18];
+#pragma unroll
+    for (int i = 0; i < 18; ++i) e[i] = (TD)s[i];
+    if (sizeof(TD) == 8) {
+#pragma unroll
+        for (int c = 0; c < 9; ++c) {
+            blk[((size_t)c * Vh + h) * 2] = e[2 * c];
+            blk[((size_t)c * Vh + h) * 2 + 1] = e[2 * c + 1];
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) blk[((size_t)j * Vh + h) * 4 + i] = e[4 * j + i];
+        blk[(size_t)16 * Vh + (size_t)h * 2] = e[16];
+        blk[(size_t)16 * Vh + (size_t)h * 2 + 1] = e[17];
+    }
+}
+
+}  // namespace hisq

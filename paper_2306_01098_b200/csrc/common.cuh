@@ -1,0 +1,111 @@
+// common.cuh -- shared device helpers of libhisq (sm_100a).  Product code; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace hisq {
+
+constexpr int kMaxNrhs = 16;
+
+// ---- 16-byte / 8-byte vector types per precision -------------------------------------------------
+template <typename T> struct Vec;
+template <> struct Vec<double> { using c1 = double2; };             // one complex
+template <> struct Vec<float>  { using c1 = float2; using c2 = float4; };  // one / two complex
+
+// ---- global loads with cache hints ---------------------------------------------------------------
+// Links are read exactly once per Dslash application (every link is used forward by its
+// own site and backward by the site it points to), so they stream: no L1 allocation, evict-first.
+__device__ __forceinline__ double2 ld_stream(const double2* p) { return __ldcs(p); }
+__device__ __forceinline__ float4 ld_stream(const float4* p) { return __ldcs(p); }
+__device__ __forceinline__ float2 ld_stream(const float2* p) { return __ldcs(p); }
+// Colour vectors are gathered by 16 different output sites: keep them in L1/L2.
+__device__ __forceinline__ double2 ld_keep(const double2* p) { return __ldg(p); }
+__device__ __forceinline__ float2 ld_keep(const float2* p) { return __ldg(p); }
+__device__ __forceinline__ float4 ld_keep(const float4* p) { return __ldg(p); }
+
+// ---- lattice geometry handed to kernels ----------------------------------------------------------
+struct Geom {
+    int L[4];       // Lx, Ly, Lz, Lt
+    int H;          // Lx / 2 : sites of one parity in an x-row
+    int Vh;         // sites of one parity
+    int sy, sz, st; // half-index strides of a unit step in y, z, t: H, H*Ly, H*Ly*Lz
+    // CTA sweep order: the lattice is cut into (tile_y x tile_z) columns in
+    // (y,z); inside a column work runs x fastest, then y, then z, then t; columns are swept last.
+    int ty, tz;     // tile extents in y and z (divide Ly, Lz)
+    int nty, ntz;   // number of tiles
+};
+
+// ---- device-side state of one CG solve (all scalars stay on the GPU) -------------
+struct CgState {
+    double rho[kMaxNrhs];      // ||r_k||^2 (recursive)
+    double rho_prev[kMaxNrhs]; // rho before the last update (for beta after a reliable update)
+    double pq[kMaxNrhs];       // Re<p_k, A p_k>
+    double beta[kMaxNrhs];
+    double bnorm2[kMaxNrhs];   // ||b_k||^2
+    double sums[kMaxNrhs];     // scratch result of stand-alone reductions
+    double tol2;               // tol^2
+    int active[kMaxNrhs];      // 1 while RHS k still iterates
+    int iter;
+    int max_iter;
+    int done;                  // 1: every RHS converged (tentatively) or max_iter hit -> kernels return at once
+    int breakdown;
+    int nrhs;
+    unsigned ticket[4];        // last-block tickets of the reducing kernels
+};
+
+// ---- deterministic two-stage reduction: block partials, then the last block to finish sums them ---
+// vals[NR] are this thread's contributions to right-hand sides k0 .. k0+NR-1.  partial is
+// [nrhs_total][ncols]; this block owns column `col` of rows k0..k0+NR-1.  Returns true in the LAST of
+// `total_blocks` blocks to arrive, where totals[k], k < nrhs_total (shared memory) then hold the grid
+// sums.  Fixed summation order: run-to-run reproducible (no floating-point atomics).
+template <int NR, int BLOCK>
+__device__ __forceinline__ bool grid_reduce(const double (&vals)[NR], int k0, double* __restrict__ partial, int ncols,
+                                            int col, unsigned* ticket, unsigned total_blocks, int nrhs_total,
+                                            double* totals /* shared, kMaxNrhs */)
+{
+    constexpr int NW = BLOCK / 32;
+    __shared__ double s_warp[NW * (NR > 1 ? NR : 1)];
+    __shared__ bool s_last;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NR; ++k) {
+        double v = vals[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) s_warp[k * NW + warp] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < NR; ++k) {
+            double s = 0.0;
+            for (int w = 0; w < NW; ++w) s += s_warp[k * NW + w];
+            partial[(size_t)(k0 + k) * ncols + col] = s;
+        }
+        __threadfence();
+        unsigned t = atomicAdd(ticket, 1u);
+        s_last = (t == total_blocks - 1u);
+    }
+    __syncthreads();
+    if (!s_last) return false;
+    __threadfence();
+    for (int k = 0; k < nrhs_total; ++k) {
+        double s = 0.0;
+        for (int i = threadIdx.x; i < ncols; i += BLOCK) s += __ldcg(partial + (size_t)k * ncols + i);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        __syncthreads();
+        if (lane == 0) s_warp[warp] = s;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double tot = 0.0;
+            for (int w = 0; w < NW; ++w) tot += s_warp[w];
+            totals[k] = tot;
+        }
+    }
+    if (threadIdx.x == 0) *ticket = 0u;
+    __syncthreads();
+    return true;
+}
+
+}  // namespace hisq

@@ -1,0 +1,255 @@
+// dslash.cuh -- the even-odd HISQ Dslash kernel for sm_100a (rows a2-a5 of SURVEY.md section 8).
+//
+//   out(x) = sum_mu [ X_mu(x) in(x+mu) - X_mu(x-mu)^+ in(x-mu) + W_mu(x) in(x+3mu) - W_mu(x-3mu)^+ in(x-3mu) ]
+//
+// One thread owns one output site and NR right-hand sides: each of the 16 links is loaded once into
+// registers with 128-bit streaming loads and applied to all NR gathered colour vectors
+// ("inner loop over N_inner RHS vectors inside each thread").  More right-hand sides
+// than NR are spread over CTAs that run back to back (the paper's N_outer, reuse through L2).
+// Neighbour indices and the antiperiodic-t sign are computed arithmetically from the
+// site coordinates: no index tables, no ghost cells.  HBM-bound by design; no tensor cores (3x3 complex
+// blocks are not a dense contraction).
+//
+// Internal link layout (written once by hisq_set_links): for field f (0 = fat, 1 = Naik), parity p of
+// the site that OWNS the link, and direction mu, one block of Vh*18 reals laid out as planes of
+// 16-byte chunks:   fp64: 9 planes of double2 (chunk c = complex entry 3*row+col)
+//                   fp32: 4 planes of float4 (entries 2j, 2j+1) followed by 1 plane of float2 (entry 8)
+// so a warp reading one chunk of 32 consecutive sites reads 512 contiguous bytes.
+// Native field layout: (k, c, h) at ((k*3 + c)*Vh + h) complex (include/hisq.h).
+#pragma once
+#include "common.cuh"
+
+namespace hisq {
+
+enum { MODE_PLAIN = 0,    // out = D in
+       MODE_APPLY_A = 1,  // out = m2*u - D in            and  result[k] = Re<u_k, out_k>     (u = p)
+       MODE_RESID = 2 };  // out = v - (m2*u - D in)      and  result[k] = ||out_k||^2        (u = x, v = b)
+
+template <typename T> struct DslashArgs {
+    Geom g;
+    const T* links;      // internal layout, this precision
+    const T* in;         // native, parity 1-par, first RHS of this launch
+    T* out;              // native, parity par
+    const T* u;          // epilogue operands, native, parity par (MODE 1, 2)
+    const T* v;
+    double* partial;     // [nrhs_total][ncols]
+    unsigned* ticket;
+    double* result;      // [nrhs_total], written by the last block
+    const int* done;     // if non-null and *done != 0 the kernel returns immediately
+    double m2;
+    int par;             // parity of the output sites
+    int k0;              // global index of the first RHS of this launch (rows of `partial`)
+    int nrhs_total;
+    int nchunks;         // RHS chunks of NR handled by this launch (consecutive CTAs)
+    int slab_blocks;     // CTAs per (tile, t) slab and chunk
+    unsigned total_blocks; // CTAs of the whole launch group (epilogue ticket)
+};
+
+template <typename T> __host__ __device__ constexpr size_t link_block_reals(int Vh) { return (size_t)Vh * 18; }
+
+// block of (field f, owner parity p, direction mu)
+template <typename T>
+__device__ __forceinline__ const T* link_block(const T* links, int Vh, int f, int p, int mu)
+{
+    return links + (size_t)((f * 2 + p) * 4 + mu) * ((size_t)Vh * 18);
+}
+
+__device__ __forceinline__ void load_link(const double* blk, int Vh, int h, double (&U)[18])
+{
+    const double2* p = reinterpret_cast<const double2*>(blk) + h;
+#pragma unroll
+    for (int c = 0; c < 9; ++c) {
+        double2 w = ld_stream(p + (size_t)c * Vh);
+        U[2 * c] = w.x;
+        U[2 * c + 1] = w.y;
+    }
+}
+
+__device__ __forceinline__ void load_link(const float* blk, int Vh, int h, float (&U)[18])
+{
+    const float4* p4 = reinterpret_cast<const float4*>(blk) + h;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        float4 w = ld_stream(p4 + (size_t)j * Vh);
+        U[4 * j] = w.x; U[4 * j + 1] = w.y; U[4 * j + 2] = w.z; U[4 * j + 3] = w.w;
+    }
+    float2 w = ld_stream(reinterpret_cast<const float2*>(blk + (size_t)16 * Vh) + h);
+    U[16] = w.x; U[17] = w.y;
+}
+
+template <typename T>
+__device__ __forceinline__ void load_vec(const T* field, int Vh, int h, T (&v)[6])
+{
+    using C = typename Vec<T>::c1;
+    const C* p = reinterpret_cast<const C*>(field) + h;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        C w = ld_keep(p + (size_t)c * Vh);
+        v[2 * c] = w.x;
+        v[2 * c + 1] = w.y;
+    }
+}
+
+// acc += U v
+template <typename T> __device__ __forceinline__ void mv_acc(const T (&U)[18], const T (&v)[6], T (&acc)[6])
+{
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const T ur = U[2 * (3 * a + b)], ui = U[2 * (3 * a + b) + 1];
+            acc[2 * a] = fma(ur, v[2 * b], acc[2 * a]);
+            acc[2 * a] = fma(-ui, v[2 * b + 1], acc[2 * a]);
+            acc[2 * a + 1] = fma(ur, v[2 * b + 1], acc[2 * a + 1]);
+            acc[2 * a + 1] = fma(ui, v[2 * b], acc[2 * a + 1]);
+        }
+}
+
+// acc += U^dagger v       ((U^+)_ab = conj(U_ba))
+template <typename T> __device__ __forceinline__ void mvdag_acc(const T (&U)[18], const T (&v)[6], T (&acc)[6])
+{
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) {
+            const T ur = U[2 * (3 * b + a)], ui = U[2 * (3 * b + a) + 1];
+            acc[2 * a] = fma(ur, v[2 * b], acc[2 * a]);
+            acc[2 * a] = fma(ui, v[2 * b + 1], acc[2 * a]);
+            acc[2 * a + 1] = fma(ur, v[2 * b + 1], acc[2 * a + 1]);
+            acc[2 * a + 1] = fma(-ui, v[2 * b], acc[2 * a + 1]);
+        }
+}
+
+// One of the 16 stencil terms for all NR right-hand sides.
+//   FWD:  acc += s * F_mu(x) in(x + hop mu)          link owned by the output site (index h, parity par)
+//   !FWD: acc -= s * F_mu(x - hop mu)^+ in(x - hop mu) link owned by the neighbour (index hn, parity 1-par)
+// s = -1 iff the hop crossed the t boundary (`flip`).
+template <typename T, int NR, bool FWD>
+__device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, int Vh, int hn, bool flip,
+                                             T (&acc)[NR][6])
+{
+    T U[18];
+    load_link(blk, Vh, hl, U);
+    T v[NR][6];
+#pragma unroll
+    for (int k = 0; k < NR; ++k) load_vec(in + (size_t)k * 3 * 2 * Vh, Vh, hn, v[k]);
+    const bool neg = FWD ? flip : !flip;
+#pragma unroll
+    for (int k = 0; k < NR; ++k) {
+        if (neg) {
+#pragma unroll
+            for (int i = 0; i < 6; ++i) v[k][i] = -v[k][i];
+        }
+        if (FWD) mv_acc(U, v[k], acc[k]);
+        else mvdag_acc(U, v[k], acc[k]);
+    }
+}
+
+template <typename T, int NR, int MODE, int BLOCK>
+__global__ void __launch_bounds__(BLOCK) dslash_kernel(const DslashArgs<T> a)
+{
+    if (a.done != nullptr && *a.done != 0) return;
+    const Geom& g = a.g;
+    const int Vh = g.Vh, H = g.H;
+    const int chunk = blockIdx.x % a.nchunks;
+    const int sc = blockIdx.x / a.nchunks;
+    const int t = blockIdx.y;
+    const int tile = blockIdx.z;
+    const int l = sc * BLOCK + threadIdx.x;
+    const bool valid = l < H * g.ty * g.tz;
+
+    T acc[NR][6];
+#pragma unroll
+    for (int k = 0; k < NR; ++k)
+#pragma unroll
+        for (int i = 0; i < 6; ++i) acc[k][i] = T(0);
+
+    int h = 0;
+    const size_t rhs_stride = (size_t)3 * 2 * Vh;  // reals per RHS
+    const T* in = a.in + (size_t)chunk * NR * rhs_stride;
+    if (valid) {
+        const int xh = l % H;
+        const int q = l / H;
+        const int yy = q % g.ty, zz = q / g.ty;
+        const int y = (tile % g.nty) * g.ty + yy;
+        const int z = (tile / g.nty) * g.tz + zz;
+        const int par = a.par;
+        const int x = 2 * xh + ((par + y + z + t) & 1);
+        h = xh + H * (y + g.L[1] * (z + g.L[2] * t));
+        const int row = h - xh;
+        const int c[4] = { x, y, z, t };
+        const int stride[4] = { 0, g.sy, g.sz, g.st };
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) {
+#pragma unroll
+            for (int f = 0; f < 2; ++f) {
+                const int hop = f ? 3 : 1;
+                const int Lmu = g.L[mu];
+                int cp = c[mu] + hop;
+                const bool wp = cp >= Lmu;
+                cp -= wp ? Lmu : 0;
+                int cm = c[mu] - hop;
+                const bool wm = cm < 0;
+                cm += wm ? Lmu : 0;
+                int hp, hm;
+                if (mu == 0) { hp = row + (cp >> 1); hm = row + (cm >> 1); }
+                else { hp = h + (cp - c[mu]) * stride[mu]; hm = h + (cm - c[mu]) * stride[mu]; }
+                stencil_term<T, NR, true>(link_block(a.links, Vh, f, par, mu), h, in, Vh, hp, mu == 3 && wp, acc);
+                stencil_term<T, NR, false>(link_block(a.links, Vh, f, 1 - par, mu), hm, in, Vh, hm, mu == 3 && wm, acc);
+            }
+        }
+    }
+
+    using C = typename Vec<T>::c1;
+    const int kg0 = a.k0 + chunk * NR;  // global index of this thread's first RHS
+    double red[NR];
+#pragma unroll
+    for (int k = 0; k < NR; ++k) red[k] = 0.0;
+    if (valid) {
+        C* out = reinterpret_cast<C*>(a.out + (size_t)chunk * NR * rhs_stride) + h;
+#pragma unroll
+        for (int k = 0; k < NR; ++k) {
+            T o[6];
+            if (MODE == MODE_PLAIN) {
+#pragma unroll
+                for (int i = 0; i < 6; ++i) o[i] = acc[k][i];
+            } else {
+                T uu[6];
+                load_vec(a.u + (size_t)(chunk * NR + k) * rhs_stride, Vh, h, uu);
+                const T m2 = (T)a.m2;
+                if (MODE == MODE_APPLY_A) {
+#pragma unroll
+                    for (int i = 0; i < 6; ++i) {
+                        o[i] = fma(m2, uu[i], -acc[k][i]);
+                        red[k] += (double)uu[i] * (double)o[i];
+                    }
+                } else {
+                    T vv[6];
+                    load_vec(a.v + (size_t)(chunk * NR + k) * rhs_stride, Vh, h, vv);
+#pragma unroll
+                    for (int i = 0; i < 6; ++i) {
+                        o[i] = vv[i] - fma(m2, uu[i], -acc[k][i]);
+                        red[k] += (double)o[i] * (double)o[i];
+                    }
+                }
+            }
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) {
+                C w;
+                w.x = o[2 * cc];
+                w.y = o[2 * cc + 1];
+                out[(size_t)(k * 3 + cc) * Vh] = w;
+            }
+        }
+    }
+    if (MODE != MODE_PLAIN) {
+        __shared__ double totals[kMaxNrhs];
+        const int col = sc + a.slab_blocks * (t + g.L[3] * tile);
+        const int ncols = a.slab_blocks * g.L[3] * g.nty * g.ntz;
+        if (grid_reduce<NR, BLOCK>(red, kg0, a.partial, ncols, col, a.ticket, a.total_blocks, a.nrhs_total, totals)) {
+            if (threadIdx.x < a.nrhs_total) a.result[threadIdx.x] = totals[threadIdx.x];
+        }
+    }
+}
+
+}  // namespace hisq

@@ -1,0 +1,556 @@
+// hisq.cu -- the C ABI of libhisq (include/hisq.h): context, workspace, link repack, Dslash dispatch,
+// multi-RHS CG drivers (fp32 / fp64 / mixed with fp64 reliable updates).  sm_100a only; no CPU path.
+#include "../../include/hisq.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "blas.cuh"
+#include "dslash_launch.cuh"
+
+using namespace hisq;
+
+struct hisq_ctx {
+    Geom g;
+    int prec;
+    cudaStream_t stream;
+    // workspace carve-up (all device pointers into the caller's buffer)
+    char* ws;
+    size_t ws_bytes;
+    int ws_nrhs;           // RHS capacity of the CG / staging part
+    double* links64;       // internal fp64 links (FP64, MIXED)
+    float* links32;        // internal fp32 links (FP32, MIXED)
+    CgState* state;
+    double* partial;       // reduction partials [kMaxNrhs][partial_cols]
+    double* true_rr;       // [kMaxNrhs] device
+    size_t partial_cols;
+    char* fields;          // CG temporaries
+    char* stage;           // host-call staging (2 canonical + 2 native fields)
+    bool have_links;
+    // options
+    int max_iter, reliable_interval, check_interval, use_graph, nrhs_inner, tile_y, tile_z;
+    double window_mb;
+    // info of the last solve
+    int info_iters, info_reliable;
+    double info_relres[kMaxNrhs];
+    LaunchStats stats;
+    CgState* host_state;   // pinned
+    std::string last_error;
+};
+
+static size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+static size_t elem_size(int prec) { return prec == HISQ_FP32 ? 4 : 8; }
+
+static int cuda_fail(hisq_ctx* h, cudaError_t e, const char* where)
+{
+    h->last_error = std::string(where) + ": " + cudaGetErrorString(e);
+    return HISQ_ECUDA;
+}
+#define CK(call)                                                      \
+    do {                                                              \
+        cudaError_t e_ = (call);                                      \
+        if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);        \
+    } while (0)
+
+// ---- CTA sweep order: (ty, tz) so that the 7 t-slices an in-flight output slice gathers from fit in L2 ----
+static void choose_tiles(hisq_ctx* h, int nrhs, size_t w)
+{
+    Geom& g = h->g;
+    int ty = g.L[1], tz = g.L[2];
+    if (h->tile_y > 0 && g.L[1] % h->tile_y == 0) ty = h->tile_y;
+    if (h->tile_z > 0 && g.L[2] % h->tile_z == 0) tz = h->tile_z;
+    if (h->tile_y <= 0 && h->tile_z <= 0) {
+        const double target = h->window_mb * 1e6;
+        const double per_site = 6.0 * nrhs * (double)w;
+        double best_cost = 1e300;
+        for (int cy = 4; cy <= g.L[1]; ++cy) {
+            if (g.L[1] % cy) continue;
+            for (int cz = 4; cz <= g.L[2]; ++cz) {
+                if (g.L[2] % cz) continue;
+                const double window = 7.0 * g.H * cy * cz * per_site;
+                const double halo = (cy == g.L[1] ? 1.0 : (cy + 6.0) / cy) * (cz == g.L[2] ? 1.0 : (cz + 6.0) / cz);
+                double cost = halo + (window > target ? 100.0 * window / target : 0.0) - 1e-9 * cy * cz;
+                if (cost < best_cost) { best_cost = cost; ty = cy; tz = cz; }
+            }
+        }
+    }
+    g.ty = ty; g.tz = tz; g.nty = g.L[1] / ty; g.ntz = g.L[2] / tz;
+}
+
+extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int prec)
+{
+    if (!out) return HISQ_EINVAL;
+    *out = nullptr;
+    const int L[4] = { Lx, Ly, Lz, Lt };
+    for (int i = 0; i < 4; ++i)
+        if (L[i] < 4 || (L[i] & 1)) return HISQ_EINVAL;
+    if (prec != HISQ_FP32 && prec != HISQ_FP64 && prec != HISQ_MIXED) return HISQ_EINVAL;
+    const long long V = (long long)Lx * Ly * Lz * Lt;
+    if (V / 2 > 0x3fffffffLL) return HISQ_EINVAL;  // half-index must fit comfortably in int
+    hisq_ctx* h = new (std::nothrow) hisq_ctx();
+    if (!h) return HISQ_EINVAL;
+    for (int i = 0; i < 4; ++i) h->g.L[i] = L[i];
+    h->g.H = Lx / 2;
+    h->g.Vh = (int)(V / 2);
+    h->g.sy = h->g.H; h->g.sz = h->g.H * Ly; h->g.st = h->g.H * Ly * Lz;
+    h->g.ty = Ly; h->g.tz = Lz; h->g.nty = 1; h->g.ntz = 1;
+    h->prec = prec;
+    h->stream = 0;
+    h->ws = nullptr; h->ws_bytes = 0; h->ws_nrhs = 0;
+    h->links64 = nullptr; h->links32 = nullptr; h->have_links = false;
+    h->max_iter = 100000;
+    h->reliable_interval = prec == HISQ_MIXED ? 100 : 0;
+    h->check_interval = 32;
+    h->use_graph = 1;
+    h->nrhs_inner = 0;
+    h->tile_y = 0; h->tile_z = 0;
+    h->window_mb = 40.0;
+    h->info_iters = 0; h->info_reliable = 0;
+    for (int k = 0; k < kMaxNrhs; ++k) h->info_relres[k] = 0.0;
+    h->host_state = nullptr;
+    if (cudaHostAlloc((void**)&h->host_state, sizeof(CgState) + kMaxNrhs * sizeof(double), cudaHostAllocDefault) != cudaSuccess) {
+        delete h;
+        return HISQ_ECUDA;
+    }
+    *out = h;
+    return HISQ_OK;
+}
+
+extern "C" int hisq_destroy(hisq_ctx* h)
+{
+    if (!h) return HISQ_EINVAL;
+    if (h->host_state) cudaFreeHost(h->host_state);
+    delete h;
+    return HISQ_OK;
+}
+
+extern "C" int hisq_set_stream(hisq_ctx* h, void* s)
+{
+    if (!h) return HISQ_EINVAL;
+    h->stream = (cudaStream_t)s;
+    return HISQ_OK;
+}
+
+// ---- workspace layout ---------------------------------------------------------------------------
+struct WsLayout {
+    size_t links64, links32, state, true_rr, partial, fields, stage, total, partial_cols;
+};
+
+static size_t field_bytes(const hisq_ctx* h, int nrhs, size_t w) { return align_up((size_t)nrhs * 6 * h->g.Vh * w); }
+
+static WsLayout ws_layout(const hisq_ctx* h, int nrhs)
+{
+    WsLayout l;
+    const size_t V = (size_t)2 * h->g.Vh;
+    size_t off = 0;
+    l.links64 = off;
+    if (h->prec != HISQ_FP32) off += align_up(2 * 4 * V * 18 * 8);
+    l.links32 = off;
+    if (h->prec != HISQ_FP64) off += align_up(2 * 4 * V * 18 * 4);
+    l.state = off; off += align_up(sizeof(CgState));
+    l.true_rr = off; off += align_up(kMaxNrhs * sizeof(double));
+    // columns: enough for the Dslash epilogue (one per CTA and chunk-slot) and the BLAS kernels
+    size_t cols_d = ((size_t)h->g.Vh / 64 + (size_t)h->g.L[3] * h->g.L[1] * h->g.L[2] / 16 + 64);
+    size_t cols_b = (size_t)blas_grid_x((size_t)6 * h->g.Vh, 2) + init_grid_x((size_t)6 * h->g.Vh) + 64;
+    l.partial_cols = cols_d > cols_b ? cols_d : cols_b;
+    l.partial = off; off += align_up((size_t)kMaxNrhs * l.partial_cols * sizeof(double));
+    l.fields = off;
+    if (h->prec == HISQ_FP64) off += 4 * field_bytes(h, nrhs, 8);                            // r p q t
+    else if (h->prec == HISQ_FP32) off += 4 * field_bytes(h, nrhs, 4);
+    else off += 5 * field_bytes(h, nrhs, 4) + 2 * field_bytes(h, nrhs, 8);                   // r p q t xlo | rhi thi
+    l.stage = off;
+    off += 4 * field_bytes(h, nrhs, elem_size(h->prec));
+    l.total = off;
+    return l;
+}
+
+extern "C" size_t hisq_workspace_bytes(const hisq_ctx* h, int nrhs)
+{
+    if (!h || nrhs < 1 || nrhs > HISQ_MAX_NRHS) return 0;
+    return ws_layout(h, nrhs).total;
+}
+
+extern "C" int hisq_set_workspace(hisq_ctx* h, void* p, size_t bytes)
+{
+    if (!h || !p || ((uintptr_t)p & 255)) return HISQ_EINVAL;
+    int nrhs = 0;
+    for (int n = HISQ_MAX_NRHS; n >= 1; --n)
+        if (ws_layout(h, n).total <= bytes) { nrhs = n; break; }
+    if (nrhs == 0) return HISQ_ENOWORKSPACE;
+    WsLayout l = ws_layout(h, nrhs);
+    h->ws = (char*)p; h->ws_bytes = bytes; h->ws_nrhs = nrhs;
+    h->links64 = h->prec != HISQ_FP32 ? (double*)(h->ws + l.links64) : nullptr;
+    h->links32 = h->prec != HISQ_FP64 ? (float*)(h->ws + l.links32) : nullptr;
+    h->state = (CgState*)(h->ws + l.state);
+    h->true_rr = (double*)(h->ws + l.true_rr);
+    h->partial = (double*)(h->ws + l.partial);
+    h->partial_cols = l.partial_cols;
+    h->fields = h->ws + l.fields;
+    h->stage = h->ws + l.stage;
+    h->have_links = false;
+    CK(cudaMemsetAsync(h->state, 0, sizeof(CgState), h->stream));
+    return HISQ_OK;
+}
+
+extern "C" int hisq_set_links(hisq_ctx* h, const void* fat, const void* naik)
+{
+    if (!h || !fat || !naik || ((uintptr_t)fat & 15) || ((uintptr_t)naik & 15)) return HISQ_EINVAL;
+    if (!h->ws) return HISQ_ENOWORKSPACE;
+    const int Vh = h->g.Vh;
+    const size_t V = (size_t)2 * Vh;
+    const unsigned grid = (unsigned)((4 * V + 255) / 256);
+    const size_t fstride = (size_t)8 * Vh * 18;  // reals per field (2 parities x 4 directions)
+    const void* src[2] = { fat, naik };
+    for (int f = 0; f < 2; ++f) {
+        if (h->prec == HISQ_FP32) {
+            link_repack_kernel<float, float><<<grid, 256, 0, h->stream>>>((const float*)src[f], h->links32 + f * fstride, Vh);
+        } else {
+            link_repack_kernel<double, double><<<grid, 256, 0, h->stream>>>((const double*)src[f], h->links64 + f * fstride, Vh);
+            if (h->prec == HISQ_MIXED)
+                link_repack_kernel<double, float><<<grid, 256, 0, h->stream>>>((const double*)src[f], h->links32 + f * fstride, Vh);
+        }
+        h->stats.launches += (h->prec == HISQ_MIXED) ? 2 : 1;
+    }
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(h->stream));
+    h->have_links = true;
+    return HISQ_OK;
+}
+
+// ---- Dslash dispatch -----------------------------------------------------------------------------
+static int default_inner_cap(int prec_bytes) { return prec_bytes == 4 ? 8 : 4; }
+
+template <typename T>
+static int run_dslash(hisq_ctx* h, const T* links, T* out, const T* in, int parity, int nrhs, int mode, const T* u,
+                      const T* v, double m2, double* result, const int* done, int ticket_slot)
+{
+    choose_tiles(h, nrhs, sizeof(T));
+    DslashArgs<T> a;
+    a.g = h->g;
+    a.links = links;
+    a.in = in; a.out = out; a.u = u; a.v = v;
+    a.partial = h->partial;
+    a.ticket = &h->state->ticket[ticket_slot];
+    a.result = result;
+    a.done = done;
+    a.m2 = m2;
+    a.par = parity;
+    a.k0 = 0; a.nrhs_total = nrhs; a.nchunks = 1; a.slab_blocks = 0; a.total_blocks = 0;
+    int cap = h->nrhs_inner > 0 ? h->nrhs_inner : default_inner_cap((int)sizeof(T));
+    int e = launch_dslash<T>(a, mode, nrhs, cap, h->stream, &h->stats);
+    if (e != 0) return cuda_fail(h, (cudaError_t)e, "dslash launch");
+    return HISQ_OK;
+}
+
+static bool overlap(const void* a, const void* b, size_t bytes)
+{
+    const char* x = (const char*)a; const char* y = (const char*)b;
+    return x < y + bytes && y < x + bytes;
+}
+
+extern "C" int hisq_dslash(hisq_ctx* h, void* out, const void* in, int parity, int nrhs)
+{
+    if (!h || !out || !in || nrhs < 1 || nrhs > HISQ_MAX_NRHS || (parity != 0 && parity != 1)) return HISQ_EINVAL;
+    if (((uintptr_t)out & 15) || ((uintptr_t)in & 15)) return HISQ_EINVAL;
+    if (!h->ws) return HISQ_ENOWORKSPACE;
+    if (!h->have_links) return HISQ_ENOLINKS;
+    const size_t bytes = (size_t)nrhs * 6 * h->g.Vh * elem_size(h->prec);
+    if (overlap(out, in, bytes)) return HISQ_EINVAL;
+    if (h->prec == HISQ_FP32)
+        return run_dslash<float>(h, h->links32, (float*)out, (const float*)in, parity, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0,
+                                 nullptr, nullptr, 2);
+    return run_dslash<double>(h, h->links64, (double*)out, (const double*)in, parity, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0,
+                              nullptr, nullptr, 2);
+}
+
+// ---- CG --------------------------------------------------------------------------------------------
+// One iteration (textbook Hestenes-Stiefel, independent scalars per RHS):
+//   p = r + beta p ; t = D_oe p ; q = m^2 p - D_eo t , <p,q> ; x += alpha p , r -= alpha q , rho' = ||r||^2
+template <typename T>
+static int enqueue_iteration(hisq_ctx* h, const T* links, T* x, T* r, T* p, T* q, T* t, double m2, int nrhs)
+{
+    const size_t nreal = (size_t)6 * h->g.Vh;
+    dim3 gb((unsigned)blas_grid_x(nreal, V16<T>::n), (unsigned)nrhs);
+    cg_update_p_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(p, r, nreal, h->state);
+    h->stats.launches++;
+    int rc = run_dslash<T>(h, links, t, p, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, &h->state->done, 2);
+    if (rc) return rc;
+    rc = run_dslash<T>(h, links, q, t, HISQ_EVEN, nrhs, MODE_APPLY_A, p, nullptr, m2, h->state->pq, &h->state->done, 2);
+    if (rc) return rc;
+    cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+
+// r_out = b - A x in fp64-or-T, sums[k] = ||r_out_k||^2, then reliable-update bookkeeping.
+template <typename T>
+static int enqueue_true_residual(hisq_ctx* h, const T* links, T* r_out, const T* x, const T* b, T* t, double m2, int nrhs)
+{
+    int rc = run_dslash<T>(h, links, t, x, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, nullptr, 2);
+    if (rc) return rc;
+    rc = run_dslash<T>(h, links, r_out, t, HISQ_EVEN, nrhs, MODE_RESID, x, b, m2, h->state->sums, nullptr, 2);
+    if (rc) return rc;
+    cg_after_residual_kernel<<<1, 1, 0, h->stream>>>(h->state, h->true_rr);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+
+static int poll_state(hisq_ctx* h)
+{
+    CK(cudaMemcpyAsync(h->host_state, h->state, sizeof(CgState), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaMemcpyAsync((char*)h->host_state + sizeof(CgState), h->true_rr, kMaxNrhs * sizeof(double), cudaMemcpyDeviceToHost,
+                       h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return HISQ_OK;
+}
+
+// Replay `count` iterations; with use_graph the batch is captured once and launched as one graph.
+struct IterBatch {
+    cudaGraphExec_t exec = nullptr;
+    int count = 0;
+};
+
+template <typename T, typename TB>
+static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_user, const TB* b, double mass, double tol, int nrhs)
+{
+    constexpr bool MIXED = !std::is_same<T, TB>::value;
+    const size_t nreal = (size_t)6 * h->g.Vh;
+    const size_t total = nreal * nrhs;
+    const double m2 = mass * mass;
+    const size_t fb = field_bytes(h, h->ws_nrhs, sizeof(T));
+    T* r = (T*)(h->fields);
+    T* p = (T*)(h->fields + fb);
+    T* q = (T*)(h->fields + 2 * fb);
+    T* t = (T*)(h->fields + 3 * fb);
+    T* x = MIXED ? (T*)(h->fields + 4 * fb) : (T*)x_user;
+    TB* r_hi = MIXED ? (TB*)(h->fields + 5 * fb) : (TB*)r;
+    TB* t_hi = MIXED ? (TB*)(h->fields + 5 * fb + field_bytes(h, h->ws_nrhs, sizeof(TB))) : (TB*)t;
+
+    h->info_iters = 0; h->info_reliable = 0;
+    // x = 0, p = 0, r = b, rho = ||b||^2
+    CK(cudaMemsetAsync(x_user, 0, total * sizeof(TB), h->stream));
+    if (MIXED) CK(cudaMemsetAsync(x, 0, total * sizeof(T), h->stream));
+    CK(cudaMemsetAsync(p, 0, total * sizeof(T), h->stream));
+    dim3 gi((unsigned)init_grid_x(nreal), (unsigned)nrhs);
+    cg_init_kernel<TB, T><<<gi, kBlasBlock, 0, h->stream>>>(b, r, nreal, h->state, h->partial, tol, h->max_iter);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+
+    const int R = h->reliable_interval;
+    int batch = h->check_interval > 0 ? h->check_interval : 32;
+    if (R > 0) {
+        int best = 1;
+        for (int d = 1; d <= R && d <= batch; ++d)
+            if (R % d == 0) best = d;
+        batch = best;
+    }
+    IterBatch ib;
+    int rc = HISQ_OK;
+    int status = HISQ_OK;
+    long long launches_per_batch = 0;
+    while (true) {
+        // ---- a batch of iterations ----
+        if (h->use_graph) {
+            if (!ib.exec) {
+                cudaGraph_t graph;
+                const long long l0 = h->stats.launches;
+                CK(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+                for (int i = 0; i < batch && rc == HISQ_OK; ++i) rc = enqueue_iteration<T>(h, links, x, r, p, q, t, m2, nrhs);
+                cudaError_t ce = cudaStreamEndCapture(h->stream, &graph);
+                if (rc != HISQ_OK) { if (ce == cudaSuccess) cudaGraphDestroy(graph); break; }
+                if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaStreamEndCapture"); break; }
+                ce = cudaGraphInstantiate(&ib.exec, graph, 0);
+                cudaGraphDestroy(graph);
+                if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaGraphInstantiate"); break; }
+                launches_per_batch = h->stats.launches - l0;
+                h->stats.launches = l0;
+            }
+            cudaError_t ce = cudaGraphLaunch(ib.exec, h->stream);
+            if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaGraphLaunch"); break; }
+            h->stats.launches += launches_per_batch;
+        } else {
+            for (int i = 0; i < batch && rc == HISQ_OK; ++i) rc = enqueue_iteration<T>(h, links, x, r, p, q, t, m2, nrhs);
+            if (rc != HISQ_OK) break;
+        }
+        if ((rc = poll_state(h)) != HISQ_OK) break;
+        const CgState& s = *h->host_state;
+        h->info_iters = s.iter;
+        if (s.breakdown) { status = HISQ_EBREAKDOWN; }
+        const bool at_reliable = R > 0 && s.iter > 0 && s.iter % R == 0;
+        if (!s.done && !at_reliable) continue;
+        // ---- reliable update / final check: true residual in the high precision ----
+        if (MIXED) {
+            acc_xhi_kernel<<<(unsigned)((total / 4 + kBlasBlock - 1) / kBlasBlock + 1), kBlasBlock, 0, h->stream>>>(
+                (double*)x_user, (float*)x, total);
+            h->stats.launches++;
+            rc = enqueue_true_residual<TB>(h, (const TB*)links_hi, r_hi, x_user, b, t_hi, m2, nrhs);
+            if (rc) break;
+            convert_kernel<TB, T><<<1184, kBlasBlock, 0, h->stream>>>(r_hi, r, total);
+            h->stats.launches++;
+        } else {
+            rc = enqueue_true_residual<TB>(h, (const TB*)links, (TB*)r, x_user, b, (TB*)t, m2, nrhs);
+            if (rc) break;
+        }
+        h->info_reliable++;
+        if ((rc = poll_state(h)) != HISQ_OK) break;
+        const CgState& s2 = *h->host_state;
+        const double* trr = (const double*)((const char*)h->host_state + sizeof(CgState));
+        for (int k = 0; k < nrhs; ++k)
+            h->info_relres[k] = s2.bnorm2[k] > 0.0 ? std::sqrt(trr[k] / s2.bnorm2[k]) : 0.0;
+        if (status == HISQ_EBREAKDOWN) break;
+        if (s2.done) {
+            bool all = true;
+            for (int k = 0; k < nrhs; ++k) all = all && !s2.active[k];
+            if (!all) status = HISQ_ENOCONV;
+            break;
+        }
+    }
+    if (ib.exec) cudaGraphExecDestroy(ib.exec);
+    if (rc != HISQ_OK) return rc;
+    return status;
+}
+
+extern "C" int hisq_cg(hisq_ctx* h, void* x, const void* b, double mass, double tol, int nrhs)
+{
+    if (!h || !x || !b || nrhs < 1 || nrhs > HISQ_MAX_NRHS || !(tol > 0.0) || !std::isfinite(mass)) return HISQ_EINVAL;
+    if (((uintptr_t)x & 15) || ((uintptr_t)b & 15)) return HISQ_EINVAL;
+    if (!h->ws) return HISQ_ENOWORKSPACE;
+    if (nrhs > h->ws_nrhs) return HISQ_ENOWORKSPACE;
+    if (!h->have_links) return HISQ_ENOLINKS;
+    const size_t bytes = (size_t)nrhs * 6 * h->g.Vh * elem_size(h->prec);
+    if (overlap(x, b, bytes)) return HISQ_EINVAL;
+    if (h->prec == HISQ_FP32) return cg_solve<float, float>(h, h->links32, nullptr, (float*)x, (const float*)b, mass, tol, nrhs);
+    if (h->prec == HISQ_FP64) return cg_solve<double, double>(h, h->links64, nullptr, (double*)x, (const double*)b, mass, tol, nrhs);
+    return cg_solve<float, double>(h, h->links32, h->links64, (double*)x, (const double*)b, mass, tol, nrhs);
+}
+
+// ---- options / info ----------------------------------------------------------------------------------
+extern "C" int hisq_set_option(hisq_ctx* h, const char* key, double value)
+{
+    if (!h || !key) return HISQ_EINVAL;
+    const int v = (int)value;
+    if (!strcmp(key, "max_iter")) { if (v < 1) return HISQ_EINVAL; h->max_iter = v; }
+    else if (!strcmp(key, "reliable_interval")) { if (v < 0) return HISQ_EINVAL; h->reliable_interval = v; }
+    else if (!strcmp(key, "check_interval")) { if (v < 1 || v > 1024) return HISQ_EINVAL; h->check_interval = v; }
+    else if (!strcmp(key, "use_graph")) h->use_graph = v != 0;
+    else if (!strcmp(key, "nrhs_inner")) { if (v < 0 || v > 8) return HISQ_EINVAL; h->nrhs_inner = v; }
+    else if (!strcmp(key, "tile_y")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[1] % v))) return HISQ_EINVAL; h->tile_y = v; }
+    else if (!strcmp(key, "tile_z")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[2] % v))) return HISQ_EINVAL; h->tile_z = v; }
+    else if (!strcmp(key, "window_mb")) { if (!(value > 0)) return HISQ_EINVAL; h->window_mb = value; }
+    else if (!strcmp(key, "dslash_block")) { if (v != 0 && v != kDslashBlock) return HISQ_EINVAL; }
+    else return HISQ_EINVAL;
+    return HISQ_OK;
+}
+
+extern "C" int hisq_get_info(const hisq_ctx* h, int* iterations, int* reliable_updates, double* true_rel_resid)
+{
+    if (!h) return HISQ_EINVAL;
+    if (iterations) *iterations = h->info_iters;
+    if (reliable_updates) *reliable_updates = h->info_reliable;
+    if (true_rel_resid)
+        for (int k = 0; k < kMaxNrhs && k < h->host_state->nrhs; ++k) true_rel_resid[k] = h->info_relres[k];
+    return HISQ_OK;
+}
+
+// ---- layout conversion ---------------------------------------------------------------------------------
+template <bool TO_NATIVE>
+static int convert_layout(hisq_ctx* h, void* dst, const void* src, int nrhs)
+{
+    if (!h || !dst || !src || nrhs < 1 || nrhs > HISQ_MAX_NRHS) return HISQ_EINVAL;
+    if (((uintptr_t)dst & 15) || ((uintptr_t)src & 15)) return HISQ_EINVAL;
+    const size_t total = (size_t)nrhs * 3 * h->g.Vh;
+    unsigned grid = (unsigned)((total + 255) / 256);
+    if (grid > 148 * 16) grid = 148 * 16;
+    if (h->prec == HISQ_FP32)
+        spinor_layout_kernel<float, TO_NATIVE><<<grid, 256, 0, h->stream>>>((float*)dst, (const float*)src, h->g.Vh, nrhs);
+    else
+        spinor_layout_kernel<double, TO_NATIVE><<<grid, 256, 0, h->stream>>>((double*)dst, (const double*)src, h->g.Vh, nrhs);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+
+extern "C" int hisq_spinor_pack(hisq_ctx* h, void* native, const void* canonical, int nrhs)
+{
+    return convert_layout<true>(h, native, canonical, nrhs);
+}
+extern "C" int hisq_spinor_unpack(hisq_ctx* h, void* canonical, const void* native, int nrhs)
+{
+    return convert_layout<false>(h, canonical, native, nrhs);
+}
+
+// ---- host-buffer entry points (end-to-end path: H2D, pack, run, unpack, D2H) ------------------------------
+extern "C" int hisq_dslash_host(hisq_ctx* h, void* out_host, const void* in_host, int parity, int nrhs)
+{
+    if (!h || !out_host || !in_host || nrhs < 1 || nrhs > HISQ_MAX_NRHS) return HISQ_EINVAL;
+    if (!h->ws || nrhs > h->ws_nrhs) return HISQ_ENOWORKSPACE;
+    const size_t fb = field_bytes(h, h->ws_nrhs, elem_size(h->prec));
+    const size_t bytes = (size_t)nrhs * 6 * h->g.Vh * elem_size(h->prec);
+    char *c_in = h->stage, *n_in = h->stage + fb, *n_out = h->stage + 2 * fb, *c_out = h->stage + 3 * fb;
+    CK(cudaMemcpyAsync(c_in, in_host, bytes, cudaMemcpyHostToDevice, h->stream));
+    int rc = hisq_spinor_pack(h, n_in, c_in, nrhs);
+    if (rc) return rc;
+    rc = hisq_dslash(h, n_out, n_in, parity, nrhs);
+    if (rc) return rc;
+    rc = hisq_spinor_unpack(h, c_out, n_out, nrhs);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(out_host, c_out, bytes, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return HISQ_OK;
+}
+
+extern "C" int hisq_cg_host(hisq_ctx* h, void* x_host, const void* b_host, double mass, double tol, int nrhs)
+{
+    if (!h || !x_host || !b_host || nrhs < 1 || nrhs > HISQ_MAX_NRHS) return HISQ_EINVAL;
+    if (!h->ws || nrhs > h->ws_nrhs) return HISQ_ENOWORKSPACE;
+    const size_t fb = field_bytes(h, h->ws_nrhs, elem_size(h->prec));
+    const size_t bytes = (size_t)nrhs * 6 * h->g.Vh * elem_size(h->prec);
+    char *c_in = h->stage, *n_in = h->stage + fb, *n_out = h->stage + 2 * fb, *c_out = h->stage + 3 * fb;
+    CK(cudaMemcpyAsync(c_in, b_host, bytes, cudaMemcpyHostToDevice, h->stream));
+    int rc = hisq_spinor_pack(h, n_in, c_in, nrhs);
+    if (rc) return rc;
+    const int solve_rc = hisq_cg(h, n_out, n_in, mass, tol, nrhs);
+    if (solve_rc != HISQ_OK && solve_rc != HISQ_ENOCONV && solve_rc != HISQ_EBREAKDOWN) return solve_rc;
+    rc = hisq_spinor_unpack(h, c_out, n_out, nrhs);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(x_host, c_out, bytes, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return solve_rc;
+}
+
+extern "C" long long hisq_launch_count(const hisq_ctx* h) { return h ? h->stats.launches : 0; }
+
+extern "C" const char* hisq_strerror(int code)
+{
+    switch (code) {
+    case HISQ_OK: return "success";
+    case HISQ_EINVAL: return "invalid argument";
+    case HISQ_ENOLINKS: return "links not set";
+    case HISQ_ENOWORKSPACE: return "workspace missing or too small";
+    case HISQ_ECUDA: return "CUDA error (see hisq_last_error)";
+    case HISQ_ENOCONV: return "CG did not converge within max_iter";
+    case HISQ_EBREAKDOWN: return "CG breakdown (<p,Ap> <= 0 or non-finite scalar)";
+    default: return "unknown error code";
+    }
+}
+
+extern "C" const char* hisq_last_error(const hisq_ctx* h) { return h ? h->last_error.c_str() : ""; }
+
+// introspection for tests / DESIGN.md tables: registers per thread of a Dslash instantiation
+extern "C" int hisq_debug_dslash_regs(int prec, int nr, int mode)
+{
+    return prec == HISQ_FP32 ? dslash_regs<float>(nr, mode) : dslash_regs<double>(nr, mode);
+}
+// the CTA sweep tiling the next Dslash launch with `nrhs` would use: out[0]=tile_y, out[1]=tile_z
+extern "C" int hisq_debug_tiles(hisq_ctx* h, int nrhs, int* out)
+{
+    if (!h || !out) return HISQ_EINVAL;
+    choose_tiles(h, nrhs, h->prec == HISQ_FP32 ? 4 : 8);
+    out[0] = h->g.ty; out[1] = h->g.tz;
+    return HISQ_OK;
+}

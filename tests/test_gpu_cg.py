@@ -1,0 +1,127 @@
+"""-m gpu: the CUDA multi-RHS CG (through the C ABI) against the CPU oracle's textbook CG."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from tests.gpu_helpers import make_ctx, make_field, rel_l2, to_full
+
+pytestmark = pytest.mark.gpu
+
+
+def _true_relres(L, X, W, m, x_full, b_full):
+    r = b_full - oracle.apply_A(L, X, W, m, x_full)
+    return [float(np.linalg.norm(r[k]) / np.linalg.norm(b_full[k])) for k in range(b_full.shape[0])]
+
+
+@pytest.mark.parametrize("use_graph", [1, 0])
+def test_cg_config1_8x8x8x8_fp64(use_graph):
+    """BASELINE.json configs[0]: 8^4, fp64, nRHS=1, m=0.1, tol 1e-10, seed 0."""
+    L, m, tol = (8, 8, 8, 8), 0.1, 1e-10
+    ctx, X, W = make_ctx(L, "fp64", 1, 0)
+    ctx.set_option("use_graph", use_graph)
+    b_dev, b_full = make_field(ctx, L, 0, 1, 0)
+    x_dev, info = ctx.cg(b_dev, m, tol)
+    x = to_full(ctx, L, x_dev, 0)
+    xo, it_o, rel_o, st, _ = oracle.cg(L, X, W, m, tol, b_full)
+    assert st == 0
+    # converged to the requested residual, judged by the ORACLE operator
+    assert _true_relres(L, X, W, m, x, b_full)[0] <= tol
+    assert info["true_rel_resid"][0] <= tol
+    # solution agrees to 10 x tol (north_star)
+    assert rel_l2(x[0], xo[0]) <= 10 * tol
+    # same textbook recurrence => same iteration count up to rounding-order effects
+    assert abs(info["iterations"] - int(it_o[0])) <= 3, (info, it_o)
+    assert np.all(x[0][oracle.site_parity(L) == 1] == 0)
+    ctx.close()
+
+
+def test_cg_multi_rhs_independent_scalars_and_freezing():
+    """RHS with very different difficulty: one is an exact eigen-direction scaled source that converges
+    early, the others keep iterating; each must match its own single-RHS oracle solve."""
+    L, m, tol = (4, 6, 8, 10), 0.2, 1e-9
+    nrhs = 3
+    ctx, X, W = make_ctx(L, "fp64", nrhs, 1)
+    b_dev, b_full = make_field(ctx, L, 1, nrhs, 0)
+    # make RHS 1 tiny in norm and RHS 2 = 1000 * RHS 0 (same iterations as RHS 0, scale invariance)
+    b_dev[1] *= 1e-6
+    b_dev[2] = 1000.0 * b_dev[0]
+    b_full[1] *= 1e-6
+    b_full[2] = 1000.0 * b_full[0]
+    x_dev, info = ctx.cg(b_dev, m, tol)
+    x = to_full(ctx, L, x_dev, 0)
+    xo, it_o, rel_o, st, _ = oracle.cg(L, X, W, m, tol, b_full)
+    rr = _true_relres(L, X, W, m, x, b_full)
+    for k in range(nrhs):
+        assert rr[k] <= tol and info["true_rel_resid"][k] <= tol
+        assert rel_l2(x[k], xo[k]) <= 10 * tol
+    assert abs(info["iterations"] - int(it_o.max())) <= 3
+    ctx.close()
+
+
+def test_cg_zero_rhs_and_max_iter():
+    L = (4, 4, 4, 4)
+    ctx, X, W = make_ctx(L, "fp64", 2, 2)
+    b_dev, _ = make_field(ctx, L, 2, 2, 0)
+    b_dev[1].zero_()                                   # a zero right-hand side: x = 0, no breakdown
+    x_dev, info = ctx.cg(b_dev, 0.1, 1e-8)
+    assert torch.all(x_dev[1] == 0) and info["true_rel_resid"][0] <= 1e-8
+    ctx.set_option("max_iter", 5)
+    x_dev, info = ctx.cg(b_dev, 0.01, 1e-12, strict=False)
+    assert info["status"] == -5 and info["iterations"] == 5
+    assert info["true_rel_resid"][0] > 1e-12
+    ctx.close()
+
+
+def test_cg_fp32_context_converges_moderate_kappa():
+    L, m, tol = (8, 8, 8, 8), 0.2, 1e-5
+    ctx, X, W = make_ctx(L, "fp32", 2, 3)
+    b_dev, b_full = make_field(ctx, L, 3, 2, 0)
+    x_dev, info = ctx.cg(b_dev, m, tol)
+    x = to_full(ctx, L, x_dev, 0)
+    for k, r in enumerate(_true_relres(L, X, W, m, x, b_full)):
+        assert r <= 2 * tol, (k, r)
+    ctx.close()
+
+
+def test_cg_mixed_precision_reliable_updates():
+    """HISQ_MIXED: fp32 operator inside, fp64 reliable update; converges to an fp64-level tolerance that
+    a pure fp32 solve cannot reach, and agrees with the oracle's fp64 solve."""
+    L, m, tol = (8, 8, 8, 8), 0.05, 1e-10
+    nrhs = 2
+    ctx, X, W = make_ctx(L, "mixed", nrhs, 4)
+    ctx.set_option("reliable_interval", 50)
+    b_dev, b_full = make_field(ctx, L, 4, nrhs, 0)
+    x_dev, info = ctx.cg(b_dev, m, tol)
+    x = to_full(ctx, L, x_dev, 0)
+    xo, it_o, rel_o, st, _ = oracle.cg(L, X, W, m, tol, b_full)
+    rr = _true_relres(L, X, W, m, x, b_full)
+    for k in range(nrhs):
+        assert rr[k] <= tol, (k, rr)
+        assert rel_l2(x[k], xo[k]) <= 10 * tol
+    assert info["reliable_updates"] >= info["iterations"] // 50
+    assert info["iterations"] <= 1.3 * it_o.max() + 50, (info, it_o)
+    ctx.close()
+
+
+def test_cg_host_entry_point():
+    L, m, tol = (4, 6, 4, 8), 0.1, 1e-10
+    ctx, X, W = make_ctx(L, "fp64", 1, 5)
+    b_dev, b_full = make_field(ctx, L, 5, 1, 0)
+    b_h = ctx.unpack(b_dev).cpu().pin_memory()
+    x_h = torch.empty_like(b_h).pin_memory()
+    _, info = ctx.cg_host(x_h, b_h, m, tol)
+    x = oracle.half_to_full(L, x_h.numpy(), 0)
+    assert _true_relres(L, X, W, m, x, b_full)[0] <= tol
+    ctx.close()
+
+
+def test_cg_is_run_to_run_reproducible():
+    L = (4, 6, 8, 10)
+    ctx, X, W = make_ctx(L, "fp64", 2, 6)
+    b_dev, _ = make_field(ctx, L, 6, 2, 0)
+    x1, i1 = ctx.cg(b_dev, 0.1, 1e-10)
+    x1 = x1.clone()
+    x2, i2 = ctx.cg(b_dev, 0.1, 1e-10)
+    assert torch.equal(x1, x2) and i1["iterations"] == i2["iterations"]
+    ctx.close()

@@ -1,0 +1,127 @@
+"""-m gpu: the CUDA Dslash (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances are north_star's: rel-L2 <= 1e-12 (fp64), <= 2e-5 (fp32) per application
+and per RHS; we additionally require the level a correct kernel reaches (SURVEY 8(c) "gates")."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from tests.gpu_helpers import make_ctx, make_field, rel_l2, to_full
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"fp64": (1e-12, 1e-14), "fp32": (2e-5, 1e-6)}   # (contract, expected level)
+
+SHAPES = [(8, 8, 8, 8), (4, 4, 4, 4), (4, 6, 8, 10), (6, 8, 8, 4), (12, 6, 10, 8), (16, 4, 4, 6)]
+
+
+def _check(L, prec, nrhs, seed, **kw):
+    ctx, X, W = make_ctx(L, prec, nrhs, seed, **kw)
+    par_sites = oracle.site_parity(L)
+    for parity in (0, 1):
+        dev_in, full_in = make_field(ctx, L, seed + 100, nrhs, 1 - parity)
+        out = ctx.dslash(dev_in, parity)
+        got = to_full(ctx, L, out, parity)
+        ref = oracle.dslash_parity(L, X, W, full_in, parity)
+        scale = np.sqrt(np.mean(np.abs(ref[:, par_sites == parity]) ** 2))
+        for k in range(nrhs):
+            err = rel_l2(got[k], ref[k])
+            assert err <= TOL[prec][0], (L, prec, nrhs, parity, k, err)
+            assert err <= TOL[prec][1], ("above the level a correct kernel reaches", L, prec, k, err)
+            # a wrong sign on a single site hides in an L2 number: also bound the worst site
+            worst = np.abs(got[k] - ref[k]).max() / scale
+            assert worst <= 50 * TOL[prec][1], (L, prec, nrhs, parity, k, worst)
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+@pytest.mark.parametrize("L", SHAPES)
+def test_dslash_single_rhs(L, prec):
+    _check(L, prec, 1, seed=0)
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+@pytest.mark.parametrize("nrhs", [2, 3, 4, 5, 6, 7, 8, 12])
+def test_dslash_multi_rhs(nrhs, prec):
+    _check((4, 6, 8, 10), prec, nrhs, seed=1)
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_dslash_fat_only_and_naik_only(prec):
+    # the Naik part is only ~6 % of the norm: check it on its own (pin P13 mirrored on the GPU side)
+    _check((8, 8, 8, 8), prec, 2, seed=2, fat_only=True)
+    _check((8, 8, 8, 8), prec, 2, seed=2, naik_only=True)
+    _check((4, 4, 6, 4), prec, 1, seed=3, naik_only=True)   # +3 and -1 hops coincide, Lt = 4 sign cases
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+@pytest.mark.parametrize("inner", [1, 2, 4, 8])
+def test_dslash_inner_outer_split_is_equivalent(prec, inner):
+    L, nrhs = (8, 4, 6, 8), 8
+    ctx, X, W = make_ctx(L, prec, nrhs, 4)
+    dev_in, full_in = make_field(ctx, L, 5, nrhs, 0)
+    ctx.set_option("nrhs_inner", inner)
+    got = to_full(ctx, L, ctx.dslash(dev_in, 1), 1)
+    ref = oracle.dslash_parity(L, X, W, full_in, 1)
+    for k in range(nrhs):
+        assert rel_l2(got[k], ref[k]) <= TOL[prec][1]
+    ctx.close()
+
+
+@pytest.mark.parametrize("tiles", [(4, 4), (4, 8), (8, 4)])
+def test_dslash_tiled_sweep_order_is_equivalent(tiles):
+    L = (8, 8, 8, 6)
+    ctx, X, W = make_ctx(L, "fp64", 2, 6)
+    dev_in, full_in = make_field(ctx, L, 7, 2, 1)
+    ctx.set_option("tile_y", tiles[0]); ctx.set_option("tile_z", tiles[1])
+    assert ctx.tiles(2) == tiles
+    got = to_full(ctx, L, ctx.dslash(dev_in, 0), 0)
+    ref = oracle.dslash_parity(L, X, W, full_in, 0)
+    assert rel_l2(got, ref) <= 1e-14
+    ctx.close()
+
+
+def test_pack_unpack_roundtrip_and_layout():
+    L = (4, 6, 4, 8)
+    ctx, _, _ = make_ctx(L, "fp64", 3, 0)
+    can = torch.randn(3, ctx.Vh, 3, dtype=torch.complex128, device=ctx.device)
+    nat = ctx.pack(can)
+    assert torch.equal(nat, can.permute(0, 2, 1).contiguous())
+    assert torch.equal(ctx.unpack(nat), can)
+    ctx.close()
+
+
+def test_dslash_host_entry_point_matches_device_path():
+    L = (8, 4, 6, 8)
+    ctx, X, W = make_ctx(L, "fp64", 2, 8)
+    dev_in, full_in = make_field(ctx, L, 9, 2, 1)
+    can_in = ctx.unpack(dev_in).cpu().pin_memory()
+    out_h = torch.empty_like(can_in).pin_memory()
+    ctx.dslash_host(out_h, can_in, 0)
+    ref = oracle.dslash_parity(L, X, W, full_in, 0)
+    assert rel_l2(oracle.half_to_full(L, out_h.numpy(), 0), ref) <= 1e-14
+    ctx.close()
+
+
+def test_error_codes():
+    from paper_2306_01098_b200 import binding
+    L = (4, 4, 4, 4)
+    ctx = binding.Hisq(L, "fp64", 1)
+    f = ctx.new_field(1)
+    with pytest.raises(binding.HisqError) as e:
+        ctx.dslash(f, 0)
+    assert e.value.code == -2                       # links not set
+    fat, naik = binding.make_links(L, 0, ctx.device)
+    ctx.set_links(fat, naik)
+    with pytest.raises(binding.HisqError) as e:
+        ctx.dslash(f, 0, out=f)
+    assert e.value.code == -1                       # aliasing
+    with pytest.raises(binding.HisqError) as e:
+        ctx.dslash(f, 2)
+    assert e.value.code == -1                       # bad parity
+    with pytest.raises(binding.HisqError) as e:
+        ctx.cg(ctx.new_field(2), 0.1, 1e-8)
+    assert e.value.code == -3                       # workspace sized for 1 RHS
+    with pytest.raises(binding.HisqError):
+        ctx.set_option("no_such_option", 1)
+    ctx.close()
