@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the multi-RHS HISQ Dslash + CG hot path on B200.
+
+A STEP is one pass of the whole hot path on BASELINE.json configs[1] (32^3 x 8, fp64, nRHS = 1): one
+`hisq_cg` solve of (m^2 - D_eo D_oe) x = b at m = 0.01 to tol 1e-10 (index maps, gathers, Dslash,
+fused A-apply, BLAS-1/reductions, convergence control: SURVEY.md 8(a) rows a1-a7) on seeded synthetic
+links and a Gaussian even-site source already resident in HBM.  `value` is the metric BASELINE.json
+names, HISQ Dslash GFLOP/s, counted as 1146 flop per output site per RHS over every
+Dslash application the solve made, divided by the whole solve time (so BLAS-1 and host polling count
+against it).  Beside it:
+  dslash     pure Dslash launches (alternating D_oe / D_eo), CUDA-event timed: GFLOP/s, algorithmic GB/s
+  roofline   the dominant kernel (Dslash fp64 n=1) against MEASURED_PEAKS.json's HBM copy bandwidth
+  sweep      configs[2] (64^3 x 16, fp32) Dslash vs nRHS = 1, 2, 4, 8     (--no-sweep to skip)
+  e2e        the same step through hisq_cg_host with pinned HOST buffers (H2D + D2H inside the timing)
+  cpu_baseline  the oracle (oracle/, as it stands) on this box's host cores on a bounded sample
+`--impl reference` times the oracle instead (this tier's reference arm).
+Multi-GPU (torchrun): independent replicas, one per rank, no collective on the data path ("replicas
+only"); value = total flops of all ranks / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FLOP_PER_SITE = 1146
+CONFIGS = {
+    "C1": dict(L=(8, 8, 8, 8), prec="fp64", nrhs=1, mass=0.1, tol=1e-10),
+    "C2": dict(L=(32, 32, 32, 8), prec="fp64", nrhs=1, mass=0.01, tol=1e-10),
+    "C3": dict(L=(64, 64, 64, 16), prec="fp32", nrhs=8, mass=None, tol=None),
+    "C4": dict(L=(48, 48, 48, 12), prec="mixed", nrhs=4, mass=0.002, tol=1e-9),
+    "C5": dict(L=(96, 96, 96, 24), prec="fp64", nrhs=8, mass=0.005, tol=1e-10),
+}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write, burst)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm = sorted(int(r[0]) for r in self.rows if r and r[0].isdigit())
+        reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        mx = [int(r[1]) for r in self.rows if len(r) > 1 and r[1].isdigit()]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def dslash_bytes(Vh: int, nrhs: int, w: int) -> int:
+    """Algorithmic (compulsory) bytes of one Dslash application: 16 links of 18 reals per output site,
+    each input and each output site's colour vector once: (288 + 12 n) words per site."""
+    return (288 + 12 * nrhs) * w * Vh
+
+
+def time_dslash(ctx, nrhs: int, reps: int, warm: int = 5):
+    """Average device time (ms) of one Dslash launch, alternating D_oe / D_eo on fixed inputs,
+    one pair of CUDA events on the launching stream around 2*reps back-to-back launches."""
+    a, c = ctx.new_field(nrhs), ctx.new_field(nrhs)
+    b, d = ctx.new_field(nrhs), ctx.new_field(nrhs)
+    a.copy_(torch.randn_like(a))
+    c.copy_(torch.randn_like(c))
+    for _ in range(warm):
+        ctx.dslash(a, 1, out=b)
+        ctx.dslash(c, 0, out=d)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        ctx.dslash(a, 1, out=b)
+        ctx.dslash(c, 0, out=d)
+    e1.record()
+    e1.synchronize()
+    return e0.elapsed_time(e1) / (2 * reps)
+
+
+def oracle_sample(cfg, seed: int, budget_s: float):
+    """Time the oracle on a bounded sample of the step: `iters` CG iterations of the same workload."""
+    import numpy as np
+    import oracle
+    from paper_2306_01098_b200 import inputs
+    L = cfg["L"]
+    V = inputs.volume(L)
+    s = torch.arange(V, dtype=torch.int64)
+    X = inputs.fat_links(L, seed, s).numpy()
+    W = inputs.naik_links(L, seed, s).numpy()
+    b = inputs.sources(L, seed, s, cfg["nrhs"]).numpy()
+    par = oracle.site_parity(L)
+    b[:, par == 1, :] = 0
+    t0 = time.perf_counter()
+    oracle.cg(L, X, W, cfg["mass"], 1e-30, b, max_iter=1)
+    t1 = time.perf_counter() - t0
+    iters = max(2, min(200, int(budget_s / max(t1 / 2, 1e-3))))   # 1 iteration = 2 A-applies incl. the final check
+    t0 = time.perf_counter()
+    oracle.cg(L, X, W, cfg["mass"], 1e-30, b, max_iter=iters)
+    dt = time.perf_counter() - t0
+    n_dslash = 2 * (iters + 1) * cfg["nrhs"]                         # + the final true-residual application
+    gflops = FLOP_PER_SITE * (V // 2) * n_dslash / dt / 1e9
+    return gflops, dt, iters, oracle.threads()
+
+
+def run_reference(args, cfg, rank, world):
+    if rank != 0:
+        return
+    vals, dts = [], []
+    for i in range(args.warmup + args.steps):
+        g, dt, iters, cores = oracle_sample(cfg, 0, args.ref_budget)
+        if i >= args.warmup:
+            vals.append(g)
+            dts.append(dt)
+    v = sum(vals) / len(vals)
+    sample = f"{iters} CG iterations (2 Dslash each, + 1 final residual) of the {args.config} solve per step"
+    print(json.dumps({
+        "impl": "reference", "metric": "hisq_dslash_gflops", "value": v, "unit": "GFLOP/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(dts) / len(dts), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(args.config, cfg)},
+        "cpu_baseline": {"value": v, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def workload_name(name, cfg):
+    L = cfg["L"]
+    return (f"{name}: {L[0]}x{L[1]}x{L[2]}x{L[3]} {cfg['prec']} nRHS={cfg['nrhs']} CG m={cfg['mass']} tol={cfg['tol']}, "
+            "Gaussian fat links (std 0.3), Haar SU(3) Naik x(-1/24), phases folded, antiperiodic t")
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C4", "C5"])
+    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=15.0)
+    ap.add_argument("--ref-budget", type=float, default=10.0)
+    ap.add_argument("--dslash-reps", type=int, default=100)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    cfg = CONFIGS[args.config]
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        return run_reference(args, cfg, rank, world)
+
+    from paper_2306_01098_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libhisq has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    L, n = cfg["L"], cfg["nrhs"]
+    w = 4 if cfg["prec"] == "fp32" else 8
+    big = binding.layout.volume(L) > (1 << 21)
+    gen_dev = dev if big else None                      # small lattices: CPU generation, bit-identical to the oracle's inputs
+    ctx = binding.Hisq(L, cfg["prec"], n, dev)
+    fat, naik = binding.make_links(L, rank, dev, ctx.cdtype, gen_device=gen_dev)
+    ctx.set_links(fat, naik)
+    del fat, naik
+    b_can = binding.make_sources(L, rank, n, 0, dev, ctx.cdtype, gen_device=gen_dev)
+    b = ctx.pack(b_can)
+    x = ctx.new_field(n)
+    b_host = b_can.cpu().pin_memory()
+    x_host = torch.empty_like(b_host).pin_memory()
+    Vh = ctx.Vh
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- the step, device-resident inputs ----
+    for _ in range(args.warmup):
+        _, info = ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    l0 = ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    n_dslash = 0
+    for _ in range(args.steps):
+        _, info = ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
+        n_dslash += 2 * (info["iterations"] + info["reliable_updates"])
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = ctx.launch_count() - l0
+    clocks = sampler.stop()
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    fl = torch.tensor([float(FLOP_PER_SITE) * Vh * n * n_dslash], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(fl, op=dist.ReduceOp.SUM)
+    ms_all, flops_all = t.item(), fl.item()
+    value = flops_all / (ms_all * 1e-3) / 1e9
+
+    # ---- the same step end to end: pinned host buffers through hisq_cg_host ----
+    ctx.cg_host(x_host, b_host, cfg["mass"], cfg["tol"])
+    barrier()
+    t0 = time.perf_counter()
+    e0.record()
+    nd2 = 0
+    for _ in range(args.steps):
+        _, info2 = ctx.cg_host(x_host, b_host, cfg["mass"], cfg["tol"])
+        nd2 += 2 * (info2["iterations"] + info2["reliable_updates"])
+    e1.record()
+    barrier()
+    ms2 = max(e0.elapsed_time(e1), 0.0)
+    t2 = torch.tensor([ms2], dtype=torch.float64, device=dev)
+    f2 = torch.tensor([float(FLOP_PER_SITE) * Vh * n * nd2], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+        dist.all_reduce(f2, op=dist.ReduceOp.SUM)
+    e2e_val = f2.item() / (t2.item() * 1e-3) / 1e9
+    field_bytes = b_host.numel() * b_host.element_size()
+
+    # ---- the dominant kernel alone: Dslash, CUDA-event timed ----
+    d_ms = time_dslash(ctx, n, args.dslash_reps)
+    peak, peak_src = measured_peaks()
+    alg_bytes = dslash_bytes(Vh, n, w)
+    achieved = alg_bytes / (d_ms * 1e-3) / 1e9
+    dsl = {"ms": d_ms, "gflops": FLOP_PER_SITE * Vh * n / (d_ms * 1e-3) / 1e9, "alg_gbs": achieved,
+           "paper_model_gbs": (288 + 102 * n) * w * Vh / (d_ms * 1e-3) / 1e9,
+           "frac_of_measured_copy": achieved / peak, "frac_of_8TBs": achieved / 8000.0, "tiles": ctx.tiles(n)}
+    ctx.close()
+    del ctx, b, x
+
+    out = {
+        "metric": "hisq_dslash_gflops", "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": {"fp32": "f32", "fp64": "f64", "mixed": "f32+f64"}[cfg["prec"]], "data": "synthetic",
+        "config": {"workload": workload_name(args.config, cfg), "l2": "inputs larger than L2 (links %.0f MB)" % (2 * 4 * 2 * Vh * 18 * w / 1e6),
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "cg": {"solve_ms": ms_all / args.steps, "iterations": info["iterations"], "true_residual_checks": info["reliable_updates"],
+               "true_rel_resid": info["true_rel_resid"], "ms_per_iteration": ms_all / args.steps / max(info["iterations"], 1)},
+        "dslash": dsl,
+        "roofline": {"bound": "hbm", "kernel": f"dslash_kernel<{'float' if w == 4 else 'double'},NR={min(n, 8 if w == 4 else 4)}>",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
+                     "timing": f"CUDA events around {2 * args.dslash_reps} back-to-back launches (alternating parity), burst"},
+        "e2e": {"value": e2e_val, "unit": "GFLOP/s", "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": field_bytes,
+                "ms_per_step": t2.item() / args.steps},
+        "gpu_launches": int(launches), "clocks": clocks,
+    }
+
+    if rank == 0 and not args.no_sweep:
+        out["sweep"] = sweep_c3(dev, peak, args.dslash_reps)
+    if rank == 0 and not args.no_cpu_baseline:
+        g, dt, iters, cores = oracle_sample(cfg, 0, args.cpu_budget)
+        out["cpu_baseline"] = {"value": g, "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
+                               "sample": f"{iters} CG iterations (2 Dslash each, + 1 final residual) of the {args.config} solve, {dt:.1f} s"}
+    if rank == 0:
+        print(json.dumps(out))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def sweep_c3(dev, peak, reps):
+    """configs[2]: 64^3 x 16, fp32 operator, nRHS = 1, 2, 4, 8: Dslash throughput vs nRHS."""
+    from paper_2306_01098_b200 import binding
+    cfg = CONFIGS["C3"]
+    L = cfg["L"]
+    ctx = binding.Hisq(L, "fp32", 8, dev)
+    fat, naik = binding.make_links(L, 0, dev, ctx.cdtype, gen_device=dev)
+    ctx.set_links(fat, naik)
+    del fat, naik
+    rows = []
+    for n in (1, 2, 4, 8):
+        ms = time_dslash(ctx, n, max(10, reps // 4))
+        by = dslash_bytes(ctx.Vh, n, 4)
+        rows.append({"nrhs": n, "ms": ms, "gflops": FLOP_PER_SITE * ctx.Vh * n / (ms * 1e-3) / 1e9,
+                     "alg_gbs": by / (ms * 1e-3) / 1e9, "frac_of_measured_copy": by / (ms * 1e-3) / 1e9 / peak,
+                     "tiles": ctx.tiles(n)})
+    ctx.close()
+    return {"workload": "C3: 64x64x64x16 fp32 Dslash", "rows": rows}
+
+
+if __name__ == "__main__":
+    main()

@@ -184,7 +184,10 @@ __global__ void cg_after_residual_kernel(CgState* st, double* true_rr_out)
         const double rt = st->sums[k];
         true_rr_out[k] = rt;
         const bool conv = rt <= st->tol2 * st->bnorm2[k];
-        st->beta[k] = (!conv && st->rho_prev[k] > 0.0) ? rt / st->rho_prev[k] : 0.0;
+        // keep the search direction while the recomputed residual is consistent with the recursive one;
+        // if it drifted far (rt > 4 rho: the recursion was below the attainable accuracy) restart with p = r
+        const bool consistent = rt <= 4.0 * st->rho[k];
+        st->beta[k] = (!conv && consistent && st->rho_prev[k] > 0.0) ? rt / st->rho_prev[k] : 0.0;
         st->rho[k] = rt;
         st->active[k] = (!conv && st->bnorm2[k] > 0.0) ? 1 : 0;
         any |= st->active[k];

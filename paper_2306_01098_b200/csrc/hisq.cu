@@ -17,6 +17,7 @@ struct hisq_ctx {
     Geom g;
     int prec;
     cudaStream_t stream;
+    cudaStream_t cap_stream;   // private stream used only to CAPTURE graphs (the legacy stream cannot be captured)
     // workspace carve-up (all device pointers into the caller's buffer)
     char* ws;
     size_t ws_bytes;
@@ -99,6 +100,7 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     h->g.ty = Ly; h->g.tz = Lz; h->g.nty = 1; h->g.ntz = 1;
     h->prec = prec;
     h->stream = 0;
+    h->cap_stream = nullptr;
     h->ws = nullptr; h->ws_bytes = 0; h->ws_nrhs = 0;
     h->links64 = nullptr; h->links32 = nullptr; h->have_links = false;
     h->max_iter = 100000;
@@ -123,6 +125,7 @@ extern "C" int hisq_destroy(hisq_ctx* h)
 {
     if (!h) return HISQ_EINVAL;
     if (h->host_state) cudaFreeHost(h->host_state);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     delete h;
     return HISQ_OK;
 }
@@ -353,15 +356,22 @@ static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_u
     int rc = HISQ_OK;
     int status = HISQ_OK;
     long long launches_per_batch = 0;
+    int stagnation = 0;
+    double best_true[kMaxNrhs];
+    for (int k = 0; k < kMaxNrhs; ++k) best_true[k] = 1e300;
     while (true) {
         // ---- a batch of iterations ----
         if (h->use_graph) {
             if (!ib.exec) {
                 cudaGraph_t graph;
                 const long long l0 = h->stats.launches;
-                CK(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+                if (!h->cap_stream) CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+                cudaStream_t user_stream = h->stream;
+                CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+                h->stream = h->cap_stream;
                 for (int i = 0; i < batch && rc == HISQ_OK; ++i) rc = enqueue_iteration<T>(h, links, x, r, p, q, t, m2, nrhs);
-                cudaError_t ce = cudaStreamEndCapture(h->stream, &graph);
+                h->stream = user_stream;
+                cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
                 if (rc != HISQ_OK) { if (ce == cudaSuccess) cudaGraphDestroy(graph); break; }
                 if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaStreamEndCapture"); break; }
                 ce = cudaGraphInstantiate(&ib.exec, graph, 0);
@@ -403,6 +413,15 @@ static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_u
         for (int k = 0; k < nrhs; ++k)
             h->info_relres[k] = s2.bnorm2[k] > 0.0 ? std::sqrt(trr[k] / s2.bnorm2[k]) : 0.0;
         if (status == HISQ_EBREAKDOWN) break;
+        if (s.done && !s2.done) {
+            // the recursion said "converged", the true residual says no: resume, unless this keeps happening
+            // without progress (tol below what this precision can reach)
+            bool improved = false;
+            for (int k = 0; k < nrhs; ++k)
+                if (s2.active[k] && h->info_relres[k] < 0.9 * best_true[k]) { best_true[k] = h->info_relres[k]; improved = true; }
+            stagnation = improved ? 0 : stagnation + 1;
+            if (stagnation >= 3) { status = HISQ_ENOCONV; break; }
+        }
         if (s2.done) {
             bool all = true;
             for (int k = 0; k < nrhs; ++k) all = all && !s2.active[k];
