@@ -88,6 +88,17 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def aggregate(ms: float, flops: float, dist, device):
+    """Whole-job throughput over ranks: (max over ranks of the device time, sum over ranks of the work).
+    No collective sits on the data path ("replicas only"): this all-reduce only combines the timings."""
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    f = torch.tensor([flops], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(f, op=dist.ReduceOp.SUM)
+    return t.item(), f.item()
+
+
 def dslash_bytes(Vh: int, nrhs: int, w: int) -> int:
     """Algorithmic (compulsory) bytes of one Dslash application: 16 links of 18 reals per output site,
     each input and each output site's colour vector once: (288 + 12 n) words per site."""
@@ -131,7 +142,7 @@ def oracle_sample(cfg, seed: int, budget_s: float):
     t0 = time.perf_counter()
     oracle.cg(L, X, W, cfg["mass"], 1e-30, b, max_iter=1)
     t1 = time.perf_counter() - t0
-    iters = max(2, min(200, int(budget_s / max(t1 / 2, 1e-3))))   # 1 iteration = 2 A-applies incl. the final check
+    iters = max(2, min(2000, int(budget_s / max(t1 / 2, 1e-3))))   # 1 iteration = 2 A-applies incl. the final check
     t0 = time.perf_counter()
     oracle.cg(L, X, W, cfg["mass"], 1e-30, b, max_iter=iters)
     dt = time.perf_counter() - t0
@@ -173,7 +184,10 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C4", "C5"])
+    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--only", default="all", choices=["all", "dslash"],
+                    help="dslash: time only the Dslash kernel of --config at --nrhs (profiling driver)")
+    ap.add_argument("--nrhs", type=int, default=0, help="override the config's nRHS (--only dslash)")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
@@ -187,6 +201,10 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         return run_reference(args, cfg, rank, world)
+    if args.only == "dslash":
+        return run_dslash_only(args, cfg)
+    if args.config == "C3":
+        raise SystemExit("C3 is a Dslash-only config: use --only dslash")
 
     from paper_2306_01098_b200 import binding
     if not torch.cuda.is_available():
@@ -236,12 +254,7 @@ def main():
     ms = e0.elapsed_time(e1)
     launches = ctx.launch_count() - l0
     clocks = sampler.stop()
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    fl = torch.tensor([float(FLOP_PER_SITE) * Vh * n * n_dslash], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(fl, op=dist.ReduceOp.SUM)
-    ms_all, flops_all = t.item(), fl.item()
+    ms_all, flops_all = aggregate(ms, float(FLOP_PER_SITE) * Vh * n * n_dslash, dist, dev)
     value = flops_all / (ms_all * 1e-3) / 1e9
 
     # ---- the same step end to end: pinned host buffers through hisq_cg_host ----
@@ -256,12 +269,8 @@ def main():
     e1.record()
     barrier()
     ms2 = max(e0.elapsed_time(e1), 0.0)
-    t2 = torch.tensor([ms2], dtype=torch.float64, device=dev)
-    f2 = torch.tensor([float(FLOP_PER_SITE) * Vh * n * nd2], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t2, op=dist.ReduceOp.MAX)
-        dist.all_reduce(f2, op=dist.ReduceOp.SUM)
-    e2e_val = f2.item() / (t2.item() * 1e-3) / 1e9
+    ms2_all, f2_all = aggregate(ms2, float(FLOP_PER_SITE) * Vh * n * nd2, dist, dev)
+    e2e_val = f2_all / (ms2_all * 1e-3) / 1e9
     field_bytes = b_host.numel() * b_host.element_size()
 
     # ---- the dominant kernel alone: Dslash, CUDA-event timed ----
@@ -289,7 +298,7 @@ def main():
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
                      "timing": f"CUDA events around {2 * args.dslash_reps} back-to-back launches (alternating parity), burst"},
         "e2e": {"value": e2e_val, "unit": "GFLOP/s", "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": field_bytes,
-                "ms_per_step": t2.item() / args.steps},
+                "ms_per_step": ms2_all / args.steps},
         "gpu_launches": int(launches), "clocks": clocks,
     }
 
@@ -304,6 +313,29 @@ def main():
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
+
+
+def run_dslash_only(args, cfg):
+    """Profiling driver: only Dslash launches of one config (ncu -k regex:dslash_kernel ...)."""
+    from paper_2306_01098_b200 import binding
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    L = cfg["L"]
+    n = args.nrhs if args.nrhs > 0 else cfg["nrhs"]
+    prec = "fp64" if cfg["prec"] == "mixed" else cfg["prec"]
+    w = 4 if prec == "fp32" else 8
+    ctx = binding.Hisq(L, prec, n, dev)
+    fat, naik = binding.make_links(L, 0, dev, ctx.cdtype, gen_device=dev)
+    ctx.set_links(fat, naik)
+    del fat, naik
+    ms = time_dslash(ctx, n, args.dslash_reps)
+    peak, src = measured_peaks()
+    by = dslash_bytes(ctx.Vh, n, w)
+    print(json.dumps({"only": "dslash", "config": args.config, "L": L, "prec": prec, "nrhs": n, "ms": ms,
+                      "gflops": FLOP_PER_SITE * ctx.Vh * n / (ms * 1e-3) / 1e9, "alg_gbs": by / (ms * 1e-3) / 1e9,
+                      "frac_of_measured_copy": by / (ms * 1e-3) / 1e9 / peak, "frac_of_8TBs": by / (ms * 1e-3) / 1e9 / 8000.0,
+                      "tiles": ctx.tiles(n), "launches": ctx.launch_count()}))
+    ctx.close()
 
 
 def sweep_c3(dev, peak, reps):

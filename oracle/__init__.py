@@ -191,3 +191,31 @@ def full_to_half(L, full, parity: int) -> np.ndarray:
     half = np.empty((full.shape[0], V // 2, 3), dtype=np.complex128)
     half[:, eo[sel] - parity * (V // 2), :] = full[:, sel, :]
     return half
+
+
+# ---- sampled evaluation on lattices too large for host arrays -------------------------------------------
+def neighbour_sites(L, sites):
+    """For lexicographic sites [n]: (plus, minus) each [n, 2, 4] = lex of x +- hop*mu, hop = 1 (f=0), 3 (f=1)."""
+    sites = np.asarray(sites, dtype=np.int64)
+    c = np.stack([sites % L[0], (sites // L[0]) % L[1], (sites // (L[0] * L[1])) % L[2], sites // (L[0] * L[1] * L[2])], axis=1)
+    plus = np.empty((sites.size, 2, 4), dtype=np.int64)
+    minus = np.empty((sites.size, 2, 4), dtype=np.int64)
+    for f, hop in enumerate((1, 3)):
+        for mu in range(4):
+            for sign, dst in ((+1, plus), (-1, minus)):
+                cc = c.copy()
+                cc[:, mu] = (cc[:, mu] + sign * hop) % L[mu]
+                dst[:, f, mu] = cc[:, 0] + L[0] * (cc[:, 1] + L[1] * (cc[:, 2] + L[2] * cc[:, 3]))
+    return plus, minus, c[:, 3].astype(np.int32)
+
+
+def dslash_gathered(Lt, t, Ff, Fb, vp, vm) -> np.ndarray:
+    """(D phi)(x_i) from pre-fetched operands: Ff, Fb [n,2,4,3,3]; vp, vm [n,2,4,3]; t [n] int32."""
+    n = len(t)
+    Ff = np.ascontiguousarray(Ff, dtype=np.complex128); Fb = np.ascontiguousarray(Fb, dtype=np.complex128)
+    vp = np.ascontiguousarray(vp, dtype=np.complex128); vm = np.ascontiguousarray(vm, dtype=np.complex128)
+    t = np.ascontiguousarray(t, dtype=np.int32)
+    assert Ff.shape == (n, 2, 4, 3, 3) and Fb.shape == Ff.shape and vp.shape == (n, 2, 4, 3) and vm.shape == vp.shape
+    out = np.empty((n, 3), dtype=np.complex128)
+    _lib().oracle_dslash_gathered(ctypes.c_int(int(Lt)), ctypes.c_long(n), _c(t), _c(Ff), _c(Fb), _c(vp), _c(vm), _c(out))
+    return out

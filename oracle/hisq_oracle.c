@@ -171,6 +171,43 @@ static void dslash_site(const int *L, const cplx *X, const cplx *W, const cplx *
     COUNT_OUT(6);
 }
 
+/* The same sum for ONE site whose 16 links and 16 neighbour vectors were fetched by the caller (used to
+ * check sampled outputs of lattices too big to hold on the host): Ff[f][mu] = F_mu(x), Fb[f][mu] =
+ * F_mu(x - hop mu), vp[f][mu] = phi(x + hop mu), vm[f][mu] = phi(x - hop mu), f = 0 fat (hop 1), 1 Naik
+ * (hop 3); t, Lt give the antiperiodic sign.  Same helpers, same order as dslash_site. */
+static void dslash_site_gathered(int t, int Lt, const cplx *Ff, const cplx *Fb, const cplx *vp_in, const cplx *vm_in,
+                                 cplx *out)
+{
+    cplx dir[4][3];
+    for (int mu = 0; mu < 4; ++mu) {
+        cplx term[2][3];
+        for (int f = 0; f < 2; ++f) {
+            int hop = f ? 3 : 1;
+            int sp = (mu == 3 && t + hop >= Lt) ? -1 : +1;
+            int sm = (mu == 3 && t - hop < 0) ? -1 : +1;
+            cplx vp[3], vm[3], fwd[3], bwd[3];
+            gather(vp_in + (f * 4 + mu) * 3, 0, sp, vp);
+            gather(vm_in + (f * 4 + mu) * 3, 0, sm, vm);
+            mat_vec(Ff + (f * 4 + mu) * 9, vp, fwd);
+            matdag_vec(Fb + (f * 4 + mu) * 9, vm, bwd);
+            vec_sub(fwd, bwd, term[f]);
+        }
+        vec_add(term[0], term[1], dir[mu]);
+    }
+    cplx s01[3], s012[3];
+    vec_add(dir[0], dir[1], s01);
+    vec_add(s01, dir[2], s012);
+    vec_add(s012, dir[3], out);
+}
+
+/* n sites: t[i]; Ff, Fb [i][2][4][9]; vp, vm [i][2][4][3]; out [i][3]. */
+void oracle_dslash_gathered(int Lt, long n, const int *t, const cplx *Ff, const cplx *Fb, const cplx *vp, const cplx *vm,
+                            cplx *out)
+{
+    for (long i = 0; i < n; ++i)
+        dslash_site_gathered(t[i], Lt, Ff + i * 72, Fb + i * 72, vp + i * 24, vm + i * 24, out + i * 3);
+}
+
 /* ---------- D on sets of sites ---------- */
 
 static int parity_of(const int *L, long lex)

@@ -388,7 +388,7 @@ static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_u
             if (rc != HISQ_OK) break;
         }
         if ((rc = poll_state(h)) != HISQ_OK) break;
-        const CgState& s = *h->host_state;
+        const CgState s = *h->host_state;  // by value: the second poll below overwrites the pinned copy
         h->info_iters = s.iter;
         if (s.breakdown) { status = HISQ_EBREAKDOWN; }
         const bool at_reliable = R > 0 && s.iter > 0 && s.iter % R == 0;

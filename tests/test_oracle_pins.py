@@ -348,3 +348,20 @@ def test_inputs_distributions_and_counter_independence():
     x, y, z, t = inputs.site_coords(L, s)
     assert torch.equal(eta[:, 3], (1 - 2 * ((x + y + z) & 1)).double()) and torch.all(eta[:, 0] == 1)
     assert inputs.fat_links(L, 1, s[:10]).ne(inputs.fat_links(L, 0, s[:10])).all()
+
+
+# ---------------------------------------------------------------- gathered evaluation == rows of D
+def test_dslash_gathered_matches_full_lattice_rows():
+    L = (4, 6, 8, 4)          # Lt = 4: every t-sign case, coinciding hops
+    V = oracle.volume(L)
+    X, W = oracle_links(L, 21)
+    phi = oracle_field(L, 21, 1)[0]
+    sites = np.arange(0, V, 7)
+    plus, minus, t = oracle.neighbour_sites(L, sites)
+    F = np.stack([X, W], axis=1)                                  # [V, 2, 4, 3, 3]
+    f_idx = np.arange(2)[None, :, None]
+    mu_idx = np.arange(4)[None, None, :]
+    Ff = F[sites][:, :, :]                                        # F_mu(x)
+    Fb = F[minus, f_idx, mu_idx]                                  # F_mu(x - hop mu)
+    out = oracle.dslash_gathered(L[3], t, Ff, Fb, phi[plus], phi[minus])
+    assert np.array_equal(out, oracle.dslash(L, X, W, phi)[0][sites])
