@@ -19,7 +19,7 @@ HISQ_MAX_NRHS = 16
 HISQ_ENOCONV, HISQ_EBREAKDOWN = -5, -6
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libhisq.so")
+LIB_PATH = os.environ.get("HISQ_LIB", os.path.join(_HERE, "libhisq.so"))
 
 EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",

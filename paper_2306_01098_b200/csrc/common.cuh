@@ -29,6 +29,7 @@ struct Geom {
     int H;          // Lx / 2 : sites of one parity in an x-row
     int Vh;         // sites of one parity
     int sy, sz, st; // half-index strides of a unit step in y, z, t: H, H*Ly, H*Ly*Lz
+    int stride[4];  // {1, sy, sz, st}: half-index step per unit of (x/2, y, z, t)
     // CTA sweep order: the lattice is cut into (tile_y x tile_z) columns in
     // (y,z); inside a column work runs x fastest, then y, then z, then t; columns are swept last.
     int ty, tz;     // tile extents in y and z (divide Ly, Lz)

@@ -123,30 +123,80 @@ template <typename T> __device__ __forceinline__ void mvdag_acc(const T (&U)[18]
 // One of the 16 stencil terms for all NR right-hand sides.
 //   FWD:  acc += s * F_mu(x) in(x + hop mu)          link owned by the output site (index h, parity par)
 //   !FWD: acc -= s * F_mu(x - hop mu)^+ in(x - hop mu) link owned by the neighbour (index hn, parity 1-par)
-// s = -1 iff the hop crossed the t boundary (`flip`).
-template <typename T, int NR, bool FWD>
+// s = -1 iff the hop crossed the t boundary (`flip`).  The gathered vectors are loaded VB at a time
+// (register budget: 18 reals of link + 6*VB of vectors live beside the 6*NR accumulators).
+template <typename T, int NR, int VB, bool FWD>
 __device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, int Vh, int hn, bool flip,
                                              T (&acc)[NR][6])
 {
     T U[18];
     load_link(blk, Vh, hl, U);
-    T v[NR][6];
-#pragma unroll
-    for (int k = 0; k < NR; ++k) load_vec(in + (size_t)k * 3 * 2 * Vh, Vh, hn, v[k]);
     const bool neg = FWD ? flip : !flip;
 #pragma unroll
-    for (int k = 0; k < NR; ++k) {
-        if (neg) {
+    for (int k0 = 0; k0 < NR; k0 += VB) {
+        T v[VB][6];
 #pragma unroll
-            for (int i = 0; i < 6; ++i) v[k][i] = -v[k][i];
+        for (int j = 0; j < VB; ++j)
+            if (k0 + j < NR) load_vec(in + (size_t)(k0 + j) * 3 * 2 * Vh, Vh, hn, v[j]);
+#pragma unroll
+        for (int j = 0; j < VB; ++j) {
+            if (k0 + j < NR) {
+                if (neg) {
+#pragma unroll
+                    for (int i = 0; i < 6; ++i) v[j][i] = -v[j][i];
+                }
+                if (FWD) mv_acc(U, v[j], acc[k0 + j]);
+                else mvdag_acc(U, v[j], acc[k0 + j]);
+            }
         }
-        if (FWD) mv_acc(U, v[k], acc[k]);
-        else mvdag_acc(U, v[k], acc[k]);
     }
 }
 
+// Kernel shape per NR: small NR are fully unrolled over the 16 terms (ptxas hoists loads across terms; the
+// code still fits the instruction cache); from NR = 3 on the 8 (mu, hop) pairs run as a real loop, because the
+// unrolled body (> 50 KB of SASS at NR = 8) thrashed the instruction cache: `no_instruction` was the second
+// largest stall in the round-1 ncu capture (profiles/r1_dslash_c3_fp32.md).
+#ifndef HISQ_ROLL_FROM
+#define HISQ_ROLL_FROM 99   // NR from which the (mu, hop) loop is rolled; 99 = never (measured slower)
+#endif
+// Tuning knobs (measured on B200): vectors gathered per batch and minimum CTAs per SM
+// (i.e. the register cap) for the 4-RHS and the 6/8-RHS kernels, per precision.
+#ifndef HISQ_F32_VB8
+#define HISQ_F32_VB8 4
+#endif
+#ifndef HISQ_F32_MINB8
+#define HISQ_F32_MINB8 4
+#endif
+#ifndef HISQ_F32_MINB4
+#define HISQ_F32_MINB4 8
+#endif
+#ifndef HISQ_F32_MINB2
+#define HISQ_F32_MINB2 8
+#endif
+#ifndef HISQ_F64_MINB2
+#define HISQ_F64_MINB2 5
+#endif
+#ifndef HISQ_F64_VB8
+#define HISQ_F64_VB8 8
+#endif
+#ifndef HISQ_F64_MINB8
+#define HISQ_F64_MINB8 1
+#endif
+#ifndef HISQ_F64_MINB4
+#define HISQ_F64_MINB4 1
+#endif
+template <typename T, int NR> struct KernelShape {
+    static constexpr bool f32 = sizeof(T) == 4;
+    static constexpr bool rolled = NR >= HISQ_ROLL_FROM;
+    static constexpr int vb8 = f32 ? HISQ_F32_VB8 : HISQ_F64_VB8;
+    static constexpr int vb = NR >= 6 ? (vb8 < NR ? vb8 : NR) : NR;
+    static constexpr int minb = NR >= 6 ? (f32 ? HISQ_F32_MINB8 : HISQ_F64_MINB8)
+                              : NR >= 3 ? (f32 ? HISQ_F32_MINB4 : HISQ_F64_MINB4)
+                              : NR == 2 ? (f32 ? HISQ_F32_MINB2 : HISQ_F64_MINB2) : 1;
+};
+
 template <typename T, int NR, int MODE, int BLOCK>
-__global__ void __launch_bounds__(BLOCK) dslash_kernel(const DslashArgs<T> a)
+__global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel(const DslashArgs<T> a)
 {
     if (a.done != nullptr && *a.done != 0) return;
     const Geom& g = a.g;
@@ -177,25 +227,53 @@ __global__ void __launch_bounds__(BLOCK) dslash_kernel(const DslashArgs<T> a)
         const int x = 2 * xh + ((par + y + z + t) & 1);
         h = xh + H * (y + g.L[1] * (z + g.L[2] * t));
         const int row = h - xh;
-        const int c[4] = { x, y, z, t };
-        const int stride[4] = { 0, g.sy, g.sz, g.st };
+        constexpr int VB = KernelShape<T, NR>::vb;
+        if (!KernelShape<T, NR>::rolled) {
+            const int c[4] = { x, y, z, t };
+            const int stride[4] = { 0, g.sy, g.sz, g.st };
 #pragma unroll
-        for (int mu = 0; mu < 4; ++mu) {
+            for (int mu = 0; mu < 4; ++mu) {
 #pragma unroll
-            for (int f = 0; f < 2; ++f) {
-                const int hop = f ? 3 : 1;
+                for (int f = 0; f < 2; ++f) {
+                    const int hop = f ? 3 : 1;
+                    const int Lmu = g.L[mu];
+                    int cp = c[mu] + hop;
+                    const bool wp = cp >= Lmu;
+                    cp -= wp ? Lmu : 0;
+                    int cm = c[mu] - hop;
+                    const bool wm = cm < 0;
+                    cm += wm ? Lmu : 0;
+                    int hp, hm;
+                    if (mu == 0) { hp = row + (cp >> 1); hm = row + (cm >> 1); }
+                    else { hp = h + (cp - c[mu]) * stride[mu]; hm = h + (cm - c[mu]) * stride[mu]; }
+                    stencil_term<T, NR, VB, true>(link_block(a.links, Vh, f, par, mu), h, in, Vh, hp, mu == 3 && wp, acc);
+                    stencil_term<T, NR, VB, false>(link_block(a.links, Vh, f, 1 - par, mu), hm, in, Vh, hm, mu == 3 && wm, acc);
+                }
+            }
+        } else {
+            const size_t blk_reals = (size_t)Vh * 18;
+#pragma unroll 1
+            for (int i = 0; i < 8; ++i) {
+                const int mu = i >> 1, f = i & 1;
+                const int hop = 1 + 2 * f;
                 const int Lmu = g.L[mu];
-                int cp = c[mu] + hop;
+                const int cmu = mu == 0 ? x : (mu == 1 ? y : (mu == 2 ? z : t));
+                int cp = cmu + hop;
                 const bool wp = cp >= Lmu;
                 cp -= wp ? Lmu : 0;
-                int cm = c[mu] - hop;
+                int cm = cmu - hop;
                 const bool wm = cm < 0;
                 cm += wm ? Lmu : 0;
-                int hp, hm;
-                if (mu == 0) { hp = row + (cp >> 1); hm = row + (cm >> 1); }
-                else { hp = h + (cp - c[mu]) * stride[mu]; hm = h + (cm - c[mu]) * stride[mu]; }
-                stencil_term<T, NR, true>(link_block(a.links, Vh, f, par, mu), h, in, Vh, hp, mu == 3 && wp, acc);
-                stencil_term<T, NR, false>(link_block(a.links, Vh, f, 1 - par, mu), hm, in, Vh, hm, mu == 3 && wm, acc);
+                // in units of the half-index stride: x counts in pairs (two sites of a row share h)
+                const int u = mu == 0 ? xh : cmu;
+                const int up = mu == 0 ? (cp >> 1) : cp;
+                const int um = mu == 0 ? (cm >> 1) : cm;
+                const int sd = g.stride[mu];
+                const int hp = h + (up - u) * sd, hm = h + (um - u) * sd;
+                const T* lf = a.links + (size_t)((f * 2 + par) * 4 + mu) * blk_reals;
+                const T* lb = a.links + (size_t)((f * 2 + (1 - par)) * 4 + mu) * blk_reals;
+                stencil_term<T, NR, VB, true>(lf, h, in, Vh, hp, mu == 3 && wp, acc);
+                stencil_term<T, NR, VB, false>(lb, hm, in, Vh, hm, mu == 3 && wm, acc);
             }
         }
     }

@@ -5,7 +5,10 @@
 
 namespace hisq {
 
-constexpr int kDslashBlock = 128;
+#ifndef HISQ_DSLASH_BLOCK
+#define HISQ_DSLASH_BLOCK 128
+#endif
+constexpr int kDslashBlock = HISQ_DSLASH_BLOCK;
 
 struct LaunchStats { long long launches = 0; };
 
