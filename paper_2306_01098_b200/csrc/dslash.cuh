@@ -105,18 +105,18 @@ template <typename T> __device__ __forceinline__ void mv_acc(const T (&U)[18], c
         }
 }
 
-// acc += U^dagger v       ((U^+)_ab = conj(U_ba))
-template <typename T> __device__ __forceinline__ void mvdag_acc(const T (&U)[18], const T (&v)[6], T (&acc)[6])
+// acc -= U^dagger v       ((U^+)_ab = conj(U_ba))
+template <typename T> __device__ __forceinline__ void mvdag_sub(const T (&U)[18], const T (&v)[6], T (&acc)[6])
 {
 #pragma unroll
     for (int a = 0; a < 3; ++a)
 #pragma unroll
         for (int b = 0; b < 3; ++b) {
             const T ur = U[2 * (3 * b + a)], ui = U[2 * (3 * b + a) + 1];
-            acc[2 * a] = fma(ur, v[2 * b], acc[2 * a]);
-            acc[2 * a] = fma(ui, v[2 * b + 1], acc[2 * a]);
-            acc[2 * a + 1] = fma(ur, v[2 * b + 1], acc[2 * a + 1]);
-            acc[2 * a + 1] = fma(-ui, v[2 * b], acc[2 * a + 1]);
+            acc[2 * a] = fma(-ur, v[2 * b], acc[2 * a]);
+            acc[2 * a] = fma(-ui, v[2 * b + 1], acc[2 * a]);
+            acc[2 * a + 1] = fma(-ur, v[2 * b + 1], acc[2 * a + 1]);
+            acc[2 * a + 1] = fma(ui, v[2 * b], acc[2 * a + 1]);
         }
 }
 
@@ -126,12 +126,18 @@ template <typename T> __device__ __forceinline__ void mvdag_acc(const T (&U)[18]
 // s = -1 iff the hop crossed the t boundary (`flip`).  The gathered vectors are loaded VB at a time
 // (register budget: 18 reals of link + 6*VB of vectors live beside the 6*NR accumulators).
 template <typename T, int NR, int VB, bool FWD>
-__device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, int Vh, int hn, bool flip,
+__device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, int Vh, int hn, bool tdir, bool flip,
                                              T (&acc)[NR][6])
 {
     T U[18];
     load_link(blk, Vh, hl, U);
-    const bool neg = FWD ? flip : !flip;
+    if (tdir) {  // compile-time after unrolling
+        // antiperiodic t: fold the sign into the link (18 multiplies by +-1, branch-free) instead of negating
+        // 6*NR gathered reals or branching; the constant minus of backward terms rides on the FMA operand modifiers
+        const T sgn = flip ? T(-1) : T(1);
+#pragma unroll
+        for (int i = 0; i < 18; ++i) U[i] *= sgn;
+    }
 #pragma unroll
     for (int k0 = 0; k0 < NR; k0 += VB) {
         T v[VB][6];
@@ -141,21 +147,13 @@ __device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, 
 #pragma unroll
         for (int j = 0; j < VB; ++j) {
             if (k0 + j < NR) {
-                if (neg) {
-#pragma unroll
-                    for (int i = 0; i < 6; ++i) v[j][i] = -v[j][i];
-                }
                 if (FWD) mv_acc(U, v[j], acc[k0 + j]);
-                else mvdag_acc(U, v[j], acc[k0 + j]);
+                else mvdag_sub(U, v[j], acc[k0 + j]);
             }
         }
     }
 }
 
-// Kernel shape per NR: small NR are fully unrolled over the 16 terms (ptxas hoists loads across terms; the
-// code still fits the instruction cache); from NR = 3 on the 8 (mu, hop) pairs run as a real loop, because the
-// unrolled body (> 50 KB of SASS at NR = 8) thrashed the instruction cache: `no_instruction` was the second
-// largest stall in the round-1 ncu capture (profiles/r1_dslash_c3_fp32.md).
 #ifndef HISQ_ROLL_FROM
 #define HISQ_ROLL_FROM 99   // NR from which the (mu, hop) loop is rolled; 99 = never (measured slower)
 #endif
@@ -246,8 +244,8 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
                     int hp, hm;
                     if (mu == 0) { hp = row + (cp >> 1); hm = row + (cm >> 1); }
                     else { hp = h + (cp - c[mu]) * stride[mu]; hm = h + (cm - c[mu]) * stride[mu]; }
-                    stencil_term<T, NR, VB, true>(link_block(a.links, Vh, f, par, mu), h, in, Vh, hp, mu == 3 && wp, acc);
-                    stencil_term<T, NR, VB, false>(link_block(a.links, Vh, f, 1 - par, mu), hm, in, Vh, hm, mu == 3 && wm, acc);
+                    stencil_term<T, NR, VB, true>(link_block(a.links, Vh, f, par, mu), h, in, Vh, hp, mu == 3, wp, acc);
+                    stencil_term<T, NR, VB, false>(link_block(a.links, Vh, f, 1 - par, mu), hm, in, Vh, hm, mu == 3, wm, acc);
                 }
             }
         } else {
@@ -272,8 +270,8 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
                 const int hp = h + (up - u) * sd, hm = h + (um - u) * sd;
                 const T* lf = a.links + (size_t)((f * 2 + par) * 4 + mu) * blk_reals;
                 const T* lb = a.links + (size_t)((f * 2 + (1 - par)) * 4 + mu) * blk_reals;
-                stencil_term<T, NR, VB, true>(lf, h, in, Vh, hp, mu == 3 && wp, acc);
-                stencil_term<T, NR, VB, false>(lb, hm, in, Vh, hm, mu == 3 && wm, acc);
+                stencil_term<T, NR, VB, true>(lf, h, in, Vh, hp, true, mu == 3 && wp, acc);
+                stencil_term<T, NR, VB, false>(lb, hm, in, Vh, hm, true, mu == 3 && wm, acc);
             }
         }
     }

@@ -11,6 +11,16 @@ __global__ void rd(const double2* __restrict__ p, size_t n, double* out, int rep
   }
   if(s==1.2345) *out=s;
 }
+// L2-resident read: n is a power of two (elements of 16 B); every thread streams `iters` 4-load groups, wrapping
+// with a mask, so the whole buffer is re-read many times from L2 inside one launch.
+__global__ void rd_l2(const double2* __restrict__ p, unsigned mask, int iters, double* out){
+  unsigned st=gridDim.x*blockDim.x; unsigned i=blockIdx.x*blockDim.x+threadIdx.x; double s=0;
+  for(int k=0;k<iters;k++){
+    double2 a=__ldcg(p+(i&mask)), b=__ldcg(p+((i+st)&mask)), c=__ldcg(p+((i+2*st)&mask)), d=__ldcg(p+((i+3*st)&mask));
+    s+=a.x+a.y+b.x+b.y+c.x+c.y+d.x+d.y; i+=4*st;
+  }
+  if(s==1.2345) *out=s;
+}
 __global__ void cp(const double2* __restrict__ p, double2* __restrict__ q, size_t n){
   size_t i = (size_t)blockIdx.x*blockDim.x+threadIdx.x; size_t st=(size_t)gridDim.x*blockDim.x;
   for(; i<n; i+=st) q[i]=p[i];
@@ -33,9 +43,10 @@ int main(){
   }
   for(int blocks: {148*8,148*32}) { cp<<<blocks,512>>>(p,q,n); cudaEventRecord(e0); for(int r=0;r<5;r++) cp<<<blocks,512>>>(p,q,n); cudaEventRecord(e1); cudaEventSynchronize(e1); cudaEventElapsedTime(&ms,e0,e1);
     printf("copy r+w   blocks=%d : %.1f GB/s\n",blocks, 5.0*2*bytes/ms/1e6); }
-  // L2-resident read: 64 MB
-  { size_t nb=(size_t)64<<20; size_t nn=nb/16; rd<<<148*16,512>>>(p,nn,o,4); cudaEventRecord(e0); rd<<<148*16,512>>>(p,nn,o,50); cudaEventRecord(e1); cudaEventSynchronize(e1); cudaEventElapsedTime(&ms,e0,e1);
-    printf("L2-resident read 64MB : %.1f GB/s\n", 50.0*nb/ms/1e6); }
+  // L2-resident read: 32 MB and 64 MB buffers (power-of-two element counts)
+  for(size_t mb: {32, 64}) { size_t nn=(mb<<20)/16; int blocks=148*8, th=512; int it=2000;
+    rd_l2<<<blocks,th>>>(p,(unsigned)(nn-1),50,o); cudaEventRecord(e0); rd_l2<<<blocks,th>>>(p,(unsigned)(nn-1),it,o); cudaEventRecord(e1); cudaEventSynchronize(e1); cudaEventElapsedTime(&ms,e0,e1);
+    printf("L2-resident read %zuMB : %.1f GB/s\n", mb, (double)blocks*th*it*64/ms/1e6); }
   int iters=20000;
   fma_k<float><<<148*8,512>>>((float*)o,iters); cudaEventRecord(e0); fma_k<float><<<148*8,512>>>((float*)o,iters); cudaEventRecord(e1); cudaEventSynchronize(e1); cudaEventElapsedTime(&ms,e0,e1);
   printf("fp32 FMA peak: %.1f TFLOP/s\n", 148.0*8*512*8*2*iters/ms/1e9);
