@@ -99,6 +99,14 @@ def aggregate(ms: float, flops: float, dist, device):
     return t.item(), f.item()
 
 
+def ncu_traffic(config: str, prec: str, nrhs: int):
+    """DRAM bytes per launch of the Dslash kernel from the committed ncu capture (profiles/traffic.json), or None."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"{config}:{prec}:{nrhs}")
+    except Exception:
+        return None
+
+
 def dslash_bytes(Vh: int, nrhs: int, w: int) -> int:
     """Algorithmic (compulsory) bytes of one Dslash application: 16 links of 18 reals per output site,
     each input and each output site's colour vector once: (288 + 12 n) words per site."""
@@ -294,7 +302,8 @@ def main():
                "true_rel_resid": info["true_rel_resid"], "ms_per_iteration": ms_all / args.steps / max(info["iterations"], 1)},
         "dslash": dsl,
         "roofline": {"bound": "hbm", "kernel": f"dslash_kernel<{'float' if w == 4 else 'double'},NR={min(n, 8 if w == 4 else 4)}>",
-                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": ncu_traffic(args.config, cfg["prec"], n),
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
                      "timing": f"CUDA events around {2 * args.dslash_reps} back-to-back launches (alternating parity), burst"},
         "e2e": {"value": e2e_val, "unit": "GFLOP/s", "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": field_bytes,

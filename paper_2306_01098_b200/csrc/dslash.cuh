@@ -131,13 +131,20 @@ __device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, 
 {
     T U[18];
     load_link(blk, Vh, hl, U);
-    if (tdir) {  // compile-time after unrolling
-        // antiperiodic t: fold the sign into the link (18 multiplies by +-1, branch-free) instead of negating
-        // 6*NR gathered reals or branching; the constant minus of backward terms rides on the FMA operand modifiers
+#if HISQ_SIGN_BRANCH
+    if (tdir && flip) {
+        // antiperiodic t: the whole CTA shares t (blockIdx.y), so `flip` is block-uniform: a real branch, taken only
+        // by the CTAs next to the t boundary, negates the 18 link registers (instead of 6*NR gathered reals)
+#pragma unroll
+        for (int i = 0; i < 18; ++i) U[i] = -U[i];
+    }
+#else
+    if (tdir) {
         const T sgn = flip ? T(-1) : T(1);
 #pragma unroll
         for (int i = 0; i < 18; ++i) U[i] *= sgn;
     }
+#endif
 #pragma unroll
     for (int k0 = 0; k0 < NR; k0 += VB) {
         T v[VB][6];
@@ -154,13 +161,25 @@ __device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, 
     }
 }
 
-#ifndef HISQ_ROLL_FROM
-#define HISQ_ROLL_FROM 99   // NR from which the (mu, hop) loop is rolled; 99 = never (measured slower)
+// NR from which the 8 (mu, hop) pairs run as a real loop of HISQ_ROLL_OUTER trips (the rest unrolled inside): the
+// fully unrolled 8-RHS body is > 100 KB of SASS and `no_instruction` became its largest stall (profiles/);
+// fp32 gains from rolling, fp64 does not (measured).
+#ifndef HISQ_F32_ROLL_FROM
+#define HISQ_F32_ROLL_FROM 6
+#endif
+#ifndef HISQ_F64_ROLL_FROM
+#define HISQ_F64_ROLL_FROM 99
+#endif
+#ifndef HISQ_SIGN_BRANCH
+#define HISQ_SIGN_BRANCH 1  // 1: block-uniform branch negates the link at the t boundary; 0: multiply by +-1 always
 #endif
 // Tuning knobs (measured on B200): vectors gathered per batch and minimum CTAs per SM
 // (i.e. the register cap) for the 4-RHS and the 6/8-RHS kernels, per precision.
+#ifndef HISQ_ROLL_OUTER
+#define HISQ_ROLL_OUTER 2    // trips of the real loop when rolled: 2, 4 or 8
+#endif
 #ifndef HISQ_F32_VB8
-#define HISQ_F32_VB8 4
+#define HISQ_F32_VB8 8
 #endif
 #ifndef HISQ_F32_MINB8
 #define HISQ_F32_MINB8 4
@@ -185,7 +204,8 @@ __device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, 
 #endif
 template <typename T, int NR> struct KernelShape {
     static constexpr bool f32 = sizeof(T) == 4;
-    static constexpr bool rolled = NR >= HISQ_ROLL_FROM;
+    static constexpr bool rolled = NR >= (sizeof(T) == 4 ? HISQ_F32_ROLL_FROM : HISQ_F64_ROLL_FROM);
+    static constexpr int roll_outer = HISQ_ROLL_OUTER;
     static constexpr int vb8 = f32 ? HISQ_F32_VB8 : HISQ_F64_VB8;
     static constexpr int vb = NR >= 6 ? (vb8 < NR ? vb8 : NR) : NR;
     static constexpr int minb = NR >= 6 ? (f32 ? HISQ_F32_MINB8 : HISQ_F64_MINB8)
@@ -250,28 +270,33 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
             }
         } else {
             const size_t blk_reals = (size_t)Vh * 18;
+            constexpr int NO = KernelShape<T, NR>::roll_outer;   // outer (real) loop trips; 8/NO (mu,hop) pairs unrolled inside
 #pragma unroll 1
-            for (int i = 0; i < 8; ++i) {
-                const int mu = i >> 1, f = i & 1;
-                const int hop = 1 + 2 * f;
-                const int Lmu = g.L[mu];
-                const int cmu = mu == 0 ? x : (mu == 1 ? y : (mu == 2 ? z : t));
-                int cp = cmu + hop;
-                const bool wp = cp >= Lmu;
-                cp -= wp ? Lmu : 0;
-                int cm = cmu - hop;
-                const bool wm = cm < 0;
-                cm += wm ? Lmu : 0;
-                // in units of the half-index stride: x counts in pairs (two sites of a row share h)
-                const int u = mu == 0 ? xh : cmu;
-                const int up = mu == 0 ? (cp >> 1) : cp;
-                const int um = mu == 0 ? (cm >> 1) : cm;
-                const int sd = g.stride[mu];
-                const int hp = h + (up - u) * sd, hm = h + (um - u) * sd;
-                const T* lf = a.links + (size_t)((f * 2 + par) * 4 + mu) * blk_reals;
-                const T* lb = a.links + (size_t)((f * 2 + (1 - par)) * 4 + mu) * blk_reals;
-                stencil_term<T, NR, VB, true>(lf, h, in, Vh, hp, true, mu == 3 && wp, acc);
-                stencil_term<T, NR, VB, false>(lb, hm, in, Vh, hm, true, mu == 3 && wm, acc);
+            for (int o = 0; o < NO; ++o) {
+#pragma unroll
+                for (int q = 0; q < 8 / NO; ++q) {
+                    const int i = o * (8 / NO) + q;
+                    const int mu = i >> 1, f = i & 1;
+                    const int hop = 1 + 2 * f;
+                    const int Lmu = g.L[mu];
+                    const int cmu = mu == 0 ? x : (mu == 1 ? y : (mu == 2 ? z : t));
+                    int cp = cmu + hop;
+                    const bool wp = cp >= Lmu;
+                    cp -= wp ? Lmu : 0;
+                    int cm = cmu - hop;
+                    const bool wm = cm < 0;
+                    cm += wm ? Lmu : 0;
+                    // in units of the half-index stride: x counts in pairs (two sites of a row share h)
+                    const int u = mu == 0 ? xh : cmu;
+                    const int up = mu == 0 ? (cp >> 1) : cp;
+                    const int um = mu == 0 ? (cm >> 1) : cm;
+                    const int sd = g.stride[mu];
+                    const int hp = h + (up - u) * sd, hm = h + (um - u) * sd;
+                    const T* lf = a.links + (size_t)((f * 2 + par) * 4 + mu) * blk_reals;
+                    const T* lb = a.links + (size_t)((f * 2 + (1 - par)) * 4 + mu) * blk_reals;
+                    stencil_term<T, NR, VB, true>(lf, h, in, Vh, hp, mu == 3, wp, acc);
+                    stencil_term<T, NR, VB, false>(lb, hm, in, Vh, hm, mu == 3, wm, acc);
+                }
             }
         }
     }
