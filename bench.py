@@ -198,6 +198,7 @@ def main():
     ap.add_argument("--nrhs", type=int, default=0, help="override the config's nRHS (--only dslash)")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-multishift", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--ref-budget", type=float, default=10.0)
     ap.add_argument("--dslash-reps", type=int, default=100)
@@ -289,6 +290,26 @@ def main():
     dsl = {"ms": d_ms, "gflops": FLOP_PER_SITE * Vh * n / (d_ms * 1e-3) / 1e9, "alg_gbs": achieved,
            "paper_model_gbs": (288 + 102 * n) * w * Vh / (d_ms * 1e-3) / 1e9,
            "frac_of_measured_copy": achieved / peak, "frac_of_8TBs": achieved / 8000.0, "tiles": ctx.tiles(n)}
+    # ---- row f1: multi-shift CG on the same lattice (10 shifts over 5 decades), one solve ----
+    ms = None
+    if not args.no_multishift and cfg["prec"] != "mixed" and n == 1:
+        import numpy as np
+        shifts = [0.0] + [float(v) for v in np.geomspace(1e-4, 5.0, 9)]
+        ctx.close()
+        ctx = binding.Hisq(L, cfg["prec"], len(shifts), dev)
+        fat, naik = binding.make_links(L, rank, dev, ctx.cdtype, gen_device=gen_dev)
+        ctx.set_links(fat, naik)
+        del fat, naik
+        xs = ctx.new_field(len(shifts))
+        ctx.cg_multishift(b, cfg["mass"], shifts, cfg["tol"], x=xs)
+        torch.cuda.synchronize()
+        e0.record()
+        _, mi = ctx.cg_multishift(b, cfg["mass"], shifts, cfg["tol"], x=xs)
+        e1.record()
+        e1.synchronize()
+        ms = {"shifts": len(shifts), "solve_ms": e0.elapsed_time(e1), "iterations": mi["iterations"],
+              "ms_per_iteration": e0.elapsed_time(e1) / max(mi["iterations"], 1), "max_true_rel_resid": max(mi["true_rel_resid"])}
+        del xs
     ctx.close()
     del ctx, b, x
 
@@ -301,6 +322,7 @@ def main():
         "cg": {"solve_ms": ms_all / args.steps, "iterations": info["iterations"], "true_residual_checks": info["reliable_updates"],
                "true_rel_resid": info["true_rel_resid"], "ms_per_iteration": ms_all / args.steps / max(info["iterations"], 1)},
         "dslash": dsl,
+        "multishift_cg": ms,
         "roofline": {"bound": "hbm", "kernel": f"dslash_kernel<{'float' if w == 4 else 'double'},NR={min(n, 8 if w == 4 else 4)}>",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": ncu_traffic(args.config, cfg["prec"], n),

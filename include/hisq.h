@@ -96,6 +96,16 @@ int hisq_dslash(hisq_ctx *h, void *out, const void *in, int parity, int nrhs);
  * Returns after the solve has finished (synchronises the stream).  HISQ_ENOCONV / HISQ_EBREAKDOWN as above. */
 int hisq_cg(hisq_ctx *h, void *x, const void *b, double mass, double tol, int nrhs);
 
+/* Multi-shift CG (AdvancedMultiShiftCG): solve (mass^2 + shifts[k] - D_eo D_oe) x_k = b for nshift
+ * shifts sigma_k >= 0 (HOST array) and ONE right-hand side b, with one operator application per iteration (on the
+ * smallest shift; the Krylov space is shift invariant, the other solutions cost extra AXPYs only).
+ * b: one NATIVE even half-lattice field; x: nshift NATIVE fields, x_k at offset k*3*Vh complex, overwritten.
+ * nshift <= the nrhs the workspace was sized for.  Each shift stops when |zeta_k| ||r|| <= tol ||b|| / 2 (the
+ * factor 2 is a margin for the drift of the recursive residual) and is frozen; afterwards the true residuals
+ * ||b - (A + sigma_k) x_k|| / ||b|| are recomputed (hisq_get_info) and HISQ_ENOCONV is returned if one exceeds tol.
+ * HISQ_FP64 and HISQ_FP32 contexts only (HISQ_MIXED: HISQ_EINVAL). */
+int hisq_cg_multishift(hisq_ctx *h, void *x, const void *b, double mass, const double *shifts, int nshift, double tol);
+
 /* Options: "max_iter" (default 100000), "reliable_interval" (default 100 for HISQ_MIXED, 0 = off for
  * the others), "check_interval" (iterations enqueued between host polls of the convergence flag,
  * default 32), "use_graph" (1: replay one CG iteration as a CUDA graph, default 1),

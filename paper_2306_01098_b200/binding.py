@@ -23,7 +23,7 @@ LIB_PATH = os.environ.get("HISQ_LIB", os.path.join(_HERE, "libhisq.so"))
 
 EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
-    "hisq_set_links", "hisq_dslash", "hisq_cg", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
+    "hisq_set_links", "hisq_dslash", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
     "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_launch_count", "hisq_strerror",
     "hisq_last_error",
 ]
@@ -56,6 +56,7 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_set_links.argtypes = [vp, vp, vp]
     lib.hisq_dslash.argtypes = [vp, vp, vp, i, i]
     lib.hisq_cg.argtypes = [vp, vp, vp, d, d, i]
+    lib.hisq_cg_multishift.argtypes = [vp, vp, vp, d, ctypes.POINTER(d), i, d]
     lib.hisq_set_option.argtypes = [vp, ctypes.c_char_p, d]
     lib.hisq_get_info.argtypes = [vp, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(d)]
     lib.hisq_spinor_pack.argtypes = [vp, vp, vp, i]
@@ -180,6 +181,18 @@ class Hisq:
                                 float(mass), float(tol), n)
         self._check(code, allow=() if strict else (HISQ_ENOCONV, HISQ_EBREAKDOWN))
         return x, self.info(n, code)
+
+    def cg_multishift(self, b: torch.Tensor, mass: float, shifts, tol: float, x: Optional[torch.Tensor] = None,
+                      strict: bool = True):
+        """(mass^2 + shifts[k] - D_eo D_oe) x_k = b; b: [1, 3, Vh]; returns (x [nshift, 3, Vh], info)."""
+        ns = len(shifts)
+        if x is None:
+            x = self.new_field(ns)
+        arr = (ctypes.c_double * ns)(*[float(v) for v in shifts])
+        code = self.lib.hisq_cg_multishift(self._h, self._ptr(x, (ns, 3, self.Vh), self.cdtype),
+                                           self._ptr(b, (1, 3, self.Vh), self.cdtype), float(mass), arr, ns, float(tol))
+        self._check(code, allow=() if strict else (HISQ_ENOCONV, HISQ_EBREAKDOWN))
+        return x, self.info(ns, code)
 
     def info(self, nrhs: int, status: int = 0) -> dict:
         it, rel = ctypes.c_int(0), ctypes.c_int(0)

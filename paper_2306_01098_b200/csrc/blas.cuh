@@ -273,3 +273,163 @@ __global__ void __launch_bounds__(256) link_repack_kernel(const TS* __restrict__
 }
 
 }  // namespace hisq
+
+// ===== multi-shift CG (row f1; PAPER.md:141 AdvancedMultiShiftCG): (A + sigma_k) x_k = b for all k with ONE
+// operator application per iteration, on the smallest shift; the other shifts cost only these AXPYs. ==========
+namespace hisq {
+
+// zeta_k^{n+1} from the three-term recurrences of the base and the shifted system (derivation in DESIGN.md):
+//   zeta' = zeta zeta_prev alpha_old / ( alpha_old zeta_prev (1 + delta alpha) + alpha beta_old (zeta_prev - zeta) )
+__device__ __forceinline__ double ms_zeta_next(double zeta, double zeta_prev, double alpha, double alpha_old, double beta_old,
+                                               double delta)
+{
+    const double den = alpha_old * zeta_prev * (1.0 + delta * alpha) + alpha * beta_old * (zeta_prev - zeta);
+    return zeta * zeta_prev * alpha_old / den;
+}
+
+// start: r = b, x_k = 0 and p_k = 0 are memset by the host; rho = ||b||^2
+template <typename T>
+__global__ void __launch_bounds__(kBlasBlock) ms_init_kernel(const T* __restrict__ b, T* __restrict__ r, size_t nreal, CgState* st,
+                                                             double* partial, double tol, int max_iter, int nshift)
+{
+    double sum[1] = { 0.0 };
+    for (int it = 0; it < kBlasItems * 4; ++it) {
+        size_t i = ((size_t)blockIdx.x * kBlasItems * 4 + it) * kBlasBlock + threadIdx.x;
+        if (i < nreal) {
+            T v = b[i];
+            r[i] = v;
+            sum[0] += (double)v * (double)v;
+        }
+    }
+    __shared__ double totals[kMaxNrhs];
+    if (grid_reduce<1, kBlasBlock>(sum, 0, partial, gridDim.x, blockIdx.x, &st->ticket[0], gridDim.x, 1, totals)) {
+        if (threadIdx.x == 0) {
+            const double bb = totals[0];
+            st->rho[0] = bb; st->rho_prev[0] = bb; st->bnorm2[0] = bb; st->pq[0] = 1.0; st->beta[0] = 0.0;
+            for (int k = 0; k < nshift; ++k) {
+                st->ms_zeta[k] = 1.0; st->ms_zeta_prev[k] = 1.0; st->ms_beta_k[k] = 0.0;
+                st->active[k] = bb > 0.0 ? 1 : 0;
+                st->bnorm2[k] = bb;
+            }
+            st->ms_alpha_old = 1.0; st->ms_beta_old = 0.0; st->ms_nshift = nshift;
+            st->tol2 = tol * tol; st->iter = 0; st->max_iter = max_iter; st->breakdown = 0; st->nrhs = nshift;
+            st->done = bb > 0.0 ? 0 : 1;
+        }
+    }
+}
+
+// p_k = zeta_k r + beta_k p_k   (blockIdx.y = shift k)
+template <typename T>
+__global__ void __launch_bounds__(kBlasBlock) ms_update_p_kernel(T* __restrict__ p, const T* __restrict__ r, size_t nreal,
+                                                                 const CgState* st)
+{
+    if (st->done) return;
+    using V = typename V16<T>::type;
+    constexpr int N = V16<T>::n;
+    const int k = blockIdx.y;
+    if (!st->active[k]) return;
+    const T zeta = (T)st->ms_zeta[k], beta = (T)st->ms_beta_k[k];
+    const size_t nvec = nreal / N;
+    V* pv = reinterpret_cast<V*>(p + (size_t)k * nreal);
+    const V* rv = reinterpret_cast<const V*>(r);
+#pragma unroll
+    for (int it = 0; it < kBlasItems; ++it) {
+        size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
+        if (i < nvec) {
+            T a[N], b[N];
+            unpack16<T>(rv[i], a); unpack16<T>(pv[i], b);
+#pragma unroll
+            for (int e = 0; e < N; ++e) b[e] = fma(beta, b[e], zeta * a[e]);
+            pv[i] = pack16<T>(b);
+        }
+    }
+}
+
+// blockIdx.y < nshift: x_k += alpha_k p_k with alpha_k = alpha zeta_k^{n+1} / zeta_k^n
+// blockIdx.y == nshift: r -= alpha q, rho' = ||r||^2; the last block advances every scalar recurrence
+template <typename T>
+__global__ void __launch_bounds__(kBlasBlock) ms_update_xr_kernel(T* __restrict__ x, T* __restrict__ r, const T* __restrict__ p,
+                                                                  const T* __restrict__ q, size_t nreal, CgState* st, double* partial)
+{
+    if (st->done) return;
+    using V = typename V16<T>::type;
+    constexpr int N = V16<T>::n;
+    const int nshift = gridDim.y - 1;
+    const int k = blockIdx.y;
+    const double pq = st->pq[0];
+    const bool ok = pq > 0.0 && isfinite(pq);
+    const double alpha = ok ? st->rho[0] / pq : 0.0;
+    const double alpha_old = st->ms_alpha_old, beta_old = st->ms_beta_old;
+    const size_t nvec = nreal / N;
+    double sum[1] = { 0.0 };
+    if (k < nshift) {
+        if (st->active[k]) {
+            const double z = st->ms_zeta[k];
+            const double zn = ms_zeta_next(z, st->ms_zeta_prev[k], alpha, alpha_old, beta_old, st->ms_delta[k]);
+            const T ak = (T)(alpha * zn / z);
+            V* xv = reinterpret_cast<V*>(x + (size_t)k * nreal);
+            const V* pv = reinterpret_cast<const V*>(p + (size_t)k * nreal);
+#pragma unroll
+            for (int it = 0; it < kBlasItems; ++it) {
+                size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
+                if (i < nvec) {
+                    T a[N], b[N];
+                    unpack16<T>(xv[i], a); unpack16<T>(pv[i], b);
+#pragma unroll
+                    for (int e = 0; e < N; ++e) a[e] = fma(ak, b[e], a[e]);
+                    xv[i] = pack16<T>(a);
+                }
+            }
+        }
+    } else {
+        const T al = (T)alpha;
+        V* rv = reinterpret_cast<V*>(r);
+        const V* qv = reinterpret_cast<const V*>(q);
+#pragma unroll
+        for (int it = 0; it < kBlasItems; ++it) {
+            size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
+            if (i < nvec) {
+                T a[N], b[N];
+                unpack16<T>(rv[i], a); unpack16<T>(qv[i], b);
+#pragma unroll
+                for (int e = 0; e < N; ++e) {
+                    a[e] = fma(-al, b[e], a[e]);
+                    sum[0] += (double)a[e] * (double)a[e];
+                }
+                rv[i] = pack16<T>(a);
+            }
+        }
+    }
+    __shared__ double totals[kMaxNrhs];
+    // row 0 of `partial` collects the residual norm; x-blocks contribute zeros to their own rows (never summed)
+    if (grid_reduce<1, kBlasBlock>(sum, k < nshift ? 1 : 0, partial, gridDim.x, blockIdx.x, &st->ticket[1], gridDim.x * gridDim.y,
+                                   1, totals)) {
+        if (threadIdx.x == 0) {
+            const double rn = totals[0];
+            if (!ok || !isfinite(rn)) st->breakdown = 1;
+            const double beta = rn / st->rho[0];
+            int any = 0;
+            for (int s = 0; s < nshift; ++s) {
+                if (!st->active[s]) continue;
+                const double z = st->ms_zeta[s];
+                const double zn = ms_zeta_next(z, st->ms_zeta_prev[s], alpha, alpha_old, beta_old, st->ms_delta[s]);
+                st->ms_beta_k[s] = beta * (zn / z) * (zn / z);
+                st->ms_zeta_prev[s] = z;
+                st->ms_zeta[s] = zn;
+                if (!isfinite(zn)) st->breakdown = 1;
+                // ||r_s|| = |zeta_s| ||r||; stop at half the requested tolerance (recursion drift margin)
+                if (zn * zn * rn <= 0.25 * st->tol2 * st->bnorm2[0]) st->active[s] = 0;
+                any |= st->active[s];
+            }
+            st->rho_prev[0] = st->rho[0];
+            st->rho[0] = rn;
+            st->ms_alpha_old = alpha;
+            st->ms_beta_old = beta;
+            const int it = st->iter + 1;
+            st->iter = it;
+            if (!any || it >= st->max_iter || st->breakdown) st->done = 1;
+        }
+    }
+}
+
+}  // namespace hisq

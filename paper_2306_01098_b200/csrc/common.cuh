@@ -52,6 +52,13 @@ struct CgState {
     int breakdown;
     int nrhs;
     unsigned ticket[4];        // last-block tickets of the reducing kernels
+    // multi-shift CG: shifted residuals stay collinear, r_k = zeta_k r
+    double ms_delta[kMaxNrhs];     // sigma_k - sigma_min
+    double ms_zeta[kMaxNrhs];      // zeta_k^n
+    double ms_zeta_prev[kMaxNrhs]; // zeta_k^{n-1}
+    double ms_beta_k[kMaxNrhs];    // beta_k^n = beta_n (zeta^{n+1}/zeta^n)^2
+    double ms_alpha_old, ms_beta_old;
+    int ms_nshift;
 };
 
 // ---- deterministic two-stage reduction: block partials, then the last block to finish sums them ---

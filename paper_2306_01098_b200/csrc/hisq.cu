@@ -471,6 +471,132 @@ static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_u
     return status;
 }
 
+// ---- multi-shift CG (row f1): (A + sigma_k) x_k = b, one operator application per iteration -----------------
+template <typename T>
+static int ms_enqueue_iteration(hisq_ctx* h, const T* links, T* x, T* r, T* p, T* q, T* t, double m2_base, int kmin, int nshift)
+{
+    const size_t nreal = (size_t)6 * h->g.Vh;
+    const unsigned gx = (unsigned)blas_grid_x(nreal, V16<T>::n);
+    ms_update_p_kernel<T><<<dim3(gx, (unsigned)nshift), kBlasBlock, 0, h->stream>>>(p, r, nreal, h->state);
+    h->stats.launches++;
+    T* pb = p + (size_t)kmin * nreal;   // the base direction: the smallest shift has zeta = 1
+    int rc = run_dslash<T>(h, links, t, pb, HISQ_ODD, 1, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, &h->state->done, 2);
+    if (rc) return rc;
+    rc = run_dslash<T>(h, links, q, t, HISQ_EVEN, 1, MODE_APPLY_A, pb, nullptr, m2_base, h->state->pq, &h->state->done, 2);
+    if (rc) return rc;
+    ms_update_xr_kernel<T><<<dim3(gx, (unsigned)nshift + 1), kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+
+template <typename T>
+static int ms_solve(hisq_ctx* h, const T* links, T* x, const T* b, double mass, const double* shifts, int nshift, double tol)
+{
+    const size_t nreal = (size_t)6 * h->g.Vh;
+    const size_t fb = field_bytes(h, h->ws_nrhs, sizeof(T));
+    T* r = (T*)(h->fields);
+    T* p = (T*)(h->fields + fb);
+    T* q = (T*)(h->fields + 2 * fb);
+    T* t = (T*)(h->fields + 3 * fb);
+    int kmin = 0;
+    for (int k = 1; k < nshift; ++k)
+        if (shifts[k] < shifts[kmin]) kmin = k;
+    const double m2_base = mass * mass + shifts[kmin];
+    h->info_iters = 0; h->info_reliable = 0;
+    CK(cudaMemsetAsync(x, 0, nreal * nshift * sizeof(T), h->stream));
+    CK(cudaMemsetAsync(p, 0, nreal * nshift * sizeof(T), h->stream));
+    ms_init_kernel<T><<<(unsigned)init_grid_x(nreal), kBlasBlock, 0, h->stream>>>(b, r, nreal, h->state, h->partial, tol,
+                                                                                   h->max_iter, nshift);
+    h->stats.launches++;
+    double delta[kMaxNrhs];
+    for (int k = 0; k < nshift; ++k) delta[k] = shifts[k] - shifts[kmin];
+    CK(cudaMemcpyAsync(h->state->ms_delta, delta, nshift * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));   // `delta` is a stack array
+
+    const int batch = h->check_interval > 0 ? h->check_interval : 32;
+    cudaGraphExec_t exec = nullptr;
+    long long launches_per_batch = 0;
+    int rc = HISQ_OK, status = HISQ_OK, cur = 0;
+    bool pending = false;
+    while (true) {
+        if (h->use_graph) {
+            if (!exec) {
+                cudaGraph_t graph;
+                const long long l0 = h->stats.launches;
+                if (!h->cap_stream) CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+                cudaStream_t user_stream = h->stream;
+                CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+                h->stream = h->cap_stream;
+                for (int i = 0; i < batch && rc == HISQ_OK; ++i) rc = ms_enqueue_iteration<T>(h, links, x, r, p, q, t, m2_base, kmin, nshift);
+                h->stream = user_stream;
+                cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
+                if (rc != HISQ_OK) { if (ce == cudaSuccess) cudaGraphDestroy(graph); break; }
+                if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaStreamEndCapture"); break; }
+                ce = cudaGraphInstantiate(&exec, graph, 0);
+                cudaGraphDestroy(graph);
+                if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaGraphInstantiate"); break; }
+                launches_per_batch = h->stats.launches - l0;
+                h->stats.launches = l0;
+            }
+            cudaError_t ce = cudaGraphLaunch(exec, h->stream);
+            if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaGraphLaunch"); break; }
+            h->stats.launches += launches_per_batch;
+        } else {
+            for (int i = 0; i < batch && rc == HISQ_OK; ++i) rc = ms_enqueue_iteration<T>(h, links, x, r, p, q, t, m2_base, kmin, nshift);
+            if (rc != HISQ_OK) break;
+        }
+        if ((rc = poll_async(h, cur)) != HISQ_OK) break;
+        if (!pending) { pending = true; cur ^= 1; continue; }
+        const CgState* sp = poll_wait(h, cur ^ 1);
+        if (!sp) { rc = cuda_fail(h, cudaGetLastError(), "cudaEventSynchronize"); break; }
+        if (!sp->done) { cur ^= 1; continue; }
+        sp = poll_wait(h, cur);
+        if (!sp) { rc = cuda_fail(h, cudaGetLastError(), "cudaEventSynchronize"); break; }
+        h->info_iters = sp->iter;
+        if (sp->breakdown) status = HISQ_EBREAKDOWN;
+        else {
+            for (int k = 0; k < nshift; ++k)
+                if (sp->active[k]) status = HISQ_ENOCONV;
+        }
+        break;
+    }
+    if (exec) cudaGraphExecDestroy(exec);
+    if (rc != HISQ_OK) return rc;
+    // true residuals ||b - (A + sigma_k) x_k|| / ||b|| per shift (q and t are free now)
+    for (int k = 0; k < nshift; ++k) {
+        const double m2k = mass * mass + shifts[k];
+        T* xk = x + (size_t)k * nreal;
+        rc = run_dslash<T>(h, links, t, xk, HISQ_ODD, 1, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, nullptr, 2);
+        if (rc) return rc;
+        rc = run_dslash<T>(h, links, q, t, HISQ_EVEN, 1, MODE_RESID, xk, b, m2k, h->state->sums + k, nullptr, 2);
+        if (rc) return rc;
+    }
+    if ((rc = poll_state(h)) != HISQ_OK) return rc;
+    const CgState& s = *h->host_state;
+    for (int k = 0; k < nshift; ++k) {
+        h->info_relres[k] = s.bnorm2[0] > 0.0 ? std::sqrt(s.sums[k] / s.bnorm2[0]) : 0.0;
+        if (status == HISQ_OK && !(h->info_relres[k] <= tol)) status = HISQ_ENOCONV;
+    }
+    return status;
+}
+
+extern "C" int hisq_cg_multishift(hisq_ctx* h, void* x, const void* b, double mass, const double* shifts, int nshift, double tol)
+{
+    if (!h || !x || !b || !shifts || nshift < 1 || nshift > HISQ_MAX_NRHS || !(tol > 0.0) || !std::isfinite(mass)) return HISQ_EINVAL;
+    if (((uintptr_t)x & 15) || ((uintptr_t)b & 15)) return HISQ_EINVAL;
+    for (int k = 0; k < nshift; ++k)
+        if (!(shifts[k] >= 0.0) || !std::isfinite(shifts[k])) return HISQ_EINVAL;
+    if (h->prec == HISQ_MIXED) return HISQ_EINVAL;   // fp64 or fp32 contexts only
+    if (!h->ws) return HISQ_ENOWORKSPACE;
+    if (nshift > h->ws_nrhs) return HISQ_ENOWORKSPACE;
+    if (!h->have_links) return HISQ_ENOLINKS;
+    const size_t bytes = (size_t)6 * h->g.Vh * elem_size(h->prec);
+    if ((const char*)x < (const char*)b + bytes && (const char*)b < (const char*)x + bytes * nshift) return HISQ_EINVAL;
+    if (h->prec == HISQ_FP32) return ms_solve<float>(h, h->links32, (float*)x, (const float*)b, mass, shifts, nshift, tol);
+    return ms_solve<double>(h, h->links64, (double*)x, (const double*)b, mass, shifts, nshift, tol);
+}
+
 extern "C" int hisq_cg(hisq_ctx* h, void* x, const void* b, double mass, double tol, int nrhs)
 {
     if (!h || !x || !b || nrhs < 1 || nrhs > HISQ_MAX_NRHS || !(tol > 0.0) || !std::isfinite(mass)) return HISQ_EINVAL;

@@ -365,3 +365,16 @@ def test_dslash_gathered_matches_full_lattice_rows():
     Fb = F[minus, f_idx, mu_idx]                                  # F_mu(x - hop mu)
     out = oracle.dslash_gathered(L[3], t, Ff, Fb, phi[plus], phi[minus])
     assert np.array_equal(out, oracle.dslash(L, X, W, phi)[0][sites])
+
+
+# ---------------------------------------------------------------- shifted systems (multi-shift CG's targets)
+def test_shifted_system_is_a_mass_shift_dense_check():
+    """(A + sigma) = (m^2 + sigma) - D_eo D_oe: the oracle CG at mass sqrt(m^2 + sigma) solves the shifted system;
+    pinned against a dense solve of A_ee + sigma on 4^4."""
+    L, m, sigma = (4, 4, 4, 4), 0.1, 0.37
+    X, W = oracle_links(L, 31)
+    A, rows_e = dense.dense_A_even(L, X, W, m)
+    b = oracle_field(L, 31, 1, parity=0)
+    xd = np.linalg.solve(A + sigma * np.eye(A.shape[0]), b[0].reshape(-1)[rows_e])
+    x, _, _, st, _ = oracle.cg(L, X, W, float(np.sqrt(m * m + sigma)), 1e-12, b)
+    assert st == 0 and rel_l2(x[0].reshape(-1)[rows_e], xd) < 1e-10
