@@ -199,6 +199,7 @@ def main():
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-multishift", action="store_true")
+    ap.add_argument("--no-compression", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--ref-budget", type=float, default=10.0)
     ap.add_argument("--dslash-reps", type=int, default=100)
@@ -290,6 +291,30 @@ def main():
     dsl = {"ms": d_ms, "gflops": FLOP_PER_SITE * Vh * n / (d_ms * 1e-3) / 1e9, "alg_gbs": achieved,
            "paper_model_gbs": (288 + 102 * n) * w * Vh / (d_ms * 1e-3) / 1e9,
            "frac_of_measured_copy": achieved / peak, "frac_of_8TBs": achieved / 8000.0, "tiles": ctx.tiles(n)}
+    # ---- row f2: the same Dslash and solve with compressed Naik links (13 instead of 18 reals per Naik link) ----
+    comp = None
+    if not args.no_compression:
+        ctx.close()
+        ctx = binding.Hisq(L, cfg["prec"], n, dev)
+        ctx.set_option("naik_compress", 1)
+        fat, naik = binding.make_links(L, rank, dev, ctx.cdtype, gen_device=gen_dev)
+        ctx.set_links(fat, naik)
+        del fat, naik
+        if ctx.naik_compressed():
+            c_ms = time_dslash(ctx, n, args.dslash_reps)
+            ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
+            torch.cuda.synchronize()
+            e0.record()
+            _, ci = ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
+            e1.record()
+            e1.synchronize()
+            stored = (8 * 18 + 8 * 13 + 12 * n) * w * Vh
+            comp = {"format": "Naik links as 13 reals (rows 0,1 and 1/c), fat links 18", "dslash_ms": c_ms,
+                    "dslash_gflops": FLOP_PER_SITE * Vh * n / (c_ms * 1e-3) / 1e9,
+                    "stored_bytes_per_launch": stored, "stored_gbs": stored / (c_ms * 1e-3) / 1e9,
+                    "uncompressed_alg_gbs": alg_bytes / (c_ms * 1e-3) / 1e9, "speedup_vs_full": d_ms / c_ms,
+                    "cg_solve_ms": e0.elapsed_time(e1), "cg_iterations": ci["iterations"],
+                    "cg_true_rel_resid": ci["true_rel_resid"]}
     # ---- row f1: multi-shift CG on the same lattice (10 shifts over 5 decades), one solve ----
     ms = None
     if not args.no_multishift and cfg["prec"] != "mixed" and n == 1:
@@ -323,6 +348,7 @@ def main():
                "true_rel_resid": info["true_rel_resid"], "ms_per_iteration": ms_all / args.steps / max(info["iterations"], 1)},
         "dslash": dsl,
         "multishift_cg": ms,
+        "naik_compression": comp,
         "roofline": {"bound": "hbm", "kernel": f"dslash_kernel<{'float' if w == 4 else 'double'},NR={min(n, 8 if w == 4 else 4)}>",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": ncu_traffic(args.config, cfg["prec"], n),

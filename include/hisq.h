@@ -110,7 +110,8 @@ int hisq_cg_multishift(hisq_ctx *h, void *x, const void *b, double mass, const d
  * the others), "check_interval" (iterations enqueued between host polls of the convergence flag,
  * default 32), "use_graph" (1: replay one CG iteration as a CUDA graph, default 1),
  * "dslash_block" (threads per CTA of the Dslash kernel, 0 = default), "nrhs_inner" (RHS per thread, 0 = auto),
- * "tile_y", "tile_z" (CTA sweep order blocking in y,z; 0 = auto). */
+ * "tile_y", "tile_z" (CTA sweep order blocking in y,z; 0 = auto),
+ * "naik_compress" (see hisq_naik_compressed; default 0). */
 int hisq_set_option(hisq_ctx *h, const char *key, double value);
 
 /* After hisq_cg: iterations done, number of fp64 true-residual recomputations, and per RHS the true
@@ -125,6 +126,12 @@ int hisq_spinor_unpack(hisq_ctx *h, void *canonical, const void *native, int nrh
  * run, unpack, copy out, synchronise.  Staging lives in the workspace. */
 int hisq_dslash_host(hisq_ctx *h, void *out_host, const void *in_host, int parity, int nrhs);
 int hisq_cg_host(hisq_ctx *h, void *x_host, const void *b_host, double mass, double tol, int nrhs);
+
+/* Row f2 (the paper's CompressionType).  With option "naik_compress" = 1, the next hisq_set_links
+ * stores each Naik link as 13 reals (rows 0, 1 and 1/c of W = c U, U in SU(3), c real; row 2 = conj(row0 x row1)/c is
+ * rebuilt in registers) PROVIDED every Naik link passes |row2 - conj(row0 x row1)/c| <= tol |c| (tol 1e-12 fp64, 1e-5
+ * fp32); otherwise the links stay uncompressed.  Returns 1 if the context currently uses the compressed format. */
+int hisq_naik_compressed(const hisq_ctx *h);
 
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */
 long long hisq_launch_count(const hisq_ctx *h);

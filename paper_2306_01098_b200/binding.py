@@ -24,7 +24,7 @@ LIB_PATH = os.environ.get("HISQ_LIB", os.path.join(_HERE, "libhisq.so"))
 EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
     "hisq_set_links", "hisq_dslash", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
-    "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_launch_count", "hisq_strerror",
+    "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count", "hisq_strerror",
     "hisq_last_error",
 ]
 
@@ -63,6 +63,7 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_spinor_unpack.argtypes = [vp, vp, vp, i]
     lib.hisq_dslash_host.argtypes = [vp, vp, vp, i, i]
     lib.hisq_cg_host.argtypes = [vp, vp, vp, d, d, i]
+    lib.hisq_naik_compressed.argtypes = [vp]
     lib.hisq_launch_count.argtypes = [vp]
     lib.hisq_launch_count.restype = ctypes.c_longlong
     lib.hisq_strerror.argtypes = [i]
@@ -220,6 +221,9 @@ class Hisq:
                                      float(mass), float(tol), n)
         self._check(code, allow=() if strict else (HISQ_ENOCONV, HISQ_EBREAKDOWN))
         return x_host, self.info(n, code)
+
+    def naik_compressed(self) -> bool:
+        return bool(self.lib.hisq_naik_compressed(self._h))
 
     def launch_count(self) -> int:
         return int(self.lib.hisq_launch_count(self._h))

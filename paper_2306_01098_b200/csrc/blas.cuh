@@ -12,7 +12,10 @@
 namespace hisq {
 
 constexpr int kBlasBlock = 256;
-constexpr int kBlasItems = 4;  // 16-byte vectors per thread
+#ifndef HISQ_BLAS_ITEMS
+#define HISQ_BLAS_ITEMS 4
+#endif
+constexpr int kBlasItems = HISQ_BLAS_ITEMS;  // 16-byte vectors per thread
 
 template <typename T> struct V16;
 template <> struct V16<double> { using type = double2; static constexpr int n = 2; };
@@ -269,6 +272,92 @@ __global__ void __launch_bounds__(256) link_repack_kernel(const TS* __restrict__
             for (int i = 0; i < 4; ++i) blk[((size_t)j * Vh + h) * 4 + i] = e[4 * j + i];
         blk[(size_t)16 * Vh + (size_t)h * 2] = e[16];
         blk[(size_t)16 * Vh + (size_t)h * 2 + 1] = e[17];
+    }
+}
+
+// ---- Naik-link compression (row f2; the paper's `CompressionType comp`) -----------------
+// A Naik link of the HISQ action is a real multiple of an SU(3) matrix, W = c U (here c = -eta/24).  Store rows 0
+// and 1 (12 reals) and 1/c (1 real): row 2 = conj(row0 x row1) / c.  13 instead of 18 reals per Naik link.
+// Layout inside the (unchanged) 18-real block: fp64: 6 planes of double2 then 1 plane of double;
+// fp32: 3 planes of float4 then 1 plane of float.  `bad` counts links whose row 2 is NOT reproduced to `tol`
+// (relative to |c|): the caller then falls back to the uncompressed format.
+// Dry run of the compression test on the caller's canonical array (writes nothing but the counter).
+template <typename TS>
+__global__ void __launch_bounds__(256) naik_check_kernel(const TS* __restrict__ src, int Vh, double tol, unsigned long long* bad)
+{
+    const size_t V = (size_t)2 * Vh;
+    const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (idx >= 4 * V) return;
+    const TS* s = src + idx * 18;
+    double e[18];
+#pragma unroll
+    for (int i = 0; i < 18; ++i) e[i] = (double)s[i];
+    double n0 = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2] + e[3] * e[3] + e[4] * e[4] + e[5] * e[5]);
+    double cr[6], det_re = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        const int b = (a + 1) % 3, c = (a + 2) % 3;
+        cr[2 * a] = (e[2 * b] * e[6 + 2 * c] - e[2 * b + 1] * e[6 + 2 * c + 1]) - (e[2 * c] * e[6 + 2 * b] - e[2 * c + 1] * e[6 + 2 * b + 1]);
+        cr[2 * a + 1] = (e[2 * b] * e[6 + 2 * c + 1] + e[2 * b + 1] * e[6 + 2 * c]) - (e[2 * c] * e[6 + 2 * b + 1] + e[2 * c + 1] * e[6 + 2 * b]);
+        det_re += cr[2 * a] * e[12 + 2 * a] - cr[2 * a + 1] * e[12 + 2 * a + 1];
+    }
+    const double c = det_re < 0.0 ? -n0 : n0, ic = c != 0.0 ? 1.0 / c : 0.0;
+    double dev = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        dev = fmax(dev, fabs(cr[2 * a] * ic - e[12 + 2 * a]));
+        dev = fmax(dev, fabs(-cr[2 * a + 1] * ic - e[12 + 2 * a + 1]));
+    }
+    if (!(dev <= tol * n0) || n0 == 0.0) atomicAdd(bad, 1ull);
+}
+
+template <typename TS, typename TD>
+__global__ void __launch_bounds__(256) naik_compress_kernel(const TS* __restrict__ src, TD* __restrict__ dst_field, int Vh,
+                                                            double tol, unsigned long long* bad)
+{
+    const size_t V = (size_t)2 * Vh;
+    const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (idx >= 4 * V) return;
+    const int mu = (int)(idx / V);
+    const size_t eo = idx % V;
+    const int par = eo >= (size_t)Vh ? 1 : 0;
+    const int h = (int)(eo - (size_t)par * Vh);
+    const TS* s = src + idx * 18;
+    TD* blk = dst_field + (size_t)(par * 4 + mu) * ((size_t)Vh * 18);
+    double e[18];
+#pragma unroll
+    for (int i = 0; i < 18; ++i) e[i] = (double)(TD)s[i];   // the values the kernel will see
+    // c = sign(Re det W) * |row 0|
+    double cr[6];  // row0 x row1 (complex 3-vector)
+    for (int a = 0; a < 3; ++a) {
+        const int b = (a + 1) % 3, c = (a + 2) % 3;
+        const double xr = e[2 * b], xi = e[2 * b + 1], yr = e[6 + 2 * c], yi = e[6 + 2 * c + 1];
+        const double zr = e[2 * c], zi = e[2 * c + 1], wr = e[6 + 2 * b], wi = e[6 + 2 * b + 1];
+        cr[2 * a] = (xr * yr - xi * yi) - (zr * wr - zi * wi);
+        cr[2 * a + 1] = (xr * yi + xi * yr) - (zr * wi + zi * wr);
+    }
+    double det_re = 0.0;  // Re( (row0 x row1) . row2 )
+    for (int a = 0; a < 3; ++a) det_re += cr[2 * a] * e[12 + 2 * a] - cr[2 * a + 1] * e[12 + 2 * a + 1];
+    const double n0 = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2] + e[3] * e[3] + e[4] * e[4] + e[5] * e[5]);
+    const double c = det_re < 0.0 ? -n0 : n0;
+    const double ic = c != 0.0 ? 1.0 / c : 0.0;
+    double dev = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        dev = fmax(dev, fabs(cr[2 * a] * ic - e[12 + 2 * a]));
+        dev = fmax(dev, fabs(-cr[2 * a + 1] * ic - e[12 + 2 * a + 1]));
+    }
+    if (!(dev <= tol * n0) || n0 == 0.0) atomicAdd(bad, 1ull);
+    if (sizeof(TD) == 8) {
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+            blk[((size_t)j * Vh + h) * 2] = (TD)e[2 * j];
+            blk[((size_t)j * Vh + h) * 2 + 1] = (TD)e[2 * j + 1];
+        }
+        blk[(size_t)12 * Vh + h] = (TD)ic;
+    } else {
+#pragma unroll
+        for (int j = 0; j < 3; ++j)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) blk[((size_t)j * Vh + h) * 4 + i] = (TD)e[4 * j + i];
+        blk[(size_t)12 * Vh + h] = (TD)ic;
     }
 }
 

@@ -43,6 +43,7 @@ template <typename T> struct DslashArgs {
     int nchunks;         // RHS chunks of NR handled by this launch (consecutive CTAs)
     int slab_blocks;     // CTAs per (tile, t) slab and chunk
     unsigned total_blocks; // CTAs of the whole launch group (epilogue ticket)
+    int naik_c13;        // 1: Naik links are stored compressed (13 reals, row f2)
 };
 
 template <typename T> __host__ __device__ constexpr size_t link_block_reals(int Vh) { return (size_t)Vh * 18; }
@@ -75,6 +76,44 @@ __device__ __forceinline__ void load_link(const float* blk, int Vh, int h, float
     }
     float2 w = ld_stream(reinterpret_cast<const float2*>(blk + (size_t)16 * Vh) + h);
     U[16] = w.x; U[17] = w.y;
+}
+
+// Compressed Naik link (row f2): rows 0, 1 and 1/c are stored, row 2 = conj(row0 x row1) / c.
+template <typename T> __device__ __forceinline__ void reconstruct_row2(T (&U)[18], T ic)
+{
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const int b = (a + 1) % 3, c = (a + 2) % 3;
+        const T re = (U[2 * b] * U[6 + 2 * c] - U[2 * b + 1] * U[6 + 2 * c + 1]) - (U[2 * c] * U[6 + 2 * b] - U[2 * c + 1] * U[6 + 2 * b + 1]);
+        const T im = (U[2 * b] * U[6 + 2 * c + 1] + U[2 * b + 1] * U[6 + 2 * c]) - (U[2 * c] * U[6 + 2 * b + 1] + U[2 * c + 1] * U[6 + 2 * b]);
+        U[12 + 2 * a] = re * ic;
+        U[12 + 2 * a + 1] = -im * ic;
+    }
+}
+
+__device__ __forceinline__ void load_link_c13(const double* blk, int Vh, int h, double (&U)[18])
+{
+    const double2* p = reinterpret_cast<const double2*>(blk) + h;
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        double2 w = ld_stream(p + (size_t)c * Vh);
+        U[2 * c] = w.x;
+        U[2 * c + 1] = w.y;
+    }
+    const double ic = __ldcs(blk + (size_t)12 * Vh + h);
+    reconstruct_row2(U, ic);
+}
+
+__device__ __forceinline__ void load_link_c13(const float* blk, int Vh, int h, float (&U)[18])
+{
+    const float4* p4 = reinterpret_cast<const float4*>(blk) + h;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        float4 w = ld_stream(p4 + (size_t)j * Vh);
+        U[4 * j] = w.x; U[4 * j + 1] = w.y; U[4 * j + 2] = w.z; U[4 * j + 3] = w.w;
+    }
+    const float ic = __ldcs(blk + (size_t)12 * Vh + h);
+    reconstruct_row2(U, ic);
 }
 
 template <typename T>
@@ -126,11 +165,12 @@ template <typename T> __device__ __forceinline__ void mvdag_sub(const T (&U)[18]
 // s = -1 iff the hop crossed the t boundary (`flip`).  The gathered vectors are loaded VB at a time
 // (register budget: 18 reals of link + 6*VB of vectors live beside the 6*NR accumulators).
 template <typename T, int NR, int VB, bool FWD>
-__device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, int Vh, int hn, bool tdir, bool flip,
+__device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, int Vh, int hn, bool tdir, bool flip, bool c13,
                                              T (&acc)[NR][6])
 {
     T U[18];
-    load_link(blk, Vh, hl, U);
+    if (c13) load_link_c13(blk, Vh, hl, U);
+    else load_link(blk, Vh, hl, U);
 #if HISQ_SIGN_BRANCH
     if (tdir && flip) {
         // antiperiodic t: the whole CTA shares t (blockIdx.y), so `flip` is block-uniform: a real branch, taken only
@@ -213,7 +253,7 @@ template <typename T, int NR> struct KernelShape {
                               : NR == 2 ? (f32 ? HISQ_F32_MINB2 : HISQ_F64_MINB2) : 1;
 };
 
-template <typename T, int NR, int MODE, int BLOCK>
+template <typename T, int NR, int MODE, int BLOCK, bool NC>
 __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel(const DslashArgs<T> a)
 {
     if (a.done != nullptr && *a.done != 0) return;
@@ -264,8 +304,8 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
                     int hp, hm;
                     if (mu == 0) { hp = row + (cp >> 1); hm = row + (cm >> 1); }
                     else { hp = h + (cp - c[mu]) * stride[mu]; hm = h + (cm - c[mu]) * stride[mu]; }
-                    stencil_term<T, NR, VB, true>(link_block(a.links, Vh, f, par, mu), h, in, Vh, hp, mu == 3, wp, acc);
-                    stencil_term<T, NR, VB, false>(link_block(a.links, Vh, f, 1 - par, mu), hm, in, Vh, hm, mu == 3, wm, acc);
+                    stencil_term<T, NR, VB, true>(link_block(a.links, Vh, f, par, mu), h, in, Vh, hp, mu == 3, wp, NC && f == 1, acc);
+                    stencil_term<T, NR, VB, false>(link_block(a.links, Vh, f, 1 - par, mu), hm, in, Vh, hm, mu == 3, wm, NC && f == 1, acc);
                 }
             }
         } else {
@@ -294,8 +334,8 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
                     const int hp = h + (up - u) * sd, hm = h + (um - u) * sd;
                     const T* lf = a.links + (size_t)((f * 2 + par) * 4 + mu) * blk_reals;
                     const T* lb = a.links + (size_t)((f * 2 + (1 - par)) * 4 + mu) * blk_reals;
-                    stencil_term<T, NR, VB, true>(lf, h, in, Vh, hp, mu == 3, wp, acc);
-                    stencil_term<T, NR, VB, false>(lb, hm, in, Vh, hm, mu == 3, wm, acc);
+                    stencil_term<T, NR, VB, true>(lf, h, in, Vh, hp, mu == 3, wp, NC && f == 1, acc);
+                    stencil_term<T, NR, VB, false>(lb, hm, in, Vh, hm, mu == 3, wm, NC && f == 1, acc);
                 }
             }
         }

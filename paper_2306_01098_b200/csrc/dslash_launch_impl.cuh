@@ -7,7 +7,8 @@ namespace hisq {
 template <typename T, int NR, int MODE>
 static cudaError_t launch_one(const DslashArgs<T>& a, dim3 grid, cudaStream_t s)
 {
-    dslash_kernel<T, NR, MODE, kDslashBlock><<<grid, kDslashBlock, 0, s>>>(a);
+    if (a.naik_c13) dslash_kernel<T, NR, MODE, kDslashBlock, true><<<grid, kDslashBlock, 0, s>>>(a);
+    else dslash_kernel<T, NR, MODE, kDslashBlock, false><<<grid, kDslashBlock, 0, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -78,9 +79,9 @@ static int regs_mode(int mode)
     cudaFuncAttributes at;
     cudaError_t e;
     switch (mode) {
-    case MODE_PLAIN: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_PLAIN, kDslashBlock>); break;
-    case MODE_APPLY_A: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_APPLY_A, kDslashBlock>); break;
-    default: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_RESID, kDslashBlock>); break;
+    case MODE_PLAIN: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_PLAIN, kDslashBlock, false>); break;
+    case MODE_APPLY_A: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_APPLY_A, kDslashBlock, false>); break;
+    default: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_RESID, kDslashBlock, false>); break;
     }
     return e == cudaSuccess ? at.numRegs : -1;
 }

@@ -31,6 +31,9 @@ struct hisq_ctx {
     char* fields;          // CG temporaries
     char* stage;           // host-call staging (2 canonical + 2 native fields)
     bool have_links;
+    bool naik_c13;         // Naik links currently stored compressed
+    int naik_compress;     // option: try to compress at the next hisq_set_links
+    unsigned long long* bad_count;  // device counter used by the compression check
     // options
     int max_iter, reliable_interval, check_interval, use_graph, nrhs_inner, tile_y, tile_z;
     double window_mb;
@@ -111,6 +114,7 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     h->check_interval = 32;
     h->use_graph = 1;
     h->nrhs_inner = 0;
+    h->naik_c13 = false; h->naik_compress = 0; h->bad_count = nullptr;
     h->tile_y = 0; h->tile_z = 0;
     h->window_mb = 40.0;
     h->info_iters = 0; h->info_reliable = 0;
@@ -161,7 +165,7 @@ static WsLayout ws_layout(const hisq_ctx* h, int nrhs)
     l.links32 = off;
     if (h->prec != HISQ_FP64) off += align_up(2 * 4 * V * 18 * 4);
     l.state = off; off += align_up(sizeof(CgState));
-    l.true_rr = off; off += align_up(kMaxNrhs * sizeof(double));
+    l.true_rr = off; off += align_up(kMaxNrhs * sizeof(double) + 64);   // + the compression check counter
     // columns: enough for the Dslash epilogue (one per CTA and chunk-slot) and the BLAS kernels
     size_t cols_d = ((size_t)h->g.Vh / 64 + (size_t)h->g.L[3] * h->g.L[1] * h->g.L[2] / 16 + 64);
     size_t cols_b = (size_t)blas_grid_x((size_t)6 * h->g.Vh, 2) + init_grid_x((size_t)6 * h->g.Vh) + 64;
@@ -196,6 +200,7 @@ extern "C" int hisq_set_workspace(hisq_ctx* h, void* p, size_t bytes)
     h->links32 = h->prec != HISQ_FP64 ? (float*)(h->ws + l.links32) : nullptr;
     h->state = (CgState*)(h->ws + l.state);
     h->true_rr = (double*)(h->ws + l.true_rr);
+    h->bad_count = (unsigned long long*)(h->ws + l.true_rr + kMaxNrhs * sizeof(double));
     h->partial = (double*)(h->ws + l.partial);
     h->partial_cols = l.partial_cols;
     h->fields = h->ws + l.fields;
@@ -214,6 +219,7 @@ extern "C" int hisq_set_links(hisq_ctx* h, const void* fat, const void* naik)
     const unsigned grid = (unsigned)((4 * V + 255) / 256);
     const size_t fstride = (size_t)8 * Vh * 18;  // reals per field (2 parities x 4 directions)
     const void* src[2] = { fat, naik };
+    h->naik_c13 = false;
     for (int f = 0; f < 2; ++f) {
         if (h->prec == HISQ_FP32) {
             link_repack_kernel<float, float><<<grid, 256, 0, h->stream>>>((const float*)src[f], h->links32 + f * fstride, Vh);
@@ -223,6 +229,34 @@ extern "C" int hisq_set_links(hisq_ctx* h, const void* fat, const void* naik)
                 link_repack_kernel<double, float><<<grid, 256, 0, h->stream>>>((const double*)src[f], h->links32 + f * fstride, Vh);
         }
         h->stats.launches += (h->prec == HISQ_MIXED) ? 2 : 1;
+    }
+    if (h->naik_compress) {
+        // row f2: try the 13-real format for the Naik links; keep it only if EVERY link is reproduced
+        // (|row2 - conj(row0 x row1)/c| <= tol |c|), otherwise the uncompressed copy written above stays
+        CK(cudaMemsetAsync(h->bad_count, 0, sizeof(unsigned long long), h->stream));
+        // scratch: the staging area is large enough only for small lattices, so test first, then overwrite in place
+        if (h->prec == HISQ_FP32) {
+            naik_check_kernel<float><<<grid, 256, 0, h->stream>>>((const float*)naik, Vh, 1e-5, h->bad_count);
+        } else {
+            naik_check_kernel<double><<<grid, 256, 0, h->stream>>>((const double*)naik, Vh, 1e-12, h->bad_count);
+        }
+        unsigned long long bad = 1;
+        CK(cudaMemcpyAsync(&bad, h->bad_count, sizeof(bad), cudaMemcpyDeviceToHost, h->stream));
+        CK(cudaStreamSynchronize(h->stream));
+        h->stats.launches++;
+        if (bad == 0) {
+            if (h->prec == HISQ_FP32) {
+                naik_compress_kernel<float, float><<<grid, 256, 0, h->stream>>>((const float*)naik, h->links32 + fstride, Vh, 1e-5, h->bad_count);
+            } else {
+                naik_compress_kernel<double, double><<<grid, 256, 0, h->stream>>>((const double*)naik, h->links64 + fstride, Vh, 1e-12, h->bad_count);
+                if (h->prec == HISQ_MIXED)
+                    naik_compress_kernel<double, float><<<grid, 256, 0, h->stream>>>((const double*)naik, h->links32 + fstride, Vh, 1e-5, h->bad_count);
+            }
+            h->stats.launches += (h->prec == HISQ_MIXED) ? 2 : 1;
+            h->naik_c13 = true;
+        } else {
+            h->last_error = "naik_compress: " + std::to_string(bad) + " Naik links are not a real multiple of an SU(3) matrix; stored uncompressed";
+        }
     }
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(h->stream));
@@ -249,6 +283,7 @@ static int run_dslash(hisq_ctx* h, const T* links, T* out, const T* in, int pari
     a.m2 = m2;
     a.par = parity;
     a.k0 = 0; a.nrhs_total = nrhs; a.nchunks = 1; a.slab_blocks = 0; a.total_blocks = 0;
+    a.naik_c13 = h->naik_c13 ? 1 : 0;
     int cap = h->nrhs_inner > 0 ? h->nrhs_inner : default_inner_cap((int)sizeof(T));
     int e = launch_dslash<T>(a, mode, nrhs, cap, h->stream, &h->stats);
     if (e != 0) return cuda_fail(h, (cudaError_t)e, "dslash launch");
@@ -621,6 +656,7 @@ extern "C" int hisq_set_option(hisq_ctx* h, const char* key, double value)
     else if (!strcmp(key, "check_interval")) { if (v < 1 || v > 1024) return HISQ_EINVAL; h->check_interval = v; }
     else if (!strcmp(key, "use_graph")) h->use_graph = v != 0;
     else if (!strcmp(key, "nrhs_inner")) { if (v < 0 || v > 8) return HISQ_EINVAL; h->nrhs_inner = v; }
+    else if (!strcmp(key, "naik_compress")) h->naik_compress = v != 0;
     else if (!strcmp(key, "tile_y")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[1] % v))) return HISQ_EINVAL; h->tile_y = v; }
     else if (!strcmp(key, "tile_z")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[2] % v))) return HISQ_EINVAL; h->tile_z = v; }
     else if (!strcmp(key, "window_mb")) { if (!(value > 0)) return HISQ_EINVAL; h->window_mb = value; }
@@ -704,6 +740,8 @@ extern "C" int hisq_cg_host(hisq_ctx* h, void* x_host, const void* b_host, doubl
     CK(cudaStreamSynchronize(h->stream));
     return solve_rc;
 }
+
+extern "C" int hisq_naik_compressed(const hisq_ctx* h) { return h && h->naik_c13 ? 1 : 0; }
 
 extern "C" long long hisq_launch_count(const hisq_ctx* h) { return h ? h->stats.launches : 0; }
 
