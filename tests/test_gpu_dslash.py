@@ -125,3 +125,23 @@ def test_error_codes():
     with pytest.raises(binding.HisqError):
         ctx.set_option("no_such_option", 1)
     ctx.close()
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_dslash_max_nrhs_and_odd_half_row(prec):
+    """HISQ_MAX_NRHS = 16 right-hand sides (two chunks of 8), and Lx = 6 (Lx/2 = 3 is odd: x-rows are not a whole
+    number of 16-byte pairs, every warp straddles rows)."""
+    _check((6, 6, 6, 6), prec, 16, seed=11)
+    _check((6, 4, 8, 4), prec, 5, seed=12)
+
+
+def test_dslash_rejects_too_many_rhs():
+    from paper_2306_01098_b200 import binding
+    ctx = binding.Hisq((4, 4, 4, 4), "fp64", 1)
+    fat, naik = binding.make_links((4, 4, 4, 4), 0, ctx.device)
+    ctx.set_links(fat, naik)
+    f = torch.zeros(17, 3, ctx.Vh, dtype=ctx.cdtype, device=ctx.device)
+    with pytest.raises(binding.HisqError) as e:
+        ctx.dslash(f, 0)
+    assert e.value.code == -1
+    ctx.close()
