@@ -227,6 +227,12 @@ __device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, 
 #ifndef HISQ_F32_MINB4
 #define HISQ_F32_MINB4 8
 #endif
+#ifndef HISQ_F32_MINB1
+#define HISQ_F32_MINB1 3
+#endif
+#ifndef HISQ_F64_MINB1
+#define HISQ_F64_MINB1 4
+#endif
 #ifndef HISQ_F32_MINB2
 #define HISQ_F32_MINB2 8
 #endif
@@ -250,7 +256,7 @@ template <typename T, int NR> struct KernelShape {
     static constexpr int vb = NR >= 6 ? (vb8 < NR ? vb8 : NR) : NR;
     static constexpr int minb = NR >= 6 ? (f32 ? HISQ_F32_MINB8 : HISQ_F64_MINB8)
                               : NR >= 3 ? (f32 ? HISQ_F32_MINB4 : HISQ_F64_MINB4)
-                              : NR == 2 ? (f32 ? HISQ_F32_MINB2 : HISQ_F64_MINB2) : 1;
+                              : NR == 2 ? (f32 ? HISQ_F32_MINB2 : HISQ_F64_MINB2) : (f32 ? HISQ_F32_MINB1 : HISQ_F64_MINB1);
 };
 
 template <typename T, int NR, int MODE, int BLOCK, bool NC>
