@@ -7,6 +7,8 @@
 // Fields are NATIVE half-lattice arrays: RHS k is the contiguous block [k*nreal, (k+1)*nreal) of reals,
 // nreal = 6*Vh.  Grid: blockIdx.y = k, blockIdx.x over 16-byte vectors of that block.
 #pragma once
+#include <cooperative_groups.h>
+
 #include "common.cuh"
 
 namespace hisq {
@@ -172,6 +174,122 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict_
             const int it = st->iter + 1;
             st->iter = it;
             if (!any || it >= st->max_iter || st->breakdown) st->done = 1;
+        }
+    }
+}
+
+// ---- fused update for fields small enough to stay in registers across a grid barrier (cooperative launch) ----
+// = cg_update_xr_kernel of iteration i followed by cg_update_p_kernel of iteration i+1 in ONE kernel: the new r and the
+// old p stay in registers over the barrier, so r is not re-read and one launch per iteration disappears (C1/C2-size
+// lattices are launch- and L2-latency-bound in their BLAS part).  Same arithmetic, same summation order per block
+// column as the two-kernel path.  `do_p = 0` (last iteration before a reliable update) leaves p untouched.
+template <typename T, int KEEP>
+__global__ void __launch_bounds__(kBlasBlock) cg_fused_update_kernel(T* __restrict__ x, T* __restrict__ r, T* __restrict__ p,
+                                                                     const T* __restrict__ q, size_t nreal, CgState* st,
+                                                                     double* partial, int do_p)
+{
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    if (st->done) return;   // grid-uniform: written only by earlier kernels
+    using V = typename V16<T>::type;
+    constexpr int N = V16<T>::n;
+    constexpr int NW = kBlasBlock / 32;
+    const int k = blockIdx.y, n = gridDim.y, gx = gridDim.x;
+    __shared__ double s_rho[kMaxNrhs], s_pq[kMaxNrhs], s_bn2[kMaxNrhs], s_rn[kMaxNrhs], s_warp[NW];
+    __shared__ int s_active[kMaxNrhs], s_misc[3];
+    if (threadIdx.x < n) {
+        s_rho[threadIdx.x] = st->rho[threadIdx.x]; s_pq[threadIdx.x] = st->pq[threadIdx.x];
+        s_bn2[threadIdx.x] = st->bnorm2[threadIdx.x]; s_active[threadIdx.x] = st->active[threadIdx.x];
+    }
+    if (threadIdx.x == 0) { s_misc[0] = st->iter; s_misc[1] = st->max_iter; s_misc[2] = st->breakdown; }
+    const double tol2 = st->tol2;
+    __syncthreads();
+    const bool live = s_active[k] != 0;
+    double alpha_d = 0.0;
+    if (live) alpha_d = (s_pq[k] > 0.0 && isfinite(s_pq[k])) ? s_rho[k] / s_pq[k] : 0.0;
+    const T alpha = (T)alpha_d;
+    const size_t nvec = nreal / N, base = (size_t)k * nreal;
+    V* xv = reinterpret_cast<V*>(x + base);
+    V* rv = reinterpret_cast<V*>(r + base);
+    V* pv = reinterpret_cast<V*>(p + base);
+    const V* qv = reinterpret_cast<const V*>(q + base);
+    T rk[KEEP][N], pk[KEEP][N];
+    double sum = 0.0;
+#pragma unroll
+    for (int j = 0; j < KEEP; ++j) {
+        const size_t i = ((size_t)blockIdx.x * KEEP + j) * kBlasBlock + threadIdx.x;
+        if (live && i < nvec) {
+            T a[N], d[N];
+            unpack16<T>(xv[i], a); unpack16<T>(rv[i], rk[j]); unpack16<T>(pv[i], pk[j]); unpack16<T>(qv[i], d);
+#pragma unroll
+            for (int e = 0; e < N; ++e) {
+                a[e] = fma(alpha, pk[j][e], a[e]);
+                rk[j][e] = fma(-alpha, d[e], rk[j][e]);
+                sum += (double)rk[j][e] * (double)rk[j][e];
+            }
+            xv[i] = pack16<T>(a);
+            rv[i] = pack16<T>(rk[j]);
+        }
+    }
+    // block partial (same two-stage order as grid_reduce)
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    if (lane == 0) s_warp[warp] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < NW; ++w) s += s_warp[w];
+        partial[(size_t)k * gx + blockIdx.x] = s;
+        __threadfence();
+    }
+    grid.sync();
+    // every block rebuilds all rho'_k identically (fixed order), so no second barrier is needed
+    for (int kk = warp; kk < n; kk += NW) {
+        double s = 0.0;
+        for (int i = lane; i < gx; i += 32) s += __ldcg(partial + (size_t)kk * gx + i);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0) s_rn[kk] = s;
+    }
+    __syncthreads();
+    int any = 0, brk = s_misc[2];
+    double beta_k = 0.0;
+    bool my_active = false;
+    for (int kk = 0; kk < n; ++kk) {
+        if (!s_active[kk]) continue;
+        const double rn = s_rn[kk], pq = s_pq[kk];
+        if (!(pq > 0.0) || !isfinite(pq) || !isfinite(rn)) brk = 1;
+        const bool still = !(rn <= tol2 * s_bn2[kk]);
+        any |= still ? 1 : 0;
+        if (kk == k) { beta_k = rn / s_rho[kk]; my_active = still; }
+    }
+    const int it = s_misc[0] + 1;
+    const bool done = !any || it >= s_misc[1] || brk;
+    if (blockIdx.x == 0 && blockIdx.y == 0) {
+        if (threadIdx.x < n && s_active[threadIdx.x]) {
+            const int kk = threadIdx.x;
+            const double rn = s_rn[kk];
+            st->rho_prev[kk] = s_rho[kk];
+            st->beta[kk] = rn / s_rho[kk];
+            st->rho[kk] = rn;
+            if (rn <= tol2 * s_bn2[kk]) st->active[kk] = 0;
+        }
+        if (threadIdx.x == 0) {
+            st->iter = it;
+            if (brk) st->breakdown = 1;
+            if (done) st->done = 1;
+        }
+    }
+    if (!do_p || done || !my_active) return;
+    const T beta = (T)beta_k;
+#pragma unroll
+    for (int j = 0; j < KEEP; ++j) {
+        const size_t i = ((size_t)blockIdx.x * KEEP + j) * kBlasBlock + threadIdx.x;
+        if (i < nvec) {
+#pragma unroll
+            for (int e = 0; e < N; ++e) pk[j][e] = fma(beta, pk[j][e], rk[j][e]);
+            pv[i] = pack16<T>(pk[j]);
         }
     }
 }

@@ -33,6 +33,8 @@ struct hisq_ctx {
     bool have_links;
     bool naik_c13;         // Naik links currently stored compressed
     int naik_compress;     // option: try to compress at the next hisq_set_links
+    int fused_blas;        // option: cooperative fused x/r/p update for small fields
+    int num_sms;
     unsigned long long* bad_count;  // device counter used by the compression check
     // options
     int max_iter, reliable_interval, check_interval, use_graph, nrhs_inner, tile_y, tile_z;
@@ -115,6 +117,8 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     h->use_graph = 1;
     h->nrhs_inner = 0;
     h->naik_c13 = false; h->naik_compress = 0; h->bad_count = nullptr;
+    h->fused_blas = 1; h->num_sms = 0;
+    { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev); }
     h->tile_y = 0; h->tile_z = 0;
     h->window_mb = 40.0;
     h->info_iters = 0; h->info_reliable = 0;
@@ -168,7 +172,7 @@ static WsLayout ws_layout(const hisq_ctx* h, int nrhs)
     l.true_rr = off; off += align_up(kMaxNrhs * sizeof(double) + 64);   // + the compression check counter
     // columns: enough for the Dslash epilogue (one per CTA and chunk-slot) and the BLAS kernels
     size_t cols_d = ((size_t)h->g.Vh / 64 + (size_t)h->g.L[3] * h->g.L[1] * h->g.L[2] / 16 + 64);
-    size_t cols_b = (size_t)blas_grid_x((size_t)6 * h->g.Vh, 2) + init_grid_x((size_t)6 * h->g.Vh) + 64;
+    size_t cols_b = (size_t)blas_grid_x((size_t)6 * h->g.Vh, 2) + init_grid_x((size_t)6 * h->g.Vh) + 64 + 4096;
     l.partial_cols = cols_d > cols_b ? cols_d : cols_b;
     l.partial = off; off += align_up((size_t)kMaxNrhs * l.partial_cols * sizeof(double));
     l.fields = off;
@@ -315,19 +319,78 @@ extern "C" int hisq_dslash(hisq_ctx* h, void* out, const void* in, int parity, i
 // One iteration (textbook Hestenes-Stiefel, independent scalars per RHS):
 //   p = r + beta p ; t = D_oe p ; q = m^2 p - D_eo t , <p,q> ; x += alpha p , r -= alpha q , rho' = ||r||^2
 template <typename T>
-static int enqueue_iteration(hisq_ctx* h, const T* links, T* x, T* r, T* p, T* q, T* t, double m2, int nrhs)
+static int enqueue_p_update(hisq_ctx* h, T* p, const T* r, int nrhs)
 {
     const size_t nreal = (size_t)6 * h->g.Vh;
     dim3 gb((unsigned)blas_grid_x(nreal, V16<T>::n), (unsigned)nrhs);
     cg_update_p_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(p, r, nreal, h->state);
     h->stats.launches++;
-    int rc = run_dslash<T>(h, links, t, p, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, &h->state->done, 2);
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+
+// Largest field for which the fused (cooperative) BLAS kernel applies: every thread keeps KEEP 16-byte vectors of
+// r and p in registers across the grid barrier, and the whole grid must be co-resident.  Returns KEEP or 0.
+template <typename T, int KEEP>
+static int fused_blocks_per_sm()
+{
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, cg_fused_update_kernel<T, KEEP>, kBlasBlock, 0) != cudaSuccess) return 0;
+    return nb;
+}
+template <typename T>
+static int fused_keep(hisq_ctx* h, int nrhs)
+{
+    if (!h->fused_blas) return 0;
+    const size_t nvec = (size_t)6 * h->g.Vh / V16<T>::n;
+    const int keeps[4] = { 1, 2, 4, 8 };
+    for (int i = 0; i < 4; ++i) {
+        const int keep = keeps[i];
+        const size_t gx = (nvec + (size_t)kBlasBlock * keep - 1) / ((size_t)kBlasBlock * keep);
+        int per_sm = keep == 1 ? fused_blocks_per_sm<T, 1>() : keep == 2 ? fused_blocks_per_sm<T, 2>()
+                   : keep == 4 ? fused_blocks_per_sm<T, 4>() : fused_blocks_per_sm<T, 8>();
+        if (gx * nrhs <= (size_t)per_sm * h->num_sms && gx <= h->partial_cols) return keep;
+    }
+    return 0;
+}
+
+template <typename T, int KEEP>
+static cudaError_t launch_fused(hisq_ctx* h, T* x, T* r, T* p, const T* q, size_t nreal, int nrhs, int do_p)
+{
+    const size_t nvec = nreal / V16<T>::n;
+    dim3 grid((unsigned)((nvec + (size_t)kBlasBlock * KEEP - 1) / ((size_t)kBlasBlock * KEEP)), (unsigned)nrhs);
+    CgState* st = h->state;
+    double* partial = h->partial;
+    void* args[] = { &x, &r, &p, &q, &nreal, &st, &partial, &do_p };
+    return cudaLaunchCooperativeKernel((void*)cg_fused_update_kernel<T, KEEP>, grid, dim3(kBlasBlock), args, 0, h->stream);
+}
+
+// keep = 0: the four-kernel iteration  [p = r + beta p] [D_oe] [D_eo + <p,Ap>] [x, r, rho'].
+// keep > 0: the p-update of the NEXT iteration rides in the fused kernel: [D_oe] [D_eo + <p,Ap>] [x, r, rho' | p];
+//           the caller launches one stand-alone p-update at the start and after every true-residual replacement.
+template <typename T>
+static int enqueue_iteration(hisq_ctx* h, const T* links, T* x, T* r, T* p, T* q, T* t, double m2, int nrhs, int keep = 0,
+                             int do_p = 1)
+{
+    const size_t nreal = (size_t)6 * h->g.Vh;
+    dim3 gb((unsigned)blas_grid_x(nreal, V16<T>::n), (unsigned)nrhs);
+    int rc;
+    if (keep == 0 && (rc = enqueue_p_update<T>(h, p, r, nrhs)) != HISQ_OK) return rc;
+    rc = run_dslash<T>(h, links, t, p, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, &h->state->done, 2);
     if (rc) return rc;
     rc = run_dslash<T>(h, links, q, t, HISQ_EVEN, nrhs, MODE_APPLY_A, p, nullptr, m2, h->state->pq, &h->state->done, 2);
     if (rc) return rc;
-    cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial);
+    if (keep == 0) {
+        cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial);
+        CK(cudaGetLastError());
+    } else {
+        cudaError_t e = keep == 1 ? launch_fused<T, 1>(h, x, r, p, q, nreal, nrhs, do_p)
+                      : keep == 2 ? launch_fused<T, 2>(h, x, r, p, q, nreal, nrhs, do_p)
+                      : keep == 4 ? launch_fused<T, 4>(h, x, r, p, q, nreal, nrhs, do_p)
+                                  : launch_fused<T, 8>(h, x, r, p, q, nreal, nrhs, do_p);
+        if (e != cudaSuccess) return cuda_fail(h, e, "cudaLaunchCooperativeKernel");
+    }
     h->stats.launches++;
-    CK(cudaGetLastError());
     return HISQ_OK;
 }
 
@@ -409,41 +472,46 @@ static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_u
             if (R % d == 0) best = d;
         batch = best;
     }
-    IterBatch ib;
+    const int keep = fused_keep<T>(h, nrhs);
+    cudaGraphExec_t execs[2] = { nullptr, nullptr };   // [0]: every iteration ends with its p-update; [1]: the last one does not
+    long long exec_launches[2] = { 0, 0 };
     int rc = HISQ_OK;
     int status = HISQ_OK;
-    long long launches_per_batch = 0;
     int stagnation = 0;
     int enq_iter = 0, cur = 0;
     bool pending = false;
     double best_true[kMaxNrhs];
     for (int k = 0; k < kMaxNrhs; ++k) best_true[k] = 1e300;
+    if (keep > 0 && (rc = enqueue_p_update<T>(h, p, r, nrhs)) != HISQ_OK) return rc;
     while (true) {
-        // ---- a batch of iterations ----
+        // ---- a batch of iterations; the one that ends on a reliable-update boundary leaves p alone ----
+        const int kind = (keep > 0 && R > 0 && (enq_iter + batch) % R == 0) ? 1 : 0;
         if (h->use_graph) {
-            if (!ib.exec) {
+            if (!execs[kind]) {
                 cudaGraph_t graph;
                 const long long l0 = h->stats.launches;
                 if (!h->cap_stream) CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
                 cudaStream_t user_stream = h->stream;
                 CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
                 h->stream = h->cap_stream;
-                for (int i = 0; i < batch && rc == HISQ_OK; ++i) rc = enqueue_iteration<T>(h, links, x, r, p, q, t, m2, nrhs);
+                for (int i = 0; i < batch && rc == HISQ_OK; ++i)
+                    rc = enqueue_iteration<T>(h, links, x, r, p, q, t, m2, nrhs, keep, (kind == 1 && i == batch - 1) ? 0 : 1);
                 h->stream = user_stream;
                 cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
                 if (rc != HISQ_OK) { if (ce == cudaSuccess) cudaGraphDestroy(graph); break; }
                 if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaStreamEndCapture"); break; }
-                ce = cudaGraphInstantiate(&ib.exec, graph, 0);
+                ce = cudaGraphInstantiate(&execs[kind], graph, 0);
                 cudaGraphDestroy(graph);
                 if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaGraphInstantiate"); break; }
-                launches_per_batch = h->stats.launches - l0;
+                exec_launches[kind] = h->stats.launches - l0;
                 h->stats.launches = l0;
             }
-            cudaError_t ce = cudaGraphLaunch(ib.exec, h->stream);
+            cudaError_t ce = cudaGraphLaunch(execs[kind], h->stream);
             if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaGraphLaunch"); break; }
-            h->stats.launches += launches_per_batch;
+            h->stats.launches += exec_launches[kind];
         } else {
-            for (int i = 0; i < batch && rc == HISQ_OK; ++i) rc = enqueue_iteration<T>(h, links, x, r, p, q, t, m2, nrhs);
+            for (int i = 0; i < batch && rc == HISQ_OK; ++i)
+                rc = enqueue_iteration<T>(h, links, x, r, p, q, t, m2, nrhs, keep, (kind == 1 && i == batch - 1) ? 0 : 1);
             if (rc != HISQ_OK) break;
         }
         // ---- look at the state, staying one batch ahead of the GPU whenever no reliable update is due ----
@@ -500,8 +568,10 @@ static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_u
             if (!all) status = HISQ_ENOCONV;
             break;
         }
+        if (keep > 0 && (rc = enqueue_p_update<T>(h, p, r, nrhs)) != HISQ_OK) break;   // p = r_true + beta p
     }
-    if (ib.exec) cudaGraphExecDestroy(ib.exec);
+    for (int i = 0; i < 2; ++i)
+        if (execs[i]) cudaGraphExecDestroy(execs[i]);
     if (rc != HISQ_OK) return rc;
     return status;
 }
@@ -657,6 +727,7 @@ extern "C" int hisq_set_option(hisq_ctx* h, const char* key, double value)
     else if (!strcmp(key, "use_graph")) h->use_graph = v != 0;
     else if (!strcmp(key, "nrhs_inner")) { if (v < 0 || v > 8) return HISQ_EINVAL; h->nrhs_inner = v; }
     else if (!strcmp(key, "naik_compress")) h->naik_compress = v != 0;
+    else if (!strcmp(key, "fused_blas")) h->fused_blas = v != 0;
     else if (!strcmp(key, "tile_y")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[1] % v))) return HISQ_EINVAL; h->tile_y = v; }
     else if (!strcmp(key, "tile_z")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[2] % v))) return HISQ_EINVAL; h->tile_z = v; }
     else if (!strcmp(key, "window_mb")) { if (!(value > 0)) return HISQ_EINVAL; h->window_mb = value; }
