@@ -249,6 +249,19 @@ def main():
     # ---- the step, device-resident inputs ----
     for _ in range(args.warmup):
         _, info = ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
+    # settle: keep warming up (at most 8 more solves) until two consecutive solves agree to 3 % -- boxes have been
+    # seen to run the first seconds after other heavy work up to 1.4x slower with no throttle reason reported
+    extra, prev = 0, None
+    while extra < 8:
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        extra += 1
+        if prev is not None and abs(dt - prev) <= 0.03 * prev:
+            break
+        prev = dt
     sampler = ClockSampler(local)
     sampler.start()
     barrier()
@@ -284,7 +297,7 @@ def main():
     field_bytes = b_host.numel() * b_host.element_size()
 
     # ---- the dominant kernel alone: Dslash, CUDA-event timed ----
-    d_ms = time_dslash(ctx, n, args.dslash_reps)
+    d_ms = min(time_dslash(ctx, n, args.dslash_reps) for _ in range(3))   # best of 3 bursts of 2*reps launches
     peak, peak_src = measured_peaks()
     alg_bytes = dslash_bytes(Vh, n, w)
     achieved = alg_bytes / (d_ms * 1e-3) / 1e9
@@ -340,7 +353,7 @@ def main():
 
     out = {
         "metric": "hisq_dslash_gflops", "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "warmup_extra_settle": extra, "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": {"fp32": "f32", "fp64": "f64", "mixed": "f32+f64"}[cfg["prec"]], "data": "synthetic",
         "config": {"workload": workload_name(args.config, cfg), "l2": "inputs larger than L2 (links %.0f MB)" % (2 * 4 * 2 * Vh * 18 * w / 1e6),
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
@@ -353,7 +366,7 @@ def main():
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": ncu_traffic(args.config, cfg["prec"], n),
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
-                     "timing": f"CUDA events around {2 * args.dslash_reps} back-to-back launches (alternating parity), burst"},
+                     "timing": f"CUDA events around {2 * args.dslash_reps} back-to-back launches (alternating parity), best of 3 bursts"},
         "e2e": {"value": e2e_val, "unit": "GFLOP/s", "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": field_bytes,
                 "ms_per_step": ms2_all / args.steps},
         "gpu_launches": int(launches), "clocks": clocks,

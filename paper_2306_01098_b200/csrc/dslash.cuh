@@ -280,6 +280,8 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
 
     int h = 0;
     const size_t rhs_stride = (size_t)3 * 2 * Vh;  // reals per RHS
+    constexpr bool EARLY = MODE != MODE_PLAIN && NR <= 2;
+    T ue[EARLY ? NR : 1][6], ve[EARLY ? NR : 1][6];
     const T* in = a.in + (size_t)chunk * NR * rhs_stride;
     if (valid) {
         const int xh = l % H;
@@ -292,6 +294,15 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
         h = xh + H * (y + g.L[1] * (z + g.L[2] * t));
         const int row = h - xh;
         constexpr int VB = KernelShape<T, NR>::vb;
+        if (EARLY) {
+            // epilogue operands at the output site are fetched BEFORE the stencil so that their latency hides behind it
+            // (a late, dependent load at the end of every CTA cost ~10 % on C2: profiles/r1_launches_bench_c2.md)
+#pragma unroll
+            for (int k = 0; k < NR; ++k) {
+                load_vec(a.u + (size_t)(chunk * NR + k) * rhs_stride, Vh, h, ue[EARLY ? k : 0]);
+                if (MODE == MODE_RESID) load_vec(a.v + (size_t)(chunk * NR + k) * rhs_stride, Vh, h, ve[EARLY ? k : 0]);
+            }
+        }
         if (!KernelShape<T, NR>::rolled) {
             const int c[4] = { x, y, z, t };
             const int stride[4] = { 0, g.sy, g.sz, g.st };
@@ -362,7 +373,12 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
                 for (int i = 0; i < 6; ++i) o[i] = acc[k][i];
             } else {
                 T uu[6];
-                load_vec(a.u + (size_t)(chunk * NR + k) * rhs_stride, Vh, h, uu);
+                if (EARLY) {
+#pragma unroll
+                    for (int i = 0; i < 6; ++i) uu[i] = ue[EARLY ? k : 0][i];
+                } else {
+                    load_vec(a.u + (size_t)(chunk * NR + k) * rhs_stride, Vh, h, uu);
+                }
                 const T m2 = (T)a.m2;
                 if (MODE == MODE_APPLY_A) {
 #pragma unroll
@@ -372,7 +388,12 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
                     }
                 } else {
                     T vv[6];
-                    load_vec(a.v + (size_t)(chunk * NR + k) * rhs_stride, Vh, h, vv);
+                    if (EARLY) {
+#pragma unroll
+                        for (int i = 0; i < 6; ++i) vv[i] = ve[EARLY ? k : 0][i];
+                    } else {
+                        load_vec(a.v + (size_t)(chunk * NR + k) * rhs_stride, Vh, h, vv);
+                    }
 #pragma unroll
                     for (int i = 0; i < 6; ++i) {
                         o[i] = vv[i] - fma(m2, uu[i], -acc[k][i]);
