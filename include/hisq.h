@@ -127,6 +127,27 @@ int hisq_spinor_unpack(hisq_ctx *h, void *canonical, const void *native, int nrh
 int hisq_dslash_host(hisq_ctx *h, void *out_host, const void *in_host, int parity, int nrhs);
 int hisq_cg_host(hisq_ctx *h, void *x_host, const void *b_host, double mass, double tol, int nrhs);
 
+/* Row f3, first step: a lattice partitioned along t over `nranks` processes / GPUs (the paper's sub-lattices with
+ * halos; "full" indices with halo Eq. (6)/(7) :467-488).  The context of rank r holds the
+ * Lt_global/nranks time slices [r*Lt_loc, (r+1)*Lt_loc) on an EXTENDED local lattice Lx x Ly x Lz x (Lt_loc + 8):
+ * local slice 4 + i is global slice r*Lt_loc + i; local slices 0..3 and Lt_loc+4..Lt_loc+7 are halos (depth 4: the Naik
+ * term needs 3, 4 keeps local site parity = global site parity).  All layouts of this header apply to the extended
+ * lattice (V = Lx*Ly*Lz*(Lt_loc+8)).  Links: the caller provides the links of the extended lattice (at least the
+ * interior and the LOWER halo slices must hold the true links; the upper halo is never read).
+ * hisq_dslash computes the interior slices only, reads t-neighbours from the halo slices of `in` (which the caller
+ * must have filled: hisq_halo_pack -> exchange with the neighbouring ranks -> hisq_halo_unpack), and applies the
+ * antiperiodic sign only on the ranks that own the global t boundary.  Halo slices of `out` are left untouched.
+ * Lt_loc must be even and >= 4.  hisq_cg / hisq_cg_multishift are not available on partitioned contexts (they would
+ * need a cross-rank reduction): HISQ_EINVAL. */
+int hisq_create_part(hisq_ctx **h, int Lx, int Ly, int Lz, int Lt_global, int prec, int rank, int nranks);
+/* Bytes of ONE halo buffer (4 slices, nrhs fields); 0 for a non-partitioned context. */
+size_t hisq_halo_bytes(const hisq_ctx *h, int nrhs);
+/* send_lo <- the 4 lowest interior slices (for the previous rank's upper halo), send_hi <- the 4 highest (for the next
+ * rank's lower halo); buffers are device memory of hisq_halo_bytes each, layout [k][c][4*S] complex.  Asynchronous. */
+int hisq_halo_pack(hisq_ctx *h, void *send_lo, void *send_hi, const void *field, int nrhs);
+/* lower halo <- recv_lo (what the previous rank packed as send_hi), upper halo <- recv_hi (the next rank's send_lo). */
+int hisq_halo_unpack(hisq_ctx *h, void *field, const void *recv_lo, const void *recv_hi, int nrhs);
+
 /* Row f2 (the paper's CompressionType).  With option "naik_compress" = 1, the next hisq_set_links
  * stores each Naik link as 13 reals (rows 0, 1 and 1/c of W = c U, U in SU(3), c real; row 2 = conj(row0 x row1)/c is
  * rebuilt in registers) PROVIDED every Naik link passes |row2 - conj(row0 x row1)/c| <= tol |c| (tol 1e-12 fp64, 1e-5

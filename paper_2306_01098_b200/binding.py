@@ -24,7 +24,8 @@ LIB_PATH = os.environ.get("HISQ_LIB", os.path.join(_HERE, "libhisq.so"))
 EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
     "hisq_set_links", "hisq_dslash", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
-    "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count", "hisq_strerror",
+    "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count",
+    "hisq_create_part", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack", "hisq_strerror",
     "hisq_last_error",
 ]
 
@@ -64,6 +65,11 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_dslash_host.argtypes = [vp, vp, vp, i, i]
     lib.hisq_cg_host.argtypes = [vp, vp, vp, d, d, i]
     lib.hisq_naik_compressed.argtypes = [vp]
+    lib.hisq_create_part.argtypes = [ctypes.POINTER(vp), i, i, i, i, i, i, i]
+    lib.hisq_halo_bytes.argtypes = [vp, i]
+    lib.hisq_halo_bytes.restype = sz
+    lib.hisq_halo_pack.argtypes = [vp, vp, vp, vp, i]
+    lib.hisq_halo_unpack.argtypes = [vp, vp, vp, vp, i]
     lib.hisq_launch_count.argtypes = [vp]
     lib.hisq_launch_count.restype = ctypes.c_longlong
     lib.hisq_strerror.argtypes = [i]
@@ -87,8 +93,18 @@ class Hisq:
     [nrhs, Vh, 3].  Links are canonical [4, V, 3, 3] complex (Eq. 5: slot mu*V + eo).
     """
 
-    def __init__(self, L: Sequence[int], prec: str = "fp64", nrhs_max: int = 1, device: Optional[torch.device] = None):
+    def __init__(self, L: Sequence[int], prec: str = "fp64", nrhs_max: int = 1, device: Optional[torch.device] = None,
+                 part: Optional[tuple] = None):
+        """part = (rank, nranks): this context is rank's share of the lattice L partitioned along t (hisq_create_part);
+        self.L then is the EXTENDED local lattice (Lt/nranks + 8 slices) that every layout refers to."""
         layout.check_extents(L)
+        self.part = part
+        self.L_global = tuple(int(v) for v in L)
+        if part is not None:
+            rank, nranks = part
+            if L[3] % nranks or (L[3] // nranks) % 2 or L[3] // nranks < 4:
+                raise ValueError("Lt / nranks must be even and >= 4")
+            L = (L[0], L[1], L[2], L[3] // nranks + 8)
         if not torch.cuda.is_available():
             raise RuntimeError("libhisq needs a CUDA device (no CPU fallback)")
         self.lib = load_library()
@@ -101,7 +117,10 @@ class Hisq:
         self.nrhs_max = int(nrhs_max)
         self._h = ctypes.c_void_p()
         with torch.cuda.device(self.device):
-            self._check(self.lib.hisq_create(ctypes.byref(self._h), *self.L, _PREC[prec]))
+            if part is None:
+                self._check(self.lib.hisq_create(ctypes.byref(self._h), *self.L, _PREC[prec]))
+            else:
+                self._check(self.lib.hisq_create_part(ctypes.byref(self._h), *self.L_global, _PREC[prec], part[0], part[1]))
             self._check(self.lib.hisq_set_stream(self._h, ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)))
             nbytes = self.lib.hisq_workspace_bytes(self._h, self.nrhs_max)
             if nbytes == 0:
@@ -221,6 +240,21 @@ class Hisq:
                                      float(mass), float(tol), n)
         self._check(code, allow=() if strict else (HISQ_ENOCONV, HISQ_EBREAKDOWN))
         return x_host, self.info(n, code)
+
+    # -- t-partitioned lattices (row f3) -----------------------------------------------------------
+    def halo_buffers(self, nrhs: int):
+        nb = self.lib.hisq_halo_bytes(self._h, nrhs)
+        if nb == 0:
+            raise HisqError(-1, "not a partitioned context")
+        S = self.Vh // self.L[3]
+        mk = lambda: torch.empty((nrhs, 3, 4 * S), dtype=self.cdtype, device=self.device)
+        return mk(), mk()
+
+    def halo_pack(self, field: torch.Tensor, lo: torch.Tensor, hi: torch.Tensor):
+        self._check(self.lib.hisq_halo_pack(self._h, self._ptr(lo), self._ptr(hi), self._ptr(field), field.shape[0]))
+
+    def halo_unpack(self, field: torch.Tensor, lo: torch.Tensor, hi: torch.Tensor):
+        self._check(self.lib.hisq_halo_unpack(self._h, self._ptr(field), self._ptr(lo), self._ptr(hi), field.shape[0]))
 
     def naik_compressed(self) -> bool:
         return bool(self.lib.hisq_naik_compressed(self._h))

@@ -360,6 +360,33 @@ __global__ void __launch_bounds__(256) spinor_layout_kernel(T* __restrict__ dst,
     }
 }
 
+// ---- t-halo pack / unpack (row f3): native field [k][c][slice][S] complex, S = sites of one parity per time slice.
+// PACK:   lo <- interior slices [t_lo, t_lo+H)            (goes to the previous rank's UPPER halo)
+//         hi <- interior slices [t_lo+t_cnt-H, t_lo+t_cnt) (goes to the next rank's LOWER halo)
+// UNPACK: lower halo [t_lo-H, t_lo) <- lo (received from the previous rank), upper halo [t_lo+t_cnt, +H) <- hi.
+// Buffers are [k][c][H*S] complex.
+template <typename T, bool PACK>
+__global__ void __launch_bounds__(256) halo_kernel(T* __restrict__ field, T* __restrict__ lo, T* __restrict__ hi, int S, int Lt_ext,
+                                                   int t_lo, int t_cnt, int H, int nrhs)
+{
+    using C = typename Vec<T>::c1;
+    C* f = reinterpret_cast<C*>(field);
+    C* l = reinterpret_cast<C*>(lo);
+    C* u = reinterpret_cast<C*>(hi);
+    const size_t chunk = (size_t)H * S, total = (size_t)nrhs * 3 * chunk;
+    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < total; i += (size_t)gridDim.x * 256) {
+        const size_t kc = i / chunk, j = i % chunk;
+        const size_t plane = kc * (size_t)Lt_ext * S;
+        if (PACK) {
+            l[i] = f[plane + (size_t)t_lo * S + j];
+            u[i] = f[plane + (size_t)(t_lo + t_cnt - H) * S + j];
+        } else {
+            f[plane + (size_t)(t_lo - H) * S + j] = l[i];
+            f[plane + (size_t)(t_lo + t_cnt) * S + j] = u[i];
+        }
+    }
+}
+
 // ---- link repack: canonical Eq. (5) [mu][eo][3][3] complex of TS -> internal planes of TD ------------
 // one thread per (mu, eo); dst block (f fixed by caller, parity, mu).
 template <typename TS, typename TD>

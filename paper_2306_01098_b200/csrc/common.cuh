@@ -34,6 +34,12 @@ struct Geom {
     // (y,z); inside a column work runs x fastest, then y, then z, then t; columns are swept last.
     int ty, tz;     // tile extents in y and z (divide Ly, Lz)
     int nty, ntz;   // number of tiles
+    // t-partitioned lattice (row f3): this context holds t_cnt time slices of a larger lattice at local slices
+    // [t_lo, t_lo + t_cnt) of an array of L[3] = t_cnt + 2*t_lo slices; the rest are halo slices filled by the
+    // neighbouring ranks.  t-hops never wrap locally; the antiperiodic sign applies where the GLOBAL boundary is.
+    int part;       // 0: ordinary periodic lattice (t_lo = 0, t_cnt = L[3])
+    int t_lo, t_cnt;
+    int flip_lo, flip_hi;  // this rank owns the lower / upper global t boundary
 };
 
 // ---- device-side state of one CG solve (all scalars stay on the GPU) -------------

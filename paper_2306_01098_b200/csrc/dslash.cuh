@@ -267,7 +267,7 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
     const int Vh = g.Vh, H = g.H;
     const int chunk = blockIdx.x % a.nchunks;
     const int sc = blockIdx.x / a.nchunks;
-    const int t = blockIdx.y;
+    const int t = blockIdx.y + g.t_lo;
     const int tile = blockIdx.z;
     const int l = sc * BLOCK + threadIdx.x;
     const bool valid = l < H * g.ty * g.tz;
@@ -313,11 +313,16 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
                     const int hop = f ? 3 : 1;
                     const int Lmu = g.L[mu];
                     int cp = c[mu] + hop;
-                    const bool wp = cp >= Lmu;
-                    cp -= wp ? Lmu : 0;
+                    bool wp = cp >= Lmu;
                     int cm = c[mu] - hop;
-                    const bool wm = cm < 0;
-                    cm += wm ? Lmu : 0;
+                    bool wm = cm < 0;
+                    if (mu == 3 && g.part) {   // partitioned in t: read the halo slices, sign only at the global boundary
+                        wp = g.flip_hi && cp >= g.t_lo + g.t_cnt;
+                        wm = g.flip_lo && cm < g.t_lo;
+                    } else {
+                        cp -= wp ? Lmu : 0;
+                        cm += wm ? Lmu : 0;
+                    }
                     int hp, hm;
                     if (mu == 0) { hp = row + (cp >> 1); hm = row + (cm >> 1); }
                     else { hp = h + (cp - c[mu]) * stride[mu]; hm = h + (cm - c[mu]) * stride[mu]; }
@@ -338,11 +343,16 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
                     const int Lmu = g.L[mu];
                     const int cmu = mu == 0 ? x : (mu == 1 ? y : (mu == 2 ? z : t));
                     int cp = cmu + hop;
-                    const bool wp = cp >= Lmu;
-                    cp -= wp ? Lmu : 0;
+                    bool wp = cp >= Lmu;
                     int cm = cmu - hop;
-                    const bool wm = cm < 0;
-                    cm += wm ? Lmu : 0;
+                    bool wm = cm < 0;
+                    if (mu == 3 && g.part) {
+                        wp = g.flip_hi && cp >= g.t_lo + g.t_cnt;
+                        wm = g.flip_lo && cm < g.t_lo;
+                    } else {
+                        cp -= wp ? Lmu : 0;
+                        cm += wm ? Lmu : 0;
+                    }
                     // in units of the half-index stride: x counts in pairs (two sites of a row share h)
                     const int u = mu == 0 ? xh : cmu;
                     const int up = mu == 0 ? (cp >> 1) : cp;
@@ -412,8 +422,8 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
     }
     if (MODE != MODE_PLAIN) {
         __shared__ double totals[kMaxNrhs];
-        const int col = sc + a.slab_blocks * (t + g.L[3] * tile);
-        const int ncols = a.slab_blocks * g.L[3] * g.nty * g.ntz;
+        const int col = sc + a.slab_blocks * ((int)blockIdx.y + g.t_cnt * tile);
+        const int ncols = a.slab_blocks * g.t_cnt * g.nty * g.ntz;
         if (grid_reduce<NR, BLOCK>(red, kg0, a.partial, ncols, col, a.ticket, a.total_blocks, a.nrhs_total, totals)) {
             if (threadIdx.x < a.nrhs_total) a.result[threadIdx.x] = totals[threadIdx.x];
         }

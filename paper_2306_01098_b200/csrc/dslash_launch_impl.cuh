@@ -44,7 +44,7 @@ int launch_dslash(DslashArgs<T> args, int mode, int nrhs, int inner_cap, cudaStr
         ++nplan;
     }
     unsigned total = 0;
-    for (int i = 0; i < nplan; ++i) total += (unsigned)args.slab_blocks * plan_cnt[i] * g.L[3] * ntiles;
+    for (int i = 0; i < nplan; ++i) total += (unsigned)args.slab_blocks * plan_cnt[i] * g.t_cnt * ntiles;
     args.total_blocks = total;
     args.nrhs_total = nrhs;
     int k = 0;
@@ -56,7 +56,7 @@ int launch_dslash(DslashArgs<T> args, int mode, int nrhs, int inner_cap, cudaStr
         if (args.v) a.v = args.v + (size_t)k * rhs_stride;
         a.k0 = k;
         a.nchunks = plan_cnt[i];
-        dim3 grid((unsigned)(a.slab_blocks * a.nchunks), (unsigned)g.L[3], (unsigned)ntiles);
+        dim3 grid((unsigned)(a.slab_blocks * a.nchunks), (unsigned)g.t_cnt, (unsigned)ntiles);
         cudaError_t e;
         switch (plan_nr[i]) {
         case 8: e = launch_mode<T, 8>(a, mode, grid, stream); break;

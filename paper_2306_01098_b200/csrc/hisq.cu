@@ -106,6 +106,7 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     h->g.sy = h->g.H; h->g.sz = h->g.H * Ly; h->g.st = h->g.H * Ly * Lz;
     h->g.stride[0] = 1; h->g.stride[1] = h->g.sy; h->g.stride[2] = h->g.sz; h->g.stride[3] = h->g.st;
     h->g.ty = Ly; h->g.tz = Lz; h->g.nty = 1; h->g.ntz = 1;
+    h->g.part = 0; h->g.t_lo = 0; h->g.t_cnt = Lt; h->g.flip_lo = 1; h->g.flip_hi = 1;
     h->prec = prec;
     h->stream = 0;
     h->cap_stream = nullptr;
@@ -132,6 +133,22 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     cudaEventCreateWithFlags(&h->poll_ev[0], cudaEventDisableTiming);
     cudaEventCreateWithFlags(&h->poll_ev[1], cudaEventDisableTiming);
     *out = h;
+    return HISQ_OK;
+}
+
+// Row f3: one rank's share of a lattice partitioned along t (the paper's sub-lattice + halo scheme, PAPER.md:187-191,
+// Eq. (6)/(7) :467-488).  The context lives on the EXTENDED local lattice Lx x Ly x Lz x (Lt/nranks + 2*kHaloT).
+static const int kHaloT = 4;   // halo slices on each side: 3 are needed (Naik reach), 4 keeps site parity = global parity
+extern "C" int hisq_create_part(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt_global, int prec, int rank, int nranks)
+{
+    if (!out || nranks < 1 || rank < 0 || rank >= nranks || Lt_global % nranks) return HISQ_EINVAL;
+    const int Lt_loc = Lt_global / nranks;
+    if (Lt_loc < 4 || (Lt_loc & 1)) return HISQ_EINVAL;   // even (parity) and >= 3 (halo comes from the nearest rank only)
+    int rc = hisq_create(out, Lx, Ly, Lz, Lt_loc + 2 * kHaloT, prec);
+    if (rc != HISQ_OK) return rc;
+    Geom& g = (*out)->g;
+    g.part = 1; g.t_lo = kHaloT; g.t_cnt = Lt_loc;
+    g.flip_lo = rank == 0; g.flip_hi = rank == nranks - 1;
     return HISQ_OK;
 }
 
@@ -692,7 +709,7 @@ extern "C" int hisq_cg_multishift(hisq_ctx* h, void* x, const void* b, double ma
     if (((uintptr_t)x & 15) || ((uintptr_t)b & 15)) return HISQ_EINVAL;
     for (int k = 0; k < nshift; ++k)
         if (!(shifts[k] >= 0.0) || !std::isfinite(shifts[k])) return HISQ_EINVAL;
-    if (h->prec == HISQ_MIXED) return HISQ_EINVAL;   // fp64 or fp32 contexts only
+    if (h->prec == HISQ_MIXED || h->g.part) return HISQ_EINVAL;   // fp64 or fp32 contexts only, not partitioned
     if (!h->ws) return HISQ_ENOWORKSPACE;
     if (nshift > h->ws_nrhs) return HISQ_ENOWORKSPACE;
     if (!h->have_links) return HISQ_ENOLINKS;
@@ -709,6 +726,7 @@ extern "C" int hisq_cg(hisq_ctx* h, void* x, const void* b, double mass, double 
     if (!h->ws) return HISQ_ENOWORKSPACE;
     if (nrhs > h->ws_nrhs) return HISQ_ENOWORKSPACE;
     if (!h->have_links) return HISQ_ENOLINKS;
+    if (h->g.part) return HISQ_EINVAL;   // the solvers need a cross-rank reduction: not built
     const size_t bytes = (size_t)nrhs * 6 * h->g.Vh * elem_size(h->prec);
     if (overlap(x, b, bytes)) return HISQ_EINVAL;
     if (h->prec == HISQ_FP32) return cg_solve<float, float>(h, h->links32, nullptr, (float*)x, (const float*)b, mass, tol, nrhs);
@@ -810,6 +828,37 @@ extern "C" int hisq_cg_host(hisq_ctx* h, void* x_host, const void* b_host, doubl
     CK(cudaMemcpyAsync(x_host, c_out, bytes, cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
     return solve_rc;
+}
+
+extern "C" size_t hisq_halo_bytes(const hisq_ctx* h, int nrhs)
+{
+    if (!h || !h->g.part || nrhs < 1 || nrhs > HISQ_MAX_NRHS) return 0;
+    return (size_t)nrhs * 3 * kHaloT * (h->g.Vh / h->g.L[3]) * 2 * elem_size(h->prec);
+}
+
+template <bool PACK>
+static int halo_move(hisq_ctx* h, void* field, void* lo, void* hi, int nrhs)
+{
+    if (!h || !field || !lo || !hi || nrhs < 1 || nrhs > HISQ_MAX_NRHS || !h->g.part) return HISQ_EINVAL;
+    const int S = h->g.Vh / h->g.L[3];
+    const size_t total = (size_t)nrhs * 3 * kHaloT * S;
+    unsigned grid = (unsigned)((total + 255) / 256);
+    if (grid > 148 * 8) grid = 148 * 8;
+    if (h->prec == HISQ_FP32)
+        halo_kernel<float, PACK><<<grid, 256, 0, h->stream>>>((float*)field, (float*)lo, (float*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHaloT, nrhs);
+    else
+        halo_kernel<double, PACK><<<grid, 256, 0, h->stream>>>((double*)field, (double*)lo, (double*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHaloT, nrhs);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+extern "C" int hisq_halo_pack(hisq_ctx* h, void* send_lo, void* send_hi, const void* field, int nrhs)
+{
+    return halo_move<true>(h, const_cast<void*>(field), send_lo, send_hi, nrhs);
+}
+extern "C" int hisq_halo_unpack(hisq_ctx* h, void* field, const void* recv_lo, const void* recv_hi, int nrhs)
+{
+    return halo_move<false>(h, field, const_cast<void*>(recv_lo), const_cast<void*>(recv_hi), nrhs);
 }
 
 extern "C" int hisq_naik_compressed(const hisq_ctx* h) { return h && h->naik_c13 ? 1 : 0; }

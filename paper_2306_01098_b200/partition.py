@@ -1,0 +1,85 @@
+"""Row f3, first step: the Dslash on a lattice partitioned along t over several ranks (one process per GPU), the
+paper's sub-lattice + halo scheme (Eq. (6)/(7)).  The kernels and the halo pack / unpack
+are in libhisq (hisq_create_part, hisq_halo_pack, hisq_halo_unpack); this module is the plumbing around them:
+which global sites a rank's extended lattice holds, and the neighbour exchange through torch.distributed
+(NCCL on GPUs, gloo in the CPU test).  No method arithmetic here."""
+from __future__ import annotations
+
+from typing import Sequence
+
+import torch
+
+from . import inputs, layout
+
+HALO_T = 4
+
+
+def extended_lattice(L: Sequence[int], nranks: int):
+    return (int(L[0]), int(L[1]), int(L[2]), int(L[3]) // nranks + 2 * HALO_T)
+
+
+def global_sites_of_rank(L: Sequence[int], rank: int, nranks: int, device="cpu") -> torch.Tensor:
+    """For every memory index eo of rank's EXTENDED lattice (Eq. 4 on that lattice), the GLOBAL lexicographic site
+    it is a copy of (halo slices wrap around the global lattice)."""
+    Le = extended_lattice(L, nranks)
+    lex = layout.lex_of_eo(Le, device=device)
+    x = lex % Le[0]
+    r = lex // Le[0]
+    y = r % Le[1]
+    r = r // Le[1]
+    z = r % Le[2]
+    t = r // Le[2]
+    tg = (rank * (L[3] // nranks) + t - HALO_T) % L[3]
+    return x + L[0] * (y + L[1] * (z + L[2] * tg))
+
+
+def make_links_part(L, seed: int, rank: int, nranks: int, device, cdtype=torch.complex128, gen_device=None):
+    """(fat, naik) canonical on rank's extended lattice: [4, V_ext, 3, 3]."""
+    g = torch.device(gen_device) if gen_device is not None else torch.device("cpu")
+    sites = global_sites_of_rank(L, rank, nranks, device=g)
+    fat = inputs.fat_links(L, seed, sites).permute(1, 0, 2, 3).to(cdtype).contiguous().to(device)
+    naik = inputs.naik_links(L, seed, sites).permute(1, 0, 2, 3).to(cdtype).contiguous().to(device)
+    return fat, naik
+
+
+def make_sources_part(L, seed: int, nrhs: int, parity: int, rank: int, nranks: int, device, cdtype=torch.complex128,
+                      gen_device=None, fill_halo: bool = False):
+    """Gaussian sources on one parity of rank's extended lattice, canonical [nrhs, Vh_ext, 3]; halo slices are zero
+    unless fill_halo (they are what the exchange must deliver)."""
+    g = torch.device(gen_device) if gen_device is not None else torch.device("cpu")
+    Le = extended_lattice(L, nranks)
+    Vh = layout.volume(Le) // 2
+    sites = global_sites_of_rank(L, rank, nranks, device=g)[parity * Vh:(parity + 1) * Vh]
+    src = inputs.sources(L, seed, sites, nrhs).to(cdtype)
+    if not fill_halo:
+        S = Vh // Le[3]
+        v = src.view(nrhs, Le[3], S, 3)
+        v[:, :HALO_T] = 0
+        v[:, Le[3] - HALO_T:] = 0
+    return src.contiguous().to(device)
+
+
+def exchange_halos(send_lo: torch.Tensor, send_hi: torch.Tensor, recv_lo: torch.Tensor, recv_hi: torch.Tensor,
+                   rank: int, nranks: int, dist=None):
+    """Periodic ring in t: my send_hi goes to rank+1's recv_lo, my send_lo to rank-1's recv_hi.
+    dist = torch.distributed (initialised) or None for a single rank (own halos: periodic wrap onto itself)."""
+    if nranks == 1 or dist is None:
+        recv_lo.copy_(send_hi)
+        recv_hi.copy_(send_lo)
+        return
+    up, down = (rank + 1) % nranks, (rank - 1) % nranks
+    ops = [dist.P2POp(dist.isend, send_hi, up), dist.P2POp(dist.irecv, recv_lo, down),
+           dist.P2POp(dist.isend, send_lo, down), dist.P2POp(dist.irecv, recv_hi, up)]
+    for w in dist.batch_isend_irecv(ops):
+        w.wait()
+
+
+def dslash_partitioned(ctx, field_in: torch.Tensor, parity: int, rank: int, nranks: int, dist=None, out=None):
+    """Halo exchange of `field_in` followed by the local Dslash (what one rank does per application)."""
+    n = field_in.shape[0]
+    slo, shi = ctx.halo_buffers(n)
+    rlo, rhi = ctx.halo_buffers(n)
+    ctx.halo_pack(field_in, slo, shi)
+    exchange_halos(slo, shi, rlo, rhi, rank, nranks, dist)
+    ctx.halo_unpack(field_in, rlo, rhi)
+    return ctx.dslash(field_in, parity, out=out)

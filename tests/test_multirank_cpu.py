@@ -50,3 +50,56 @@ def test_replicas_use_distinct_seeded_inputs():
     a = inputs.fat_links((4, 4, 4, 4), 0, s)
     b = inputs.fat_links((4, 4, 4, 4), 1, s)
     assert not torch.equal(a, b)
+
+
+# ---- row f3: halo exchange routing over a periodic ring of ranks (gloo, CPU tensors) ----
+def _halo_worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    from paper_2306_01098_b200 import partition
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    slo = torch.full((2, 3, 8), 10.0 * rank + 1, dtype=torch.complex128)   # my lowest interior slices
+    shi = torch.full((2, 3, 8), 10.0 * rank + 2, dtype=torch.complex128)   # my highest interior slices
+    rlo, rhi = torch.zeros_like(slo), torch.zeros_like(slo)
+    partition.exchange_halos(slo, shi, rlo, rhi, rank, world, dist)
+    q.put((rank, rlo[0, 0, 0].real.item(), rhi[0, 0, 0].real.item()))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_halo_exchange_ring_routing():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 31500 + os.getpid() % 2000
+    world = 3
+    ps = [ctx.Process(target=_halo_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in ps:
+        p.start()
+    res = {r: (lo, hi) for r, lo, hi in (q.get(timeout=120) for _ in ps)}
+    for p in ps:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for r in range(world):
+        lo, hi = res[r]
+        assert lo == 10.0 * ((r - 1) % world) + 2      # lower halo <- previous rank's highest slices
+        assert hi == 10.0 * ((r + 1) % world) + 1      # upper halo <- next rank's lowest slices
+
+
+def test_global_sites_of_rank_cover_the_lattice_once():
+    from paper_2306_01098_b200 import layout, partition
+    L, G = (4, 6, 4, 16), 4
+    Le = partition.extended_lattice(L, G)
+    V, Ve = layout.volume(L), layout.volume(Le)
+    S2 = Ve // Le[3]
+    count = torch.zeros(V, dtype=torch.int64)
+    for r in range(G):
+        sites = partition.global_sites_of_rank(L, r, G)
+        lex_e = layout.lex_of_eo(Le)
+        t_e = lex_e // (Le[0] * Le[1] * Le[2])
+        interior = (t_e >= partition.HALO_T) & (t_e < Le[3] - partition.HALO_T)
+        count.index_add_(0, sites[interior], torch.ones(int(interior.sum()), dtype=torch.int64))
+        # parity is preserved by the even halo depth: local parity half == global parity
+        x = sites % L[0]; y = (sites // L[0]) % L[1]; z = (sites // (L[0] * L[1])) % L[2]; t = sites // (L[0] * L[1] * L[2])
+        gpar = (x + y + z + t) & 1
+        assert torch.all(gpar[: Ve // 2] == 0) and torch.all(gpar[Ve // 2:] == 1)
+    assert torch.all(count == 1)
