@@ -46,8 +46,6 @@ template <typename T> struct DslashArgs {
     int naik_c13;        // 1: Naik links are stored compressed (13 reals, row f2)
 };
 
-template <typename T> __host__ __device__ constexpr size_t link_block_reals(int Vh) { return (size_t)Vh * 18; }
-
 // block of (field f, owner parity p, direction mu)
 template <typename T>
 __device__ __forceinline__ const T* link_block(const T* links, int Vh, int f, int p, int mu)

@@ -449,11 +449,6 @@ static const CgState* poll_wait(hisq_ctx* h, int slot)
     return (const CgState*)((char*)h->host_state + (size_t)slot * kPollSlot);
 }
 
-// Replay `count` iterations; with use_graph the batch is captured once and launched as one graph.
-struct IterBatch {
-    cudaGraphExec_t exec = nullptr;
-    int count = 0;
-};
 
 template <typename T, typename TB>
 static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_user, const TB* b, double mass, double tol, int nrhs)

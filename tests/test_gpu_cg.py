@@ -140,3 +140,25 @@ def test_cg_is_run_to_run_reproducible():
     x2, i2 = ctx.cg(b_dev, 0.1, 1e-10)
     assert torch.equal(x1, x2) and i1["iterations"] == i2["iterations"]
     ctx.close()
+
+
+def test_cg_on_a_side_stream_and_varying_nrhs():
+    """The context follows the caller's stream (torch side stream), and one context serves calls with different nrhs."""
+    L, m, tol = (4, 6, 8, 10), 0.15, 1e-9
+    ctx, X, W = make_ctx(L, "fp64", 4, 7)
+    side = torch.cuda.Stream()
+    b4, b4_full = make_field(ctx, L, 7, 4, 0)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        ctx.use_current_stream()
+        for n in (4, 1, 3):
+            b = b4[:n].contiguous()
+            x_dev, info = ctx.cg(b, m, tol)
+            x = to_full(ctx, L, x_dev, 0)
+            rr = _true_relres(L, X, W, m, x, b4_full[:n])
+            assert max(rr) <= tol, (n, rr)
+        t = ctx.dslash(b4, 1)
+        side.synchronize()
+    ref = oracle.dslash_parity(L, X, W, b4_full, 1)
+    assert rel_l2(to_full(ctx, L, t, 1), ref) <= 1e-14
+    ctx.close()
