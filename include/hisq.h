@@ -150,6 +150,26 @@ int hisq_halo_pack(hisq_ctx *h, void *send_lo, void *send_hi, const void *field,
 /* lower halo <- recv_lo (what the previous rank packed as send_hi), upper halo <- recv_hi (the next rank's send_lo). */
 int hisq_halo_unpack(hisq_ctx *h, void *field, const void *recv_lo, const void *recv_hi, int nrhs);
 
+/* CG on a t-partitioned lattice, phase by phase.  The solver's reductions span all ranks, so the iteration is cut where
+ * a cross-rank step is due and the CALLER performs it between the calls (halo exchange of a field through
+ * hisq_halo_pack / unpack, all-reduce (sum) of nrhs doubles); paper_2306_01098_b200/partition.py holds the loop.
+ *   hisq_cgp_begin(h, x, b, tol, nrhs)   x := 0, r := b (halo slices zeroed), LOCAL ||b_k||^2 -> rho
+ *       -> all-reduce rho ->                                      hisq_cgp_phase(h, 0, mass)
+ *   per iteration:  hisq_cgp_phase(h, 1, mass)   p = r + beta p                  -> halo exchange of p
+ *                   hisq_cgp_phase(h, 2, mass)   t = D_oe p                      -> halo exchange of t
+ *                   hisq_cgp_phase(h, 3, mass)   q = mass^2 p - D_eo t, LOCAL Re<p_k,q_k> -> pq      -> all-reduce pq
+ *                   hisq_cgp_phase(h, 4, mass)   x += alpha p, r -= alpha q, LOCAL ||r_k||^2 -> sums -> all-reduce sums
+ *                   hisq_cgp_phase(h, 5, mass)   beta_k, convergence flags, iteration count
+ *   hisq_cgp_status: synchronises and reports iterations, done, breakdown, recursive relative residuals (HOST arrays).
+ * x, b: NATIVE even fields on the extended lattice (halo slices of b are ignored, those of x are undefined).
+ * Same arithmetic and stopping rule as hisq_cg (no final true-residual check).  Works on ordinary contexts too
+ * (then no exchange is needed).  hisq_cgp_ptr: device pointers the caller needs: 0 = p, 1 = t (fields),
+ * 2 = rho, 3 = pq, 4 = sums (arrays of HISQ_MAX_NRHS doubles, the first nrhs are used). */
+int hisq_cgp_begin(hisq_ctx *h, void *x, const void *b, double tol, int nrhs);
+int hisq_cgp_phase(hisq_ctx *h, int phase, double mass);
+void *hisq_cgp_ptr(hisq_ctx *h, int which);
+int hisq_cgp_status(hisq_ctx *h, int *iterations, int *done, int *breakdown, double *rel_resid);
+
 /* Row f2 (the paper's CompressionType).  With option "naik_compress" = 1, the next hisq_set_links
  * stores each Naik link as 13 reals (rows 0, 1 and 1/c of W = c U, U in SU(3), c real; row 2 = conj(row0 x row1)/c is
  * rebuilt in registers) PROVIDED every Naik link passes |row2 - conj(row0 x row1)/c| <= tol |c| (tol 1e-12 fp64, 1e-5

@@ -25,7 +25,8 @@ EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
     "hisq_set_links", "hisq_dslash", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
     "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count",
-    "hisq_create_part", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack", "hisq_strerror",
+    "hisq_create_part", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
+    "hisq_cgp_begin", "hisq_cgp_phase", "hisq_cgp_ptr", "hisq_cgp_status", "hisq_strerror",
     "hisq_last_error",
 ]
 
@@ -70,6 +71,11 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_halo_bytes.restype = sz
     lib.hisq_halo_pack.argtypes = [vp, vp, vp, vp, i]
     lib.hisq_halo_unpack.argtypes = [vp, vp, vp, vp, i]
+    lib.hisq_cgp_begin.argtypes = [vp, vp, vp, d, i]
+    lib.hisq_cgp_phase.argtypes = [vp, i, d]
+    lib.hisq_cgp_ptr.argtypes = [vp, i]
+    lib.hisq_cgp_ptr.restype = vp
+    lib.hisq_cgp_status.argtypes = [vp, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(d)]
     lib.hisq_launch_count.argtypes = [vp]
     lib.hisq_launch_count.restype = ctypes.c_longlong
     lib.hisq_strerror.argtypes = [i]
@@ -255,6 +261,34 @@ class Hisq:
 
     def halo_unpack(self, field: torch.Tensor, lo: torch.Tensor, hi: torch.Tensor):
         self._check(self.lib.hisq_halo_unpack(self._h, self._ptr(field), self._ptr(lo), self._ptr(hi), field.shape[0]))
+
+    # -- phase-wise CG (partitioned lattices) ------------------------------------------------------
+    def cgp_begin(self, x: torch.Tensor, b: torch.Tensor, tol: float):
+        n = b.shape[0]
+        self._check(self.lib.hisq_cgp_begin(self._h, self._ptr(x, (n, 3, self.Vh), self.cdtype),
+                                            self._ptr(b, (n, 3, self.Vh), self.cdtype), float(tol), n))
+
+    def cgp_phase(self, phase: int, mass: float):
+        self._check(self.lib.hisq_cgp_phase(self._h, int(phase), float(mass)))
+
+    def cgp_tensor(self, which: int, nrhs: int) -> torch.Tensor:
+        """A torch view (no copy) of library-owned device memory: 0/1 = the p / t field [nrhs, 3, Vh]; 2/3/4 = rho / pq /
+        sums [nrhs] float64 -- what the caller exchanges / all-reduces between phases."""
+        ptr = self.lib.hisq_cgp_ptr(self._h, int(which))
+        if not ptr:
+            raise HisqError(-1, "hisq_cgp_ptr")
+        base = ptr - self.workspace.data_ptr()
+        if which in (0, 1):
+            nbytes = nrhs * 3 * self.Vh * (8 if self.prec == "fp32" else 16)
+            return self.workspace[base:base + nbytes].view(self.cdtype).view(nrhs, 3, self.Vh)
+        return self.workspace[base:base + 8 * nrhs].view(torch.float64)
+
+    def cgp_status(self, nrhs: int) -> dict:
+        it, dn, br = ctypes.c_int(0), ctypes.c_int(0), ctypes.c_int(0)
+        res = (ctypes.c_double * HISQ_MAX_NRHS)()
+        self._check(self.lib.hisq_cgp_status(self._h, ctypes.byref(it), ctypes.byref(dn), ctypes.byref(br), res))
+        return {"iterations": it.value, "done": bool(dn.value), "breakdown": bool(br.value),
+                "rel_resid": [res[k] for k in range(nrhs)]}
 
     def naik_compressed(self) -> bool:
         return bool(self.lib.hisq_naik_compressed(self._h))

@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_p_kernel(T* __restrict__
 template <typename T>
 __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict__ x, T* __restrict__ r, const T* __restrict__ p,
                                                                   const T* __restrict__ q, size_t nreal, CgState* st,
-                                                                  double* partial)
+                                                                  double* partial, int defer = 0)
 {
     if (st->done) return;
     using V = typename V16<T>::type;
@@ -156,6 +156,10 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict_
     if (grid_reduce<1, kBlasBlock>(sum, k, partial, gridDim.x, blockIdx.x, &st->ticket[1], gridDim.x * gridDim.y, gridDim.y,
                                    totals)) {
         const int n = gridDim.y;
+        if (defer) {   // partitioned lattice: only the LOCAL sums; the scalar update runs after the cross-rank all-reduce
+            if (threadIdx.x < n) st->sums[threadIdx.x] = totals[threadIdx.x];
+            return;
+        }
         if (threadIdx.x < n) {
             const int kk = threadIdx.x;
             if (st->active[kk]) {
@@ -291,6 +295,56 @@ __global__ void __launch_bounds__(kBlasBlock) cg_fused_update_kernel(T* __restri
             for (int e = 0; e < N; ++e) pk[j][e] = fma(beta, pk[j][e], rk[j][e]);
             pv[i] = pack16<T>(pk[j]);
         }
+    }
+}
+
+// ---- partitioned-lattice CG (row f3): scalar updates that consume GLOBAL (all-reduced) sums ------------------------
+__global__ void cgp_finalize_init_kernel(CgState* st, int n, double tol, int max_iter)
+{
+    int any = 0;
+    for (int k = 0; k < n; ++k) {
+        const double bb = st->rho[k];       // all-reduced ||b_k||^2
+        st->rho_prev[k] = bb; st->bnorm2[k] = bb; st->pq[k] = 1.0; st->beta[k] = 0.0; st->sums[k] = 0.0;
+        st->active[k] = bb > 0.0 ? 1 : 0;
+        any |= st->active[k];
+    }
+    st->tol2 = tol * tol; st->iter = 0; st->max_iter = max_iter; st->breakdown = 0; st->nrhs = n;
+    st->done = any ? 0 : 1;
+}
+
+__global__ void cgp_finalize_xr_kernel(CgState* st, int n)
+{
+    if (st->done) return;
+    int any = 0;
+    for (int k = 0; k < n; ++k) {
+        if (st->active[k]) {
+            const double rn = st->sums[k], pq = st->pq[k];   // both all-reduced
+            if (!(pq > 0.0) || !isfinite(pq) || !isfinite(rn)) st->breakdown = 1;
+            st->rho_prev[k] = st->rho[k];
+            st->beta[k] = rn / st->rho[k];
+            st->rho[k] = rn;
+            if (rn <= st->tol2 * st->bnorm2[k]) st->active[k] = 0;
+        }
+        any |= st->active[k];
+    }
+    const int it = st->iter + 1;
+    st->iter = it;
+    if (!any || it >= st->max_iter || st->breakdown) st->done = 1;
+}
+
+// zero the halo slices of a native field, so that sums over the whole extended array are sums over the interior
+template <typename T>
+__global__ void __launch_bounds__(256) zero_halo_kernel(T* __restrict__ field, int S, int Lt_ext, int t_lo, int t_cnt, int nrhs)
+{
+    using C = typename Vec<T>::c1;
+    C* f = reinterpret_cast<C*>(field);
+    const size_t per_plane = (size_t)(Lt_ext - t_cnt) * S, total = (size_t)nrhs * 3 * per_plane;
+    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < total; i += (size_t)gridDim.x * 256) {
+        const size_t kc = i / per_plane;
+        size_t j = i % per_plane;
+        if (j >= (size_t)t_lo * S) j += (size_t)t_cnt * S;     // skip the interior
+        C z; z.x = 0; z.y = 0;
+        f[kc * (size_t)Lt_ext * S + j] = z;
     }
 }
 

@@ -34,6 +34,7 @@ struct hisq_ctx {
     bool naik_c13;         // Naik links currently stored compressed
     int naik_compress;     // option: try to compress at the next hisq_set_links
     int fused_blas;        // option: cooperative fused x/r/p update for small fields
+    void* cgp_x; int cgp_nrhs; double cgp_tol;   // phase-wise CG on partitioned lattices
     int num_sms;
     unsigned long long* bad_count;  // device counter used by the compression check
     // options
@@ -119,6 +120,7 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     h->nrhs_inner = 0;
     h->naik_c13 = false; h->naik_compress = 0; h->bad_count = nullptr;
     h->fused_blas = 1; h->num_sms = 0;
+    h->cgp_x = nullptr; h->cgp_nrhs = 0; h->cgp_tol = 0.0;
     { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev); }
     h->tile_y = 0; h->tile_z = 0;
     h->window_mb = 40.0;
@@ -823,6 +825,109 @@ extern "C" int hisq_cg_host(hisq_ctx* h, void* x_host, const void* b_host, doubl
     CK(cudaMemcpyAsync(x_host, c_out, bytes, cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
     return solve_rc;
+}
+
+// ---- partitioned-lattice CG (row f3): the iteration is cut into phases; between phases the CALLER exchanges halos
+// and all-reduces the per-RHS sums across ranks (torch.distributed / NCCL), see partition.PartitionedCG. -----------------
+struct CgpFields { void *r, *p, *q, *t; };
+static CgpFields cgp_fields(hisq_ctx* h)
+{
+    const size_t fb = field_bytes(h, h->ws_nrhs, elem_size(h->prec));
+    return { h->fields, h->fields + fb, h->fields + 2 * fb, h->fields + 3 * fb };
+}
+
+template <typename T>
+static int cgp_begin(hisq_ctx* h, T* x, const T* b, double tol, int nrhs)
+{
+    const size_t nreal = (size_t)6 * h->g.Vh, total = nreal * nrhs;
+    CgpFields f = cgp_fields(h);
+    CK(cudaMemsetAsync(x, 0, total * sizeof(T), h->stream));
+    CK(cudaMemsetAsync(f.p, 0, total * sizeof(T), h->stream));
+    CK(cudaMemsetAsync(f.q, 0, total * sizeof(T), h->stream));
+    CK(cudaMemsetAsync(f.t, 0, total * sizeof(T), h->stream));
+    const int S = h->g.Vh / h->g.L[3];
+    // r = b, then r's halo := 0 so that ||r||^2 over the extended array is the interior sum; LOCAL ||b||^2 -> state.rho
+    cudaMemcpyAsync(f.r, b, total * sizeof(T), cudaMemcpyDeviceToDevice, h->stream);
+    zero_halo_kernel<T><<<148 * 4, 256, 0, h->stream>>>((T*)f.r, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, nrhs);
+    dim3 gi((unsigned)init_grid_x(nreal), (unsigned)nrhs);
+    cg_init_kernel<T, T><<<gi, kBlasBlock, 0, h->stream>>>((const T*)f.r, (T*)f.r, nreal, h->state, h->partial, tol, h->max_iter);
+    h->stats.launches += 2;
+    CK(cudaGetLastError());
+    h->cgp_x = x; h->cgp_nrhs = nrhs; h->cgp_tol = tol;
+    return HISQ_OK;
+}
+
+template <typename T>
+static int cgp_phase(hisq_ctx* h, const T* links, int phase, double mass)
+{
+    const int nrhs = h->cgp_nrhs;
+    if (nrhs < 1 || !h->cgp_x) return HISQ_EINVAL;
+    const size_t nreal = (size_t)6 * h->g.Vh;
+    CgpFields f = cgp_fields(h);
+    T *r = (T*)f.r, *p = (T*)f.p, *q = (T*)f.q, *t = (T*)f.t, *x = (T*)h->cgp_x;
+    dim3 gb((unsigned)blas_grid_x(nreal, V16<T>::n), (unsigned)nrhs);
+    switch (phase) {
+    case 0:  // after the all-reduce of rho (= ||b||^2)
+        cgp_finalize_init_kernel<<<1, 1, 0, h->stream>>>(h->state, nrhs, h->cgp_tol, h->max_iter);
+        h->stats.launches++;
+        break;
+    case 1: return enqueue_p_update<T>(h, p, r, nrhs);
+    case 2: return run_dslash<T>(h, links, t, p, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, &h->state->done, 2);
+    case 3: return run_dslash<T>(h, links, q, t, HISQ_EVEN, nrhs, MODE_APPLY_A, p, nullptr, mass * mass, h->state->pq, &h->state->done, 2);
+    case 4:
+        cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial, 1);
+        h->stats.launches++;
+        break;
+    case 5:  // after the all-reduce of sums (= ||r||^2)
+        cgp_finalize_xr_kernel<<<1, 1, 0, h->stream>>>(h->state, nrhs);
+        h->stats.launches++;
+        break;
+    default: return HISQ_EINVAL;
+    }
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+
+extern "C" int hisq_cgp_begin(hisq_ctx* h, void* x, const void* b, double tol, int nrhs)
+{
+    if (!h || !x || !b || nrhs < 1 || nrhs > HISQ_MAX_NRHS || !(tol > 0.0)) return HISQ_EINVAL;
+    if (!h->ws || nrhs > h->ws_nrhs) return HISQ_ENOWORKSPACE;
+    if (!h->have_links) return HISQ_ENOLINKS;
+    if (h->prec == HISQ_MIXED) return HISQ_EINVAL;
+    return h->prec == HISQ_FP32 ? cgp_begin<float>(h, (float*)x, (const float*)b, tol, nrhs)
+                                : cgp_begin<double>(h, (double*)x, (const double*)b, tol, nrhs);
+}
+extern "C" int hisq_cgp_phase(hisq_ctx* h, int phase, double mass)
+{
+    if (!h || h->prec == HISQ_MIXED) return HISQ_EINVAL;
+    return h->prec == HISQ_FP32 ? cgp_phase<float>(h, h->links32, phase, mass) : cgp_phase<double>(h, h->links64, phase, mass);
+}
+// which: 0 = p field, 1 = t field (halo exchange); 2 = rho, 3 = pq, 4 = sums (kMaxNrhs doubles each; all-reduce the first nrhs)
+extern "C" void* hisq_cgp_ptr(hisq_ctx* h, int which)
+{
+    if (!h || !h->ws) return nullptr;
+    CgpFields f = cgp_fields(h);
+    switch (which) {
+    case 0: return f.p;
+    case 1: return f.t;
+    case 2: return h->state->rho;
+    case 3: return h->state->pq;
+    case 4: return h->state->sums;
+    default: return nullptr;
+    }
+}
+extern "C" int hisq_cgp_status(hisq_ctx* h, int* iterations, int* done, int* breakdown, double* rel_resid)
+{
+    if (!h || !h->ws) return HISQ_EINVAL;
+    int rc = poll_state(h);
+    if (rc) return rc;
+    const CgState& s = *h->host_state;
+    if (iterations) *iterations = s.iter;
+    if (done) *done = s.done;
+    if (breakdown) *breakdown = s.breakdown;
+    if (rel_resid)
+        for (int k = 0; k < s.nrhs && k < kMaxNrhs; ++k) rel_resid[k] = s.bnorm2[k] > 0.0 ? std::sqrt(s.rho[k] / s.bnorm2[k]) : 0.0;
+    return HISQ_OK;
 }
 
 extern "C" size_t hisq_halo_bytes(const hisq_ctx* h, int nrhs)

@@ -83,3 +83,49 @@ def dslash_partitioned(ctx, field_in: torch.Tensor, parity: int, rank: int, nran
     exchange_halos(slo, shi, rlo, rhi, rank, nranks, dist)
     ctx.halo_unpack(field_in, rlo, rhi)
     return ctx.dslash(field_in, parity, out=out)
+
+
+class PartitionedCG:
+    """One rank's side of the multi-RHS CG on a t-partitioned lattice (include/hisq.h, hisq_cgp_*): every kernel is the
+    library's; this class only sequences the phases and performs the two cross-rank steps between them -- halo
+    exchange of a field and all-reduce of nrhs doubles -- through `dist` (torch.distributed: NCCL between GPUs)."""
+
+    def __init__(self, ctx, rank: int, nranks: int, dist=None):
+        self.ctx, self.rank, self.nranks, self.dist = ctx, rank, nranks, dist
+
+    def _halo(self, field):
+        n = field.shape[0]
+        slo, shi = self.ctx.halo_buffers(n)
+        rlo, rhi = self.ctx.halo_buffers(n)
+        self.ctx.halo_pack(field, slo, shi)
+        exchange_halos(slo, shi, rlo, rhi, self.rank, self.nranks, self.dist)
+        self.ctx.halo_unpack(field, rlo, rhi)
+
+    def _allreduce(self, t):
+        if self.dist is not None and self.nranks > 1:
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
+
+    def solve(self, b, mass: float, tol: float, x=None, check_every: int = 16, max_iter: int = 100000):
+        c = self.ctx
+        n = b.shape[0]
+        if x is None:
+            x = c.new_field(n)
+        p, t = c.cgp_tensor(0, n), c.cgp_tensor(1, n)
+        rho, pq, sums = c.cgp_tensor(2, n), c.cgp_tensor(3, n), c.cgp_tensor(4, n)
+        c.cgp_begin(x, b, tol)
+        self._allreduce(rho)
+        c.cgp_phase(0, mass)
+        st = c.cgp_status(n)
+        while not st["done"] and st["iterations"] < max_iter:
+            for _ in range(check_every):
+                c.cgp_phase(1, mass)
+                self._halo(p)
+                c.cgp_phase(2, mass)
+                self._halo(t)
+                c.cgp_phase(3, mass)
+                self._allreduce(pq)
+                c.cgp_phase(4, mass)
+                self._allreduce(sums)
+                c.cgp_phase(5, mass)
+            st = c.cgp_status(n)
+        return x, st

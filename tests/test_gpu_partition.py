@@ -94,3 +94,103 @@ def test_partitioned_context_rejects_solvers_and_bad_splits():
         binding.Hisq((4, 4, 4, 12), "fp64", 1, part=(0, 4))      # Lt_loc = 3: odd
     with pytest.raises(ValueError):
         binding.Hisq((4, 4, 4, 8), "fp64", 1, part=(0, 4))       # Lt_loc = 2 < 4
+
+
+def _emulated_cg(L, prec, nranks, nrhs, m, tol, seed):
+    """All ranks in lockstep on one GPU: every phase is run for rank 0..G-1 in turn, the cross-rank steps (ring halo
+    exchange, all-reduce) are done by hand between the phases -- the same sequence as partition.PartitionedCG.solve."""
+    dev = torch.device("cuda:0")
+    ctxs, bs, xs = [], [], []
+    for r in range(nranks):
+        ctx = binding.Hisq(L, prec, nrhs, dev, part=(r, nranks))
+        fat, naik = partition.make_links_part(L, seed, r, nranks, dev, ctx.cdtype)
+        ctx.set_links(fat, naik)
+        b = ctx.pack(partition.make_sources_part(L, seed + 1, nrhs, 0, r, nranks, dev, ctx.cdtype, fill_halo=True))
+        x = ctx.new_field(nrhs)
+        ctx.cgp_begin(x, b, tol)
+        ctxs.append(ctx); bs.append(b); xs.append(x)
+
+    def allreduce(which):
+        ts = [c.cgp_tensor(which, nrhs) for c in ctxs]
+        tot = torch.stack(ts).sum(0)
+        for t in ts:
+            t.copy_(tot)
+
+    def halo(which):
+        fields = [c.cgp_tensor(which, nrhs) for c in ctxs]
+        bufs = []
+        for c, f in zip(ctxs, fields):
+            slo, shi = c.halo_buffers(nrhs)
+            c.halo_pack(f, slo, shi)
+            bufs.append((slo, shi))
+        for r, (c, f) in enumerate(zip(ctxs, fields)):
+            c.halo_unpack(f, bufs[(r - 1) % nranks][1], bufs[(r + 1) % nranks][0])
+
+    allreduce(2)
+    for c in ctxs:
+        c.cgp_phase(0, m)
+    st = ctxs[0].cgp_status(nrhs)
+    while not st["done"] and st["iterations"] < 5000:
+        for _ in range(16):
+            for c in ctxs: c.cgp_phase(1, m)
+            halo(0)
+            for c in ctxs: c.cgp_phase(2, m)
+            halo(1)
+            for c in ctxs: c.cgp_phase(3, m)
+            allreduce(3)
+            for c in ctxs: c.cgp_phase(4, m)
+            allreduce(4)
+            for c in ctxs: c.cgp_phase(5, m)
+        st = ctxs[0].cgp_status(nrhs)
+    for c in ctxs[1:]:
+        assert c.cgp_status(nrhs)["iterations"] == st["iterations"]
+    # gather the interiors of x
+    V = layout.volume(L)
+    full = np.zeros((nrhs, V, 3), dtype=np.complex128)
+    Le = partition.extended_lattice(L, nranks)
+    Vh_e = layout.volume(Le) // 2
+    S = Vh_e // Le[3]
+    for r, c in enumerate(ctxs):
+        sites = partition.global_sites_of_rank(L, r, nranks).numpy()[:Vh_e]
+        interior = np.zeros(Vh_e, dtype=bool)
+        interior.reshape(Le[3], S)[partition.HALO_T:Le[3] - partition.HALO_T] = True
+        full[:, sites[interior]] = c.unpack(xs[r]).cpu().numpy().astype(np.complex128)[:, interior]
+        c.close()
+    return full, st
+
+
+@pytest.mark.parametrize("nranks", [1, 2, 4])
+def test_partitioned_cg_matches_oracle_and_single_lattice(nranks):
+    L, nrhs, m, tol, seed = (4, 6, 4, 16), 2, 0.1, 1e-10, 5
+    x, st = _emulated_cg(L, "fp64", nranks, nrhs, m, tol, seed)
+    X, W = oracle_links(L, seed)
+    b = oracle_field(L, seed + 1, nrhs, parity=0)
+    r = b - oracle.apply_A(L, X, W, m, x)
+    for k in range(nrhs):
+        assert np.linalg.norm(r[k]) / np.linalg.norm(b[k]) <= 1.05 * tol, (k, st)
+    xo, it_o, _, ok, _ = oracle.cg(L, X, W, m, tol, b)
+    assert ok == 0 and rel_l2(x, xo) <= 10 * tol
+    assert abs(st["iterations"] - int(it_o.max())) <= 16 + 3      # status is polled every 16 iterations
+
+
+def test_partitioned_cg_driver_single_rank_equals_hisq_cg():
+    """partition.PartitionedCG itself (dist = None: the ring closes on the rank) against hisq_cg on the plain lattice."""
+    L, m, tol, seed = (4, 4, 6, 8), 0.2, 1e-10, 6
+    dev = torch.device("cuda:0")
+    ctx = binding.Hisq(L, "fp64", 1, dev, part=(0, 1))
+    fat, naik = partition.make_links_part(L, seed, 0, 1, dev)
+    ctx.set_links(fat, naik)
+    b = ctx.pack(partition.make_sources_part(L, seed + 1, 1, 0, 0, 1, dev))
+    x, st = partition.PartitionedCG(ctx, 0, 1).solve(b, m, tol, check_every=8)
+    assert st["done"] and max(st["rel_resid"]) <= tol
+    ref = binding.Hisq(L, "fp64", 1, dev)
+    f2, n2 = binding.make_links(L, seed, dev)
+    ref.set_links(f2, n2)
+    xr, info = ref.cg(ref.pack(binding.make_sources(L, seed + 1, 1, 0, dev)), m, tol)
+    # interior of the partitioned solution == the plain solution
+    Le = partition.extended_lattice(L, 1)
+    S = ctx.Vh // Le[3]
+    xi = ctx.unpack(x).view(1, Le[3], S, 3)[:, partition.HALO_T:Le[3] - partition.HALO_T].reshape(1, -1, 3)
+    assert rel_l2(xi.cpu().numpy(), ref.unpack(xr).cpu().numpy()) <= 1e-9
+    assert abs(st["iterations"] - info["iterations"]) <= 8 + 2
+    ctx.close(); ref.close()
