@@ -68,10 +68,29 @@ def exchange_halos(send_lo: torch.Tensor, send_hi: torch.Tensor, recv_lo: torch.
         recv_hi.copy_(send_lo)
         return
     up, down = (rank + 1) % nranks, (rank - 1) % nranks
-    ops = [dist.P2POp(dist.isend, send_hi, up), dist.P2POp(dist.irecv, recv_lo, down),
-           dist.P2POp(dist.isend, send_lo, down), dist.P2POp(dist.irecv, recv_hi, up)]
-    for w in dist.batch_isend_irecv(ops):
-        w.wait()
+    # NCCL moves device buffers directly (NVLink); gloo (CPU tests, or two processes sharing one GPU) goes through the host
+    stage = send_lo.is_cuda and dist.get_backend() != "nccl"
+    # communicate as real arrays (not every backend knows complex dtypes)
+    real = lambda t: torch.view_as_real(t) if t.is_complex() else t
+    s_lo, s_hi = (real(send_lo.cpu()), real(send_hi.cpu())) if stage else (real(send_lo), real(send_hi))
+    r_lo, r_hi = (torch.empty_like(s_lo), torch.empty_like(s_hi)) if stage else (real(recv_lo), real(recv_hi))
+    if nranks == 2:
+        # both neighbours are the same peer: two tagged exchanges, lower rank sends first (no reliance on message order)
+        for tag, (snd, rcv) in enumerate(((s_hi, r_lo), (s_lo, r_hi))):
+            if rank == 0:
+                dist.send(snd, up, tag=tag)
+                dist.recv(rcv, up, tag=tag)
+            else:
+                dist.recv(rcv, up, tag=tag)
+                dist.send(snd, up, tag=tag)
+    else:
+        ops = [dist.P2POp(dist.isend, s_hi, up), dist.P2POp(dist.irecv, r_lo, down),
+               dist.P2POp(dist.isend, s_lo, down), dist.P2POp(dist.irecv, r_hi, up)]
+        for w in dist.batch_isend_irecv(ops):
+            w.wait()
+    if stage:
+        real(recv_lo).copy_(r_lo)
+        real(recv_hi).copy_(r_hi)
 
 
 def dslash_partitioned(ctx, field_in: torch.Tensor, parity: int, rank: int, nranks: int, dist=None, out=None):
@@ -103,7 +122,12 @@ class PartitionedCG:
 
     def _allreduce(self, t):
         if self.dist is not None and self.nranks > 1:
-            self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
+            if t.is_cuda and self.dist.get_backend() != "nccl":
+                h = t.cpu()
+                self.dist.all_reduce(h, op=self.dist.ReduceOp.SUM)
+                t.copy_(h)
+            else:
+                self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
 
     def solve(self, b, mass: float, tol: float, x=None, check_every: int = 16, max_iter: int = 100000):
         c = self.ctx

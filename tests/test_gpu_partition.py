@@ -194,3 +194,52 @@ def test_partitioned_cg_driver_single_rank_equals_hisq_cg():
     assert rel_l2(xi.cpu().numpy(), ref.unpack(xr).cpu().numpy()) <= 1e-9
     assert abs(st["iterations"] - info["iterations"]) <= 8 + 2
     ctx.close(); ref.close()
+
+
+def _mp_worker(rank, world, port, L, m, tol, seed, q):
+    import os, sys
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import torch.distributed as dist
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    dev = torch.device("cuda:0")                       # both ranks share the one GPU; no kernel waits on another
+    ctx = binding.Hisq(L, "fp64", 1, dev, part=(rank, world))
+    fat, naik = partition.make_links_part(L, seed, rank, world, dev)
+    ctx.set_links(fat, naik)
+    b = ctx.pack(partition.make_sources_part(L, seed + 1, 1, 0, rank, world, dev))
+    x, st = partition.PartitionedCG(ctx, rank, world, dist).solve(b, m, tol, check_every=8)
+    Le = partition.extended_lattice(L, world)
+    S = ctx.Vh // Le[3]
+    xi = ctx.unpack(x).view(1, Le[3], S, 3)[:, partition.HALO_T:Le[3] - partition.HALO_T].reshape(1, -1, 3).cpu()
+    xr = torch.view_as_real(xi).contiguous()
+    parts = [torch.empty_like(xr) for _ in range(world)] if rank == 0 else None
+    dist.gather(xr, parts, dst=0)
+    if rank == 0:
+        q.put((st, [torch.view_as_complex(p).numpy() for p in parts]))
+    dist.barrier()
+    ctx.close()
+    dist.destroy_process_group()
+
+
+def test_partitioned_cg_two_processes_gloo_on_one_gpu():
+    """The real thing minus the second GPU: two PROCESSES, each with its own context, exchanging halos and all-reducing
+    through torch.distributed (gloo here, NCCL between GPUs), run partition.PartitionedCG.solve."""
+    import torch.multiprocessing as mp
+    L, m, tol, seed, world = (4, 4, 6, 16), 0.15, 1e-9, 8, 2
+    ctxmp = mp.get_context("spawn")
+    q = ctxmp.Queue()
+    port = 33500 + __import__("os").getpid() % 2000
+    ps = [ctxmp.Process(target=_mp_worker, args=(r, world, port, L, m, tol, seed, q)) for r in range(world)]
+    for p in ps:
+        p.start()
+    st, parts = q.get(timeout=150)
+    for p in ps:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    assert st["done"] and not st["breakdown"]
+    # rank r's interior = global even sites with t in [r*Lt_loc, (r+1)*Lt_loc), in global half-index order
+    xh = np.concatenate(parts, axis=1).astype(np.complex128)
+    x = oracle.half_to_full(L, xh, 0)
+    X, W = oracle_links(L, seed)
+    b = oracle_field(L, seed + 1, 1, parity=0)
+    r = b - oracle.apply_A(L, X, W, m, x)
+    assert np.linalg.norm(r) / np.linalg.norm(b) <= 1.05 * tol

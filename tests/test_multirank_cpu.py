@@ -67,11 +67,14 @@ def _halo_worker(rank, world, port, q):
     dist.destroy_process_group()
 
 
-def test_halo_exchange_ring_routing():
+import pytest
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_halo_exchange_ring_routing(world):
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    port = 31500 + os.getpid() % 2000
-    world = 3
+    port = 31500 + os.getpid() % 2000 + world
     ps = [ctx.Process(target=_halo_worker, args=(r, world, port, q)) for r in range(world)]
     for p in ps:
         p.start()
