@@ -374,6 +374,8 @@ def main():
 
     if rank == 0 and not args.no_sweep:
         out["sweep"] = sweep_c3(dev, peak, args.dslash_reps)
+    if rank == 0 and not args.no_sweep:
+        out["paper_shape_sweep"] = sweep_paper_shape(dev, max(10, args.dslash_reps // 4))
     if rank == 0 and not args.no_cpu_baseline:
         g, dt, iters, cores = oracle_sample(cfg, 0, args.cpu_budget)
         out["cpu_baseline"] = {"value": g, "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
@@ -406,6 +408,27 @@ def run_dslash_only(args, cfg):
                       "frac_of_measured_copy": by / (ms * 1e-3) / 1e9 / peak, "frac_of_8TBs": by / (ms * 1e-3) / 1e9 / 8000.0,
                       "tiles": ctx.tiles(n), "launches": ctx.launch_count()}))
     ctx.close()
+
+
+# Table 1 of the paper: Dslash TFLOP/s on a 32^4 lattice, other hardware -- context, not a target
+PAPER_TABLE1 = {"nrhs": [1, 2, 3, 4, 6, 8], "A100_fp32": [1.36, 2.36, 2.85, 3.98, 4.97, 4.95], "A100_fp64": [0.70, 1.19, 1.45, 1.92, 2.20, 2.51],
+                "MI250x_GCD_fp32": [0.93, 1.65, 2.06, 2.36, 2.96, 2.79], "MI250x_GCD_fp64": [0.45, 0.85, 1.14, 0.97, 0.91, 0.95]}
+
+
+def sweep_paper_shape(dev, reps):
+    """The paper's own benchmark shape (32^4, nRHS = 1,2,3,4,6,8, fp32 and fp64; Fig. 5 / Table 1), on this B200."""
+    from paper_2306_01098_b200 import binding
+    L = (32, 32, 32, 32)
+    res = {"workload": "32x32x32x32 Dslash, TFLOP/s at 1146 flop/site/RHS", "paper_table1_context": PAPER_TABLE1}
+    for prec in ("fp32", "fp64"):
+        ctx = binding.Hisq(L, prec, 8, dev)
+        fat, naik = binding.make_links(L, 0, dev, ctx.cdtype, gen_device=dev)
+        ctx.set_links(fat, naik)
+        del fat, naik
+        res["b200_" + prec] = [round(FLOP_PER_SITE * ctx.Vh * n / (time_dslash(ctx, n, reps) * 1e-3) / 1e12, 3)
+                               for n in PAPER_TABLE1["nrhs"]]
+        ctx.close()
+    return res
 
 
 def sweep_c3(dev, peak, reps):

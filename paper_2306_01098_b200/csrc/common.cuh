@@ -15,12 +15,69 @@ template <> struct Vec<float>  { using c1 = float2; using c2 = float4; };  // on
 // ---- global loads with cache hints ---------------------------------------------------------------
 // Links are read exactly once per Dslash application (every link is used forward by its
 // own site and backward by the site it points to), so they stream: no L1 allocation, evict-first.
-__device__ __forceinline__ double2 ld_stream(const double2* p) { return __ldcs(p); }
-__device__ __forceinline__ float4 ld_stream(const float4* p) { return __ldcs(p); }
-__device__ __forceinline__ float2 ld_stream(const float2* p) { return __ldcs(p); }
+#ifndef HISQ_LINK_LD
+#define HISQ_LINK_LD 0   // 0: ld.global.cs (streaming); 1: ld.global.nc.L1::no_allocate; 2: plain read-only (ld.global.nc)
+#endif
+#ifndef HISQ_VEC_LD
+#define HISQ_VEC_LD 0    // 0: ld.global.nc; 1: ld.global.nc.L1::evict_last
+#endif
+__device__ __forceinline__ double2 ld_stream(const double2* p)
+{
+#if HISQ_LINK_LD == 1
+    double2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    return r;
+#elif HISQ_LINK_LD == 2
+    return __ldg(p);
+#else
+    return __ldcs(p);
+#endif
+}
+__device__ __forceinline__ float4 ld_stream(const float4* p)
+{
+#if HISQ_LINK_LD == 1
+    float4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+    return r;
+#elif HISQ_LINK_LD == 2
+    return __ldg(p);
+#else
+    return __ldcs(p);
+#endif
+}
+__device__ __forceinline__ float2 ld_stream(const float2* p)
+{
+#if HISQ_LINK_LD == 1
+    float2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
+    return r;
+#elif HISQ_LINK_LD == 2
+    return __ldg(p);
+#else
+    return __ldcs(p);
+#endif
+}
 // Colour vectors are gathered by 16 different output sites: keep them in L1/L2.
-__device__ __forceinline__ double2 ld_keep(const double2* p) { return __ldg(p); }
-__device__ __forceinline__ float2 ld_keep(const float2* p) { return __ldg(p); }
+__device__ __forceinline__ double2 ld_keep(const double2* p)
+{
+#if HISQ_VEC_LD == 1
+    double2 r;
+    asm volatile("ld.global.nc.L1::evict_last.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+    return r;
+#else
+    return __ldg(p);
+#endif
+}
+__device__ __forceinline__ float2 ld_keep(const float2* p)
+{
+#if HISQ_VEC_LD == 1
+    float2 r;
+    asm volatile("ld.global.nc.L1::evict_last.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
+    return r;
+#else
+    return __ldg(p);
+#endif
+}
 __device__ __forceinline__ float4 ld_keep(const float4* p) { return __ldg(p); }
 
 // ---- lattice geometry handed to kernels ----------------------------------------------------------
