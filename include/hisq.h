@@ -86,6 +86,12 @@ int hisq_set_links(hisq_ctx *h, const void *fat, const void *naik);
  * (PAPER.md:582-586).  in / out: NATIVE half-lattice fields, must not overlap.  Asynchronous. */
 int hisq_dslash(hisq_ctx *h, void *out, const void *in, int parity, int nrhs);
 
+/* out = (mass^2 - D_eo D_oe) in on even sites for nrhs fields: the operator the solvers invert (PAPER.md:139-141
+ * `applyMdaggM`), two Dslash launches, the second fused with the m^2 term.  in / out: NATIVE even half-lattice fields,
+ * must not overlap; uses the workspace (sized for >= nrhs).  HISQ_MIXED runs it in fp64.  Asynchronous.  Not available on
+ * partitioned contexts. */
+int hisq_apply_A(hisq_ctx *h, void *out, const void *in, double mass, int nrhs);
+
 /* Solve (mass^2 - D_eo D_oe) x_k = b_k, k < nrhs, on even sites by conjugate gradient with
  * independent alpha_k, beta_k per right-hand side and a shared operator application
  * (PAPER.md:135, :141).  b, x: NATIVE even half-lattice fields; x is overwritten (initial guess 0).

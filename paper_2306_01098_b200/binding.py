@@ -23,7 +23,7 @@ LIB_PATH = os.environ.get("HISQ_LIB", os.path.join(_HERE, "libhisq.so"))
 
 EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
-    "hisq_set_links", "hisq_dslash", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
+    "hisq_set_links", "hisq_dslash", "hisq_apply_A", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
     "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count",
     "hisq_create_part", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
     "hisq_cgp_begin", "hisq_cgp_phase", "hisq_cgp_ptr", "hisq_cgp_status", "hisq_strerror",
@@ -58,6 +58,7 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_set_links.argtypes = [vp, vp, vp]
     lib.hisq_dslash.argtypes = [vp, vp, vp, i, i]
     lib.hisq_cg.argtypes = [vp, vp, vp, d, d, i]
+    lib.hisq_apply_A.argtypes = [vp, vp, vp, d, i]
     lib.hisq_cg_multishift.argtypes = [vp, vp, vp, d, ctypes.POINTER(d), i, d]
     lib.hisq_set_option.argtypes = [vp, ctypes.c_char_p, d]
     lib.hisq_get_info.argtypes = [vp, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(d)]
@@ -196,6 +197,14 @@ class Hisq:
             out = self.new_field(n)
         self._check(self.lib.hisq_dslash(self._h, self._ptr(out, (n, 3, self.Vh), self.cdtype),
                                          self._ptr(inp, (n, 3, self.Vh), self.cdtype), int(parity), n))
+        return out
+
+    def apply_A(self, inp: torch.Tensor, mass: float, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        n = inp.shape[0]
+        if out is None:
+            out = self.new_field(n)
+        self._check(self.lib.hisq_apply_A(self._h, self._ptr(out, (n, 3, self.Vh), self.cdtype),
+                                          self._ptr(inp, (n, 3, self.Vh), self.cdtype), float(mass), n))
         return out
 
     def cg(self, b: torch.Tensor, mass: float, tol: float, x: Optional[torch.Tensor] = None, strict: bool = True):

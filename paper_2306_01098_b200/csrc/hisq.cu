@@ -334,6 +334,32 @@ extern "C" int hisq_dslash(hisq_ctx* h, void* out, const void* in, int parity, i
                               nullptr, nullptr, 2);
 }
 
+// out = (mass^2 - D_eo D_oe) in on even sites: the operator the solvers work on, as a call of its own (fused second
+// Dslash: m^2 in - D_eo t and Re<in, out> in one kernel; the scalar products land in hisq_get_info-independent state).
+extern "C" int hisq_apply_A(hisq_ctx* h, void* out, const void* in, double mass, int nrhs)
+{
+    if (!h || !out || !in || nrhs < 1 || nrhs > HISQ_MAX_NRHS || !std::isfinite(mass)) return HISQ_EINVAL;
+    if (((uintptr_t)out & 15) || ((uintptr_t)in & 15)) return HISQ_EINVAL;
+    if (!h->ws || nrhs > h->ws_nrhs) return HISQ_ENOWORKSPACE;
+    if (!h->have_links) return HISQ_ENOLINKS;
+    if (h->g.part) return HISQ_EINVAL;   // needs a halo exchange between the two hops: use the phase-wise calls
+    const size_t bytes = (size_t)nrhs * 6 * h->g.Vh * elem_size(h->prec);
+    if (overlap(out, in, bytes)) return HISQ_EINVAL;
+    const size_t fb = field_bytes(h, h->ws_nrhs, elem_size(h->prec));
+    void* t = h->fields + 3 * fb;
+    int rc;
+    if (h->prec == HISQ_FP32) {
+        rc = run_dslash<float>(h, h->links32, (float*)t, (const float*)in, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, nullptr, 2);
+        if (rc) return rc;
+        return run_dslash<float>(h, h->links32, (float*)out, (const float*)t, HISQ_EVEN, nrhs, MODE_APPLY_A, (const float*)in, nullptr,
+                                 mass * mass, h->state->sums, nullptr, 2);
+    }
+    rc = run_dslash<double>(h, h->links64, (double*)t, (const double*)in, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, nullptr, 2);
+    if (rc) return rc;
+    return run_dslash<double>(h, h->links64, (double*)out, (const double*)t, HISQ_EVEN, nrhs, MODE_APPLY_A, (const double*)in, nullptr,
+                              mass * mass, h->state->sums, nullptr, 2);
+}
+
 // ---- CG --------------------------------------------------------------------------------------------
 // One iteration (textbook Hestenes-Stiefel, independent scalars per RHS):
 //   p = r + beta p ; t = D_oe p ; q = m^2 p - D_eo t , <p,q> ; x += alpha p , r -= alpha q , rho' = ||r||^2

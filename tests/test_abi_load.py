@@ -23,7 +23,7 @@ def lib():
 def test_header_symbols_are_exported(lib):
     text = open(os.path.join(ROOT, "include", "hisq.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    declared = set(re.findall(r"\b(hisq_[a-z_0-9]+)\s*\(", text))
+    declared = set(re.findall(r"\b(hisq_[A-Za-z_0-9]+)\s*\(", text))
     assert declared == set(binding.EXPORTS), declared ^ set(binding.EXPORTS)
     for name in declared:
         assert hasattr(lib, name), name

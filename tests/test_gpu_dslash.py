@@ -145,3 +145,15 @@ def test_dslash_rejects_too_many_rhs():
         ctx.dslash(f, 0)
     assert e.value.code == -1
     ctx.close()
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32", "mixed"])
+def test_apply_A_matches_oracle(prec):
+    L, n, m = (4, 6, 8, 10), 3, 0.37
+    ctx, X, W = make_ctx(L, prec, n, 21)
+    dev_in, full_in = make_field(ctx, L, 22, n, 0)
+    got = to_full(ctx, L, ctx.apply_A(dev_in, m), 0)
+    ref = oracle.apply_A(L, X, W, m, full_in)
+    for k in range(n):
+        assert rel_l2(got[k], ref[k]) <= (1e-6 if prec == "fp32" else 1e-14)
+    ctx.close()
