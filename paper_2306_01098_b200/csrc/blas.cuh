@@ -37,7 +37,7 @@ inline int blas_grid_x(size_t nreal, int vec_n) {
 
 // ---- start of a solve: r = b (rounded to T), rho = ||b||^2 in fp64, state reset ---------------------
 template <typename TB, typename T>
-__global__ void __launch_bounds__(kBlasBlock) cg_init_kernel(const TB* __restrict__ b, T* __restrict__ r, size_t nreal,
+__global__ void __launch_bounds__(kBlasBlock) cg_init_kernel(const TB* b, T* r /* may alias b (phase-wise CG) */, size_t nreal,
                                                              CgState* st, double* partial, double tol, int max_iter)
 {
     const int k = blockIdx.y;
