@@ -33,6 +33,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 FLOP_PER_SITE = 1146
+# Context denominators measured on this pool's B200 with `python -m paper_2306_01098_b200.peaks`
+# (profiles/r1_peaks_microbench.txt); the roofline `peak` itself comes from MEASURED_PEAKS.json.
+READ_ONLY_GBS = 7420.0                       # 128-bit read-only stream over 8 GB
+FMA_PEAK_GFLOPS = {4: 69600.0, 8: 36900.0}   # plain FFMA / DFMA, all SMs
 CONFIGS = {
     "C1": dict(L=(8, 8, 8, 8), prec="fp64", nrhs=1, mass=0.1, tol=1e-10),
     "C2": dict(L=(32, 32, 32, 8), prec="fp64", nrhs=1, mass=0.01, tol=1e-10),
@@ -303,7 +307,9 @@ def main():
     achieved = alg_bytes / (d_ms * 1e-3) / 1e9
     dsl = {"ms": d_ms, "gflops": FLOP_PER_SITE * Vh * n / (d_ms * 1e-3) / 1e9, "alg_gbs": achieved,
            "paper_model_gbs": (288 + 102 * n) * w * Vh / (d_ms * 1e-3) / 1e9,
-           "frac_of_measured_copy": achieved / peak, "frac_of_8TBs": achieved / 8000.0, "tiles": ctx.tiles(n)}
+           "frac_of_measured_copy": achieved / peak, "frac_of_8TBs": achieved / 8000.0,
+           "frac_of_measured_read_only": achieved / READ_ONLY_GBS,
+           "frac_of_fma_peak": FLOP_PER_SITE * Vh * n / (d_ms * 1e-3) / 1e9 / FMA_PEAK_GFLOPS[w], "tiles": ctx.tiles(n)}
     # ---- row f2: the same Dslash and solve with compressed Naik links (13 instead of 18 reals per Naik link) ----
     comp = None
     if not args.no_compression:
@@ -446,6 +452,8 @@ def sweep_c3(dev, peak, reps):
         by = dslash_bytes(ctx.Vh, n, 4)
         rows.append({"nrhs": n, "ms": ms, "gflops": FLOP_PER_SITE * ctx.Vh * n / (ms * 1e-3) / 1e9,
                      "alg_gbs": by / (ms * 1e-3) / 1e9, "frac_of_measured_copy": by / (ms * 1e-3) / 1e9 / peak,
+                     "frac_of_8TBs": by / (ms * 1e-3) / 1e9 / 8000.0,
+                     "frac_of_fma_peak": FLOP_PER_SITE * ctx.Vh * n / (ms * 1e-3) / 1e9 / FMA_PEAK_GFLOPS[4],
                      "tiles": ctx.tiles(n)})
     ctx.close()
     return {"workload": "C3: 64x64x64x16 fp32 Dslash", "rows": rows}
