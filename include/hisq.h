@@ -119,7 +119,7 @@ int hisq_cg_multishift(hisq_ctx *h, void *x, const void *b, double mass, const d
  * "tile_y", "tile_z" (CTA sweep order blocking in y,z; 0 = auto),
  * "naik_compress" (see hisq_naik_compressed; default 0), "fused_blas" (1: cooperative fused x/r/p update kernel when the
  * fields are small enough to stay in registers across a grid barrier, default 1), "window_mb" (L2 budget of the CTA sweep
- * order, default 40). */
+ * order, default 20). */
 int hisq_set_option(hisq_ctx *h, const char *key, double value);
 
 /* After hisq_cg: iterations done, number of fp64 true-residual recomputations, and per RHS the true

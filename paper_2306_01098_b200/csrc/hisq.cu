@@ -123,7 +123,7 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     h->cgp_x = nullptr; h->cgp_nrhs = 0; h->cgp_tol = 0.0;
     { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev); }
     h->tile_y = 0; h->tile_z = 0;
-    h->window_mb = 40.0;
+    h->window_mb = 20.0;   // measured on C5 and C3: 10-20 MB windows are 2-3 % faster than 40, 10 % faster than none
     h->info_iters = 0; h->info_reliable = 0;
     for (int k = 0; k < kMaxNrhs; ++k) h->info_relres[k] = 0.0;
     h->host_state = nullptr;
