@@ -161,8 +161,20 @@ __device__ __forceinline__ bool grid_reduce(const double (&vals)[NR], int k0, do
     if (!s_last) return false;
     __threadfence();
     for (int k = 0; k < nrhs_total; ++k) {
-        double s = 0.0;
-        for (int i = threadIdx.x; i < ncols; i += BLOCK) s += __ldcg(partial + (size_t)k * ncols + i);
+        // 8 loads in flight per thread (the partials sit in L2: ~1 us each if serialised); fixed order: deterministic
+        double acc8[8] = { 0, 0, 0, 0, 0, 0, 0, 0 };
+        const double* row = partial + (size_t)k * ncols;
+        for (int i0 = threadIdx.x; i0 < ncols; i0 += BLOCK * 8) {
+            double v[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int i = i0 + j * BLOCK;
+                v[j] = i < ncols ? __ldcg(row + i) : 0.0;
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) acc8[j] += v[j];
+        }
+        double s = ((acc8[0] + acc8[1]) + (acc8[2] + acc8[3])) + ((acc8[4] + acc8[5]) + (acc8[6] + acc8[7]));
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
         __syncthreads();

@@ -142,6 +142,48 @@ template <typename T> __device__ __forceinline__ void mv_acc(const T (&U)[18], c
         }
 }
 
+#ifndef HISQ_F32X2
+#define HISQ_F32X2 1   // 1: fp32 complex multiply-adds as packed FFMA2 (fma.rn.f32x2, sm_100+): 2/3 of the FMA issue slots
+#endif
+#if HISQ_F32X2
+// (dx, dy) += (ax, ay) * s   as ONE packed instruction (the scalar rides as a broadcast operand)
+__device__ __forceinline__ void fma2(float& dx, float& dy, float ax, float ay, float s)
+{
+    unsigned long long d, a, b;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(dx), "f"(dy));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(a) : "f"(ax), "f"(ay));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b) : "f"(s), "f"(s));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(dx), "=f"(dy) : "l"(d));
+}
+// acc += U v:   (re, im) += ur * (vr, vi) + ui * (-vi, vr)
+__device__ __forceinline__ void mv_acc(const float (&U)[18], const float (&v)[6], float (&acc)[6])
+{
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        const float sx = -v[2 * b + 1], sy = v[2 * b];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            fma2(acc[2 * a], acc[2 * a + 1], v[2 * b], v[2 * b + 1], U[2 * (3 * a + b)]);
+            fma2(acc[2 * a], acc[2 * a + 1], sx, sy, U[2 * (3 * a + b) + 1]);
+        }
+    }
+}
+// acc -= U^dagger v:   (re, im) += (-ur) * (vr, vi) + ui * (-vi, vr)   with u = U_ba
+__device__ __forceinline__ void mvdag_sub(const float (&U)[18], const float (&v)[6], float (&acc)[6])
+{
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        const float sx = -v[2 * b + 1], sy = v[2 * b];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            fma2(acc[2 * a], acc[2 * a + 1], v[2 * b], v[2 * b + 1], -U[2 * (3 * b + a)]);
+            fma2(acc[2 * a], acc[2 * a + 1], sx, sy, U[2 * (3 * b + a) + 1]);
+        }
+    }
+}
+#endif
+
 // acc -= U^dagger v       ((U^+)_ab = conj(U_ba))
 template <typename T> __device__ __forceinline__ void mvdag_sub(const T (&U)[18], const T (&v)[6], T (&acc)[6])
 {
@@ -203,7 +245,7 @@ __device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, 
 // fully unrolled 8-RHS body is > 100 KB of SASS and `no_instruction` became its largest stall (profiles/);
 // fp32 gains from rolling, fp64 does not (measured).
 #ifndef HISQ_F32_ROLL_FROM
-#define HISQ_F32_ROLL_FROM 6
+#define HISQ_F32_ROLL_FROM 99
 #endif
 #ifndef HISQ_F64_ROLL_FROM
 #define HISQ_F64_ROLL_FROM 99
@@ -223,13 +265,19 @@ __device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, 
 #define HISQ_F32_MINB8 4
 #endif
 #ifndef HISQ_F32_MINB4
-#define HISQ_F32_MINB4 8
+#define HISQ_F32_MINB4 6
 #endif
 #ifndef HISQ_F32_MINB1
 #define HISQ_F32_MINB1 3
 #endif
 #ifndef HISQ_F64_MINB1
 #define HISQ_F64_MINB1 4
+#endif
+#ifndef HISQ_EARLY_MAX
+#define HISQ_EARLY_MAX 4   // kernels with NR <= this fetch the epilogue operands before the stencil
+#endif
+#ifndef HISQ_F32_MINB4_EPI
+#define HISQ_F32_MINB4_EPI 4   // register cap of the NR = 3, 4 fp32 kernels WITH an epilogue
 #endif
 #ifndef HISQ_F32_MINB2
 #define HISQ_F32_MINB2 8
@@ -246,19 +294,19 @@ __device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, 
 #ifndef HISQ_F64_MINB4
 #define HISQ_F64_MINB4 1
 #endif
-template <typename T, int NR> struct KernelShape {
+template <typename T, int NR, int MODE = 0> struct KernelShape {
     static constexpr bool f32 = sizeof(T) == 4;
     static constexpr bool rolled = NR >= (sizeof(T) == 4 ? HISQ_F32_ROLL_FROM : HISQ_F64_ROLL_FROM);
     static constexpr int roll_outer = HISQ_ROLL_OUTER;
     static constexpr int vb8 = f32 ? HISQ_F32_VB8 : HISQ_F64_VB8;
     static constexpr int vb = NR >= 6 ? (vb8 < NR ? vb8 : NR) : NR;
     static constexpr int minb = NR >= 6 ? (f32 ? HISQ_F32_MINB8 : HISQ_F64_MINB8)
-                              : NR >= 3 ? (f32 ? HISQ_F32_MINB4 : HISQ_F64_MINB4)
+                              : NR >= 3 ? (f32 ? (MODE == 0 ? HISQ_F32_MINB4 : HISQ_F32_MINB4_EPI) : HISQ_F64_MINB4)
                               : NR == 2 ? (f32 ? HISQ_F32_MINB2 : HISQ_F64_MINB2) : (f32 ? HISQ_F32_MINB1 : HISQ_F64_MINB1);
 };
 
 template <typename T, int NR, int MODE, int BLOCK, bool NC>
-__global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel(const DslashArgs<T> a)
+__global__ void __launch_bounds__(BLOCK, KernelShape<T, NR, MODE>::minb) dslash_kernel(const DslashArgs<T> a)
 {
     if (a.done != nullptr && *a.done != 0) return;
     const Geom& g = a.g;
@@ -278,7 +326,7 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
 
     int h = 0;
     const size_t rhs_stride = (size_t)3 * 2 * Vh;  // reals per RHS
-    constexpr bool EARLY = MODE != MODE_PLAIN && NR <= 2;
+    constexpr bool EARLY = MODE != MODE_PLAIN && NR <= HISQ_EARLY_MAX;
     T ue[EARLY ? NR : 1][6], ve[EARLY ? NR : 1][6];
     const T* in = a.in + (size_t)chunk * NR * rhs_stride;
     if (valid) {
@@ -390,10 +438,14 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
                 const T m2 = (T)a.m2;
                 if (MODE == MODE_APPLY_A) {
 #pragma unroll
+                    // the 6 products of one site are summed in T and widened once: fp32 -> fp64 conversions run at a
+                    // fraction of the FMA rate (12 per RHS and site cost ~25 % of the fp32 n = 4 kernel); sites add in fp64
+                    T part = T(0);
                     for (int i = 0; i < 6; ++i) {
                         o[i] = fma(m2, uu[i], -acc[k][i]);
-                        red[k] += (double)uu[i] * (double)o[i];
+                        part = fma(uu[i], o[i], part);
                     }
+                    red[k] += (double)part;
                 } else {
                     T vv[6];
                     if (EARLY) {
@@ -403,10 +455,12 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR>::minb) dslash_kernel
                         load_vec(a.v + (size_t)(chunk * NR + k) * rhs_stride, Vh, h, vv);
                     }
 #pragma unroll
+                    T part = T(0);
                     for (int i = 0; i < 6; ++i) {
                         o[i] = vv[i] - fma(m2, uu[i], -acc[k][i]);
-                        red[k] += (double)o[i] * (double)o[i];
+                        part = fma(o[i], o[i], part);
                     }
+                    red[k] += (double)part;
                 }
             }
 #pragma unroll
