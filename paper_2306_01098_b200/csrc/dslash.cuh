@@ -292,7 +292,7 @@ __device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, 
 #define HISQ_F64_MINB8 1
 #endif
 #ifndef HISQ_F64_MINB4
-#define HISQ_F64_MINB4 1
+#define HISQ_F64_MINB4 3
 #endif
 template <typename T, int NR, int MODE = 0> struct KernelShape {
     static constexpr bool f32 = sizeof(T) == 4;
