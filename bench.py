@@ -104,11 +104,16 @@ def aggregate(ms: float, flops: float, dist, device):
 
 
 def ncu_traffic(config: str, prec: str, nrhs: int):
-    """DRAM bytes per launch of the Dslash kernel from the committed ncu capture (profiles/traffic.json), or None."""
+    """DRAM bytes per launch of the Dslash kernel from the committed ncu captures (profiles/r1_traffic.csv), or None."""
     try:
-        return json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"{config}:{prec}:{nrhs}")
+        with open(os.path.join(ROOT, "profiles", "r1_traffic.csv")) as f:
+            for line in f:
+                k, _, v = line.strip().partition(",")
+                if k == f"{config}:{prec}:{nrhs}":
+                    return int(v)
     except Exception:
-        return None
+        pass
+    return None
 
 
 def dslash_bytes(Vh: int, nrhs: int, w: int) -> int:
