@@ -148,6 +148,15 @@ int hisq_cg_host(hisq_ctx *h, void *x_host, const void *b_host, double mass, dou
  * Lt_loc must be even and >= 4.  hisq_cg / hisq_cg_multishift are not available on partitioned contexts (they would
  * need a cross-rank reduction): HISQ_EINVAL. */
 int hisq_create_part(hisq_ctx **h, int Lx, int Ly, int Lz, int Lt_global, int prec, int rank, int nranks);
+/* hisq_dslash restricted to the OWNED time slices [t_first, t_first + t_count) (0 <= t_first, t_first + t_count <= the
+ * number of owned slices: Lt_loc on a partitioned context, Lt otherwise); all other slices of `out` are left untouched.
+ * The slices [3, Lt_loc - 3) read no halo slice (the stencil reaches 3 sites), so the caller can compute
+ * them while the halo exchange of `in` is in flight and the first and last 3 after hisq_halo_unpack: that is how
+ * communication hides behind computation.  Errors as hisq_dslash; HISQ_EINVAL for a bad range. */
+int hisq_dslash_slices(hisq_ctx *h, void *out, const void *in, int parity, int nrhs, int t_first, int t_count);
+/* The first `width` and the last `width` owned slices in ONE launch (all owned slices if 2*width >= their number):
+ * with width = 3, what is left to do once the halo has arrived. */
+int hisq_dslash_edges(hisq_ctx *h, void *out, const void *in, int parity, int nrhs, int width);
 /* Bytes of ONE halo buffer (4 slices, nrhs fields); 0 for a non-partitioned context. */
 size_t hisq_halo_bytes(const hisq_ctx *h, int nrhs);
 /* send_lo <- the 4 lowest interior slices (for the previous rank's upper halo), send_hi <- the 4 highest (for the next
@@ -166,6 +175,9 @@ int hisq_halo_unpack(hisq_ctx *h, void *field, const void *recv_lo, const void *
  *                   hisq_cgp_phase(h, 3, mass)   q = mass^2 p - D_eo t, LOCAL Re<p_k,q_k> -> pq      -> all-reduce pq
  *                   hisq_cgp_phase(h, 4, mass)   x += alpha p, r -= alpha q, LOCAL ||r_k||^2 -> sums -> all-reduce sums
  *                   hisq_cgp_phase(h, 5, mass)   beta_k, convergence flags, iteration count
+ *   overlapped form: phase 2 = 20 (owned slices [3, Lt_loc-3), needs no halo) + 21 (the first and last 3 slices, after
+ *                   the halo of p has arrived); phase 3 = 30 + 31 in the same way with the halo of t.  20/30 are empty
+ *                   and 21/31 do everything when Lt_loc <= 6.  pq after 30 + 31 is bit-identical to phase 3's.
  *   hisq_cgp_status: synchronises and reports iterations, done, breakdown, recursive relative residuals (HOST arrays).
  * x, b: NATIVE even fields on the extended lattice (halo slices of b are ignored, those of x are undefined).
  * Same arithmetic and stopping rule as hisq_cg (no final true-residual check).  Works on ordinary contexts too

@@ -25,7 +25,7 @@ EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
     "hisq_set_links", "hisq_dslash", "hisq_apply_A", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
     "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count",
-    "hisq_create_part", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
+    "hisq_create_part", "hisq_dslash_slices", "hisq_dslash_edges", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
     "hisq_cgp_begin", "hisq_cgp_phase", "hisq_cgp_ptr", "hisq_cgp_status", "hisq_strerror",
     "hisq_last_error",
 ]
@@ -57,6 +57,8 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_set_workspace.argtypes = [vp, vp, sz]
     lib.hisq_set_links.argtypes = [vp, vp, vp]
     lib.hisq_dslash.argtypes = [vp, vp, vp, i, i]
+    lib.hisq_dslash_slices.argtypes = [vp, vp, vp, i, i, i, i]
+    lib.hisq_dslash_edges.argtypes = [vp, vp, vp, i, i, i]
     lib.hisq_cg.argtypes = [vp, vp, vp, d, d, i]
     lib.hisq_apply_A.argtypes = [vp, vp, vp, d, i]
     lib.hisq_cg_multishift.argtypes = [vp, vp, vp, d, ctypes.POINTER(d), i, d]
@@ -197,6 +199,21 @@ class Hisq:
             out = self.new_field(n)
         self._check(self.lib.hisq_dslash(self._h, self._ptr(out, (n, 3, self.Vh), self.cdtype),
                                          self._ptr(inp, (n, 3, self.Vh), self.cdtype), int(parity), n))
+        return out
+
+    def dslash_slices(self, inp: torch.Tensor, parity: int, out: torch.Tensor, t_first: int, t_count: int) -> torch.Tensor:
+        """hisq_dslash_slices: only the owned time slices [t_first, t_first + t_count) of `out` are written."""
+        n = inp.shape[0]
+        self._check(self.lib.hisq_dslash_slices(self._h, self._ptr(out, (n, 3, self.Vh), self.cdtype),
+                                                self._ptr(inp, (n, 3, self.Vh), self.cdtype), int(parity), n,
+                                                int(t_first), int(t_count)))
+        return out
+
+    def dslash_edges(self, inp: torch.Tensor, parity: int, out: torch.Tensor, width: int) -> torch.Tensor:
+        """hisq_dslash_edges: the first and last `width` owned time slices of `out`, one launch."""
+        n = inp.shape[0]
+        self._check(self.lib.hisq_dslash_edges(self._h, self._ptr(out, (n, 3, self.Vh), self.cdtype),
+                                               self._ptr(inp, (n, 3, self.Vh), self.cdtype), int(parity), n, int(width)))
         return out
 
     def apply_A(self, inp: torch.Tensor, mass: float, out: Optional[torch.Tensor] = None) -> torch.Tensor:

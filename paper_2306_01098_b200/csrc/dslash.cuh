@@ -44,6 +44,9 @@ template <typename T> struct DslashArgs {
     int slab_blocks;     // CTAs per (tile, t) slab and chunk
     unsigned total_blocks; // CTAs of the whole launch group (epilogue ticket)
     int naik_c13;        // 1: Naik links are stored compressed (13 reals, row f2)
+    int t0, tn;          // this launch covers tn owned slices: blockIdx.y = j is slice g.t_lo + t0 + j, plus t_skip for
+    int t_skip_at, t_skip;  // j >= t_skip_at (two ranges in one launch: the first and last slices around an interior).
+                         // A launch GROUP (the launches that share one ticket) covers every owned slice exactly once
 };
 
 // block of (field f, owner parity p, direction mu)
@@ -313,7 +316,8 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR, MODE>::minb) dslash_
     const int Vh = g.Vh, H = g.H;
     const int chunk = blockIdx.x % a.nchunks;
     const int sc = blockIdx.x / a.nchunks;
-    const int t = blockIdx.y + g.t_lo;
+    const int trel = (int)blockIdx.y + a.t0 + ((int)blockIdx.y >= a.t_skip_at ? a.t_skip : 0);
+    const int t = trel + g.t_lo;
     const int tile = blockIdx.z;
     const int l = sc * BLOCK + threadIdx.x;
     const bool valid = l < H * g.ty * g.tz;
@@ -474,7 +478,7 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR, MODE>::minb) dslash_
     }
     if (MODE != MODE_PLAIN) {
         __shared__ double totals[kMaxNrhs];
-        const int col = sc + a.slab_blocks * ((int)blockIdx.y + g.t_cnt * tile);
+        const int col = sc + a.slab_blocks * (trel + g.t_cnt * tile);
         const int ncols = a.slab_blocks * g.t_cnt * g.nty * g.ntz;
         if (grid_reduce<NR, BLOCK>(red, kg0, a.partial, ncols, col, a.ticket, a.total_blocks, a.nrhs_total, totals)) {
             if (threadIdx.x < a.nrhs_total) a.result[threadIdx.x] = totals[threadIdx.x];

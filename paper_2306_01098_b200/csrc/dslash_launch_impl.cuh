@@ -56,7 +56,7 @@ int launch_dslash(DslashArgs<T> args, int mode, int nrhs, int inner_cap, cudaStr
         if (args.v) a.v = args.v + (size_t)k * rhs_stride;
         a.k0 = k;
         a.nchunks = plan_cnt[i];
-        dim3 grid((unsigned)(a.slab_blocks * a.nchunks), (unsigned)g.t_cnt, (unsigned)ntiles);
+        dim3 grid((unsigned)(a.slab_blocks * a.nchunks), (unsigned)a.tn, (unsigned)ntiles);
         cudaError_t e;
         switch (plan_nr[i]) {
         case 8: e = launch_mode<T, 8>(a, mode, grid, stream); break;

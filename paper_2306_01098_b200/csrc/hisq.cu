@@ -140,6 +140,7 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
 
 // Row f3: one rank's share of a lattice partitioned along t (the paper's sub-lattice + halo scheme, PAPER.md:187-191,
 // Eq. (6)/(7) :467-488).  The context lives on the EXTENDED local lattice Lx x Ly x Lz x (Lt/nranks + 2*kHaloT).
+static const int kHopMax = 3;  // reach of the stencil in one direction (Naik term)
 static const int kHaloT = 4;   // halo slices on each side: 3 are needed (Naik reach), 4 keeps site parity = global parity
 extern "C" int hisq_create_part(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt_global, int prec, int rank, int nranks)
 {
@@ -292,7 +293,8 @@ static int default_inner_cap(int) { return 8; }  // measured: 8 RHS per thread b
 
 template <typename T>
 static int run_dslash(hisq_ctx* h, const T* links, T* out, const T* in, int parity, int nrhs, int mode, const T* u,
-                      const T* v, double m2, double* result, const int* done, int ticket_slot)
+                      const T* v, double m2, double* result, const int* done, int ticket_slot, int t_first = 0,
+                      int t_count = -1, int t_skip_at = 1 << 30, int t_skip = 0)
 {
     choose_tiles(h, nrhs, sizeof(T));
     DslashArgs<T> a;
@@ -307,6 +309,9 @@ static int run_dslash(hisq_ctx* h, const T* links, T* out, const T* in, int pari
     a.par = parity;
     a.k0 = 0; a.nrhs_total = nrhs; a.nchunks = 1; a.slab_blocks = 0; a.total_blocks = 0;
     a.naik_c13 = h->naik_c13 ? 1 : 0;
+    a.t0 = t_first; a.tn = t_count < 0 ? h->g.t_cnt - t_first : t_count;
+    a.t_skip_at = t_skip_at; a.t_skip = t_skip;
+    if (a.tn <= 0) return HISQ_OK;
     int cap = h->nrhs_inner > 0 ? h->nrhs_inner : default_inner_cap((int)sizeof(T));
     int e = launch_dslash<T>(a, mode, nrhs, cap, h->stream, &h->stats);
     if (e != 0) return cuda_fail(h, (cudaError_t)e, "dslash launch");
@@ -332,6 +337,36 @@ extern "C" int hisq_dslash(hisq_ctx* h, void* out, const void* in, int parity, i
                                  nullptr, nullptr, 2);
     return run_dslash<double>(h, h->links64, (double*)out, (const double*)in, parity, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0,
                               nullptr, nullptr, 2);
+}
+
+// hisq_dslash on some of the owned time slices only (the other slices of `out` are left untouched): `count` slices
+// starting at `first`; with skip > 0 the slices from the skip_at-th on lie `skip` further up (two ranges, one launch).
+static int dslash_some_slices(hisq_ctx* h, void* out, const void* in, int parity, int nrhs, int first, int count, int skip_at, int skip)
+{
+    if (!h || !out || !in || nrhs < 1 || nrhs > HISQ_MAX_NRHS || (parity != 0 && parity != 1)) return HISQ_EINVAL;
+    if (first < 0 || count < 0 || skip < 0 || first + count + skip > h->g.t_cnt) return HISQ_EINVAL;
+    if (((uintptr_t)out & 15) || ((uintptr_t)in & 15)) return HISQ_EINVAL;
+    if (!h->ws) return HISQ_ENOWORKSPACE;
+    if (!h->have_links) return HISQ_ENOLINKS;
+    const size_t bytes = (size_t)nrhs * 6 * h->g.Vh * elem_size(h->prec);
+    if (overlap(out, in, bytes)) return HISQ_EINVAL;
+    if (count == 0) return HISQ_OK;
+    if (h->prec == HISQ_FP32)
+        return run_dslash<float>(h, h->links32, (float*)out, (const float*)in, parity, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0,
+                                 nullptr, nullptr, 2, first, count, skip_at, skip);
+    return run_dslash<double>(h, h->links64, (double*)out, (const double*)in, parity, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0,
+                              nullptr, nullptr, 2, first, count, skip_at, skip);
+}
+extern "C" int hisq_dslash_slices(hisq_ctx* h, void* out, const void* in, int parity, int nrhs, int t_first, int t_count)
+{
+    return dslash_some_slices(h, out, in, parity, nrhs, t_first, t_count, 1 << 30, 0);
+}
+extern "C" int hisq_dslash_edges(hisq_ctx* h, void* out, const void* in, int parity, int nrhs, int width)
+{
+    if (!h || width < 0) return HISQ_EINVAL;
+    const int n = h->g.t_cnt;
+    if (2 * width >= n) return dslash_some_slices(h, out, in, parity, nrhs, 0, n, 1 << 30, 0);
+    return dslash_some_slices(h, out, in, parity, nrhs, 0, 2 * width, width, n - 2 * width);
 }
 
 // out = (mass^2 - D_eo D_oe) in on even sites: the operator the solvers work on, as a call of its own (fused second
@@ -900,6 +935,27 @@ static int cgp_phase(hisq_ctx* h, const T* links, int phase, double mass)
     case 1: return enqueue_p_update<T>(h, p, r, nrhs);
     case 2: return run_dslash<T>(h, links, t, p, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, &h->state->done, 2);
     case 3: return run_dslash<T>(h, links, q, t, HISQ_EVEN, nrhs, MODE_APPLY_A, p, nullptr, mass * mass, h->state->pq, &h->state->done, 2);
+    // Phases 2 and 3 split so that the halo exchange overlaps the slices that do not read the halo: 20 / 30 compute the
+    // owned slices [3, n-3) (no t-hop leaves the owned range), 21 / 31 the first and last 3.  The launches of 30 + 31 share
+    // one ticket and one table of partial sums, so pq is the same sum, in the same order, as phase 3 gives.
+    case 20: case 21: case 30: case 31: {
+        const int n = h->g.t_cnt, w = kHopMax;
+        const bool second = phase >= 30, boundary = (phase % 10) == 1;
+        // interior: [w, n-w); boundary: [0, w) and [n-w, n) in ONE launch (blockIdx.y >= w skips the interior)
+        int first = 0, count = 0, skip_at = 1 << 30, skip = 0;
+        if (n > 2 * w) {
+            if (!boundary) { first = w; count = n - 2 * w; }
+            else { count = 2 * w; skip_at = w; skip = n - 2 * w; }
+        } else if (boundary) count = n;
+        if (count > 0) {
+            int rc = second ? run_dslash<T>(h, links, q, t, HISQ_EVEN, nrhs, MODE_APPLY_A, p, nullptr, mass * mass, h->state->pq,
+                                            &h->state->done, 2, first, count, skip_at, skip)
+                            : run_dslash<T>(h, links, t, p, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr,
+                                            &h->state->done, 2, first, count, skip_at, skip);
+            if (rc) return rc;
+        }
+        return HISQ_OK;
+    }
     case 4:
         cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial, 1);
         h->stats.launches++;

@@ -12,6 +12,7 @@ import torch
 from . import inputs, layout
 
 HALO_T = 4
+HOP_MAX = 3   # reach of the stencil along one direction (Naik term)
 
 
 def extended_lattice(L: Sequence[int], nranks: int):
@@ -59,22 +60,40 @@ def make_sources_part(L, seed: int, nrhs: int, parity: int, rank: int, nranks: i
     return src.contiguous().to(device)
 
 
-def exchange_halos(send_lo: torch.Tensor, send_hi: torch.Tensor, recv_lo: torch.Tensor, recv_hi: torch.Tensor,
-                   rank: int, nranks: int, dist=None):
+class HaloExchange:
+    """A halo exchange in flight (begin_exchange): finish() makes the received halos visible to the current stream."""
+
+    def __init__(self, works=(), staged=None):
+        self.works, self.staged = list(works), staged
+
+    def finish(self):
+        for w in self.works:
+            w.wait()
+        if self.staged is not None:
+            for dst, src in self.staged:
+                dst.copy_(src)
+        self.works, self.staged = [], None
+
+
+def begin_exchange(send_lo: torch.Tensor, send_hi: torch.Tensor, recv_lo: torch.Tensor, recv_hi: torch.Tensor,
+                   rank: int, nranks: int, dist=None) -> HaloExchange:
     """Periodic ring in t: my send_hi goes to rank+1's recv_lo, my send_lo to rank-1's recv_hi.
-    dist = torch.distributed (initialised) or None for a single rank (own halos: periodic wrap onto itself)."""
+    dist = torch.distributed (initialised) or None for a single rank (own halos: periodic wrap onto itself).
+    With NCCL the transfers are enqueued behind what the current stream holds so far (the pack kernel) and run on
+    NCCL's own stream: kernels launched between begin_exchange and finish() overlap them.  Other backends (gloo: CPU
+    tests, or two processes sharing one GPU) go through the host and complete inside this call."""
     if nranks == 1 or dist is None:
         recv_lo.copy_(send_hi)
         recv_hi.copy_(send_lo)
-        return
+        return HaloExchange()
     up, down = (rank + 1) % nranks, (rank - 1) % nranks
-    # NCCL moves device buffers directly (NVLink); gloo (CPU tests, or two processes sharing one GPU) goes through the host
     stage = send_lo.is_cuda and dist.get_backend() != "nccl"
     # communicate as real arrays (not every backend knows complex dtypes)
     real = lambda t: torch.view_as_real(t) if t.is_complex() else t
     s_lo, s_hi = (real(send_lo.cpu()), real(send_hi.cpu())) if stage else (real(send_lo), real(send_hi))
     r_lo, r_hi = (torch.empty_like(s_lo), torch.empty_like(s_hi)) if stage else (real(recv_lo), real(recv_hi))
-    if nranks == 2:
+    staged = [(real(recv_lo), r_lo), (real(recv_hi), r_hi)] if stage else None
+    if nranks == 2 and dist.get_backend() != "nccl":
         # both neighbours are the same peer: two tagged exchanges, lower rank sends first (no reliance on message order)
         for tag, (snd, rcv) in enumerate(((s_hi, r_lo), (s_lo, r_hi))):
             if rank == 0:
@@ -83,25 +102,40 @@ def exchange_halos(send_lo: torch.Tensor, send_hi: torch.Tensor, recv_lo: torch.
             else:
                 dist.recv(rcv, up, tag=tag)
                 dist.send(snd, up, tag=tag)
-    else:
-        ops = [dist.P2POp(dist.isend, s_hi, up), dist.P2POp(dist.irecv, r_lo, down),
-               dist.P2POp(dist.isend, s_lo, down), dist.P2POp(dist.irecv, r_hi, up)]
-        for w in dist.batch_isend_irecv(ops):
-            w.wait()
-    if stage:
-        real(recv_lo).copy_(r_lo)
-        real(recv_hi).copy_(r_hi)
+        return HaloExchange(staged=staged)
+    # one grouped call: NCCL matches sends and receives between a pair of ranks in issue order, the same on both sides
+    # (hi -> lo first, then lo -> hi), which also covers nranks == 2 where up == down
+    ops = [dist.P2POp(dist.isend, s_hi, up), dist.P2POp(dist.irecv, r_lo, down),
+           dist.P2POp(dist.isend, s_lo, down), dist.P2POp(dist.irecv, r_hi, up)]
+    return HaloExchange(dist.batch_isend_irecv(ops), staged)
 
 
-def dslash_partitioned(ctx, field_in: torch.Tensor, parity: int, rank: int, nranks: int, dist=None, out=None):
-    """Halo exchange of `field_in` followed by the local Dslash (what one rank does per application)."""
+def exchange_halos(send_lo, send_hi, recv_lo, recv_hi, rank: int, nranks: int, dist=None):
+    begin_exchange(send_lo, send_hi, recv_lo, recv_hi, rank, nranks, dist).finish()
+
+
+def dslash_partitioned(ctx, field_in: torch.Tensor, parity: int, rank: int, nranks: int, dist=None, out=None,
+                       overlap: bool = True):
+    """What one rank does per Dslash application: pack the halo of `field_in`, exchange it, compute.  overlap: the owned
+    slices that read no halo are computed while the exchange is in flight, the first and last 3 afterwards
+    (hisq_dslash_slices; PAPER.md:340-348 'communication hidden behind computation')."""
     n = field_in.shape[0]
     slo, shi = ctx.halo_buffers(n)
     rlo, rhi = ctx.halo_buffers(n)
     ctx.halo_pack(field_in, slo, shi)
-    exchange_halos(slo, shi, rlo, rhi, rank, nranks, dist)
+    ex = begin_exchange(slo, shi, rlo, rhi, rank, nranks, dist)
+    nt = ctx.L[3] - 2 * HALO_T
+    if not overlap or nt <= 2 * HOP_MAX:
+        ex.finish()
+        ctx.halo_unpack(field_in, rlo, rhi)
+        return ctx.dslash(field_in, parity, out=out)
+    if out is None:
+        out = ctx.new_field(n)
+    ctx.dslash_slices(field_in, parity, out, HOP_MAX, nt - 2 * HOP_MAX)
+    ex.finish()
     ctx.halo_unpack(field_in, rlo, rhi)
-    return ctx.dslash(field_in, parity, out=out)
+    ctx.dslash_edges(field_in, parity, out, HOP_MAX)
+    return out
 
 
 class PartitionedCG:
@@ -112,12 +146,16 @@ class PartitionedCG:
     def __init__(self, ctx, rank: int, nranks: int, dist=None):
         self.ctx, self.rank, self.nranks, self.dist = ctx, rank, nranks, dist
 
-    def _halo(self, field):
+    def _halo_begin(self, field):
         n = field.shape[0]
         slo, shi = self.ctx.halo_buffers(n)
         rlo, rhi = self.ctx.halo_buffers(n)
         self.ctx.halo_pack(field, slo, shi)
-        exchange_halos(slo, shi, rlo, rhi, self.rank, self.nranks, self.dist)
+        return begin_exchange(slo, shi, rlo, rhi, self.rank, self.nranks, self.dist), rlo, rhi
+
+    def _halo_end(self, field, pending):
+        ex, rlo, rhi = pending
+        ex.finish()
         self.ctx.halo_unpack(field, rlo, rhi)
 
     def _allreduce(self, t):
@@ -129,7 +167,10 @@ class PartitionedCG:
             else:
                 self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
 
-    def solve(self, b, mass: float, tol: float, x=None, check_every: int = 16, max_iter: int = 100000):
+    def solve(self, b, mass: float, tol: float, x=None, check_every: int = 16, max_iter: int = 100000,
+              overlap: bool = True):
+        """overlap: each Dslash is split (phases 20/21, 30/31) so that the slices reading no halo run while the halo
+        exchange is in flight; the iterates are bit-identical to the unsplit phases 2, 3."""
         c = self.ctx
         n = b.shape[0]
         if x is None:
@@ -143,10 +184,22 @@ class PartitionedCG:
         while not st["done"] and st["iterations"] < max_iter:
             for _ in range(check_every):
                 c.cgp_phase(1, mass)
-                self._halo(p)
-                c.cgp_phase(2, mass)
-                self._halo(t)
-                c.cgp_phase(3, mass)
+                pend = self._halo_begin(p)
+                if overlap:
+                    c.cgp_phase(20, mass)
+                    self._halo_end(p, pend)
+                    c.cgp_phase(21, mass)
+                else:
+                    self._halo_end(p, pend)
+                    c.cgp_phase(2, mass)
+                pend = self._halo_begin(t)
+                if overlap:
+                    c.cgp_phase(30, mass)
+                    self._halo_end(t, pend)
+                    c.cgp_phase(31, mass)
+                else:
+                    self._halo_end(t, pend)
+                    c.cgp_phase(3, mass)
                 self._allreduce(pq)
                 c.cgp_phase(4, mass)
                 self._allreduce(sums)

@@ -14,7 +14,7 @@ from tests.helpers import oracle_field, oracle_links
 pytestmark = pytest.mark.gpu
 
 
-def _run(L, prec, nranks, nrhs, parity, seed):
+def _run(L, prec, nranks, nrhs, parity, seed, overlap=False):
     dev = torch.device("cuda:0")
     ctxs, fields, bufs = [], [], []
     for r in range(nranks):
@@ -27,13 +27,24 @@ def _run(L, prec, nranks, nrhs, parity, seed):
         ctx.halo_pack(f, slo, shi)
         ctxs.append(ctx); fields.append(f); bufs.append((slo, shi))
     outs = []
+    nt, w = L[3] // nranks, partition.HOP_MAX
     for r, ctx in enumerate(ctxs):
         rlo = bufs[(r - 1) % nranks][1]      # previous rank's highest interior slices
         rhi = bufs[(r + 1) % nranks][0]      # next rank's lowest interior slices
-        ctx.halo_unpack(fields[r], rlo, rhi)
         out = ctx.new_field(nrhs)
         out.zero_()
-        ctx.dslash(fields[r], parity, out=out)
+        if overlap and nt > 2 * w:
+            # the slices that read no halo BEFORE the halo arrives (it holds NaN until then), the rest after
+            S = ctx.Vh // ctx.L[3]
+            v = fields[r].view(nrhs, 3, ctx.L[3], S)
+            v[:, :, :partition.HALO_T] = float("nan")
+            v[:, :, ctx.L[3] - partition.HALO_T:] = float("nan")
+            ctx.dslash_slices(fields[r], parity, out, w, nt - 2 * w)
+            ctx.halo_unpack(fields[r], rlo, rhi)
+            ctx.dslash_edges(fields[r], parity, out, w)
+        else:
+            ctx.halo_unpack(fields[r], rlo, rhi)
+            ctx.dslash(fields[r], parity, out=out)
         outs.append(ctx.unpack(out).cpu().numpy().astype(np.complex128))
     # gather the interiors into a global full-lattice field
     V = layout.volume(L)
@@ -79,6 +90,42 @@ def test_partitioned_dslash_equals_single_lattice_and_oracle(nranks, prec):
         one = oracle.half_to_full(L, ctx.unpack(ctx.dslash(s1, parity)).cpu().numpy().astype(np.complex128), parity)
         ctx.close()
         assert np.array_equal(full, one)
+        # interior / boundary split around the exchange (hisq_dslash_slices): the same bits
+        full_o, seen_o = _run(L, prec, nranks, nrhs, parity, seed, overlap=True)
+        assert np.array_equal(seen_o, seen) and np.array_equal(full_o, full)
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_dslash_slices_compose_to_the_full_dslash(prec):
+    L, nrhs, seed = (6, 4, 4, 10), 3, 8
+    ctx = binding.Hisq(L, prec, nrhs)
+    fat, naik = binding.make_links(L, seed, ctx.device, ctx.cdtype)
+    ctx.set_links(fat, naik)
+    S = ctx.Vh // L[3]
+    for parity in (0, 1):
+        src = ctx.pack(binding.make_sources(L, seed + 1, nrhs, 1 - parity, ctx.device, ctx.cdtype))
+        ref = ctx.dslash(src, parity)
+        out = ctx.new_field(nrhs)
+        out.fill_(7.0)
+        ctx.dslash_slices(src, parity, out, 2, 5)
+        v, vr = out.view(nrhs, 3, L[3], S), ref.view(nrhs, 3, L[3], S)
+        assert torch.equal(v[:, :, 2:7], vr[:, :, 2:7])
+        assert torch.all(v[:, :, :2] == 7.0) and torch.all(v[:, :, 7:] == 7.0)     # the other slices are untouched
+        ctx.dslash_slices(src, parity, out, 0, 2)
+        ctx.dslash_slices(src, parity, out, 7, 3)
+        ctx.dslash_slices(src, parity, out, 4, 0)                                 # empty range: nothing happens
+        assert torch.equal(out, ref)
+        out.fill_(7.0)
+        ctx.dslash_edges(src, parity, out, 3)                                     # slices 0-2 and 7-9
+        assert torch.equal(v[:, :, :3], vr[:, :, :3]) and torch.equal(v[:, :, 7:], vr[:, :, 7:])
+        assert torch.all(v[:, :, 3:7] == 7.0)
+        ctx.dslash_edges(src, parity, out, 5)                                     # 2 * width >= Lt: everything
+        assert torch.equal(out, ref)
+    for bad in ((-1, 2), (0, 11), (9, 2), (3, -1)):
+        with pytest.raises(binding.HisqError) as e:
+            ctx.dslash_slices(src, 0, out, *bad)
+        assert e.value.code == -1
+    ctx.close()
 
 
 def test_partitioned_context_rejects_solvers_and_bad_splits():
@@ -96,7 +143,7 @@ def test_partitioned_context_rejects_solvers_and_bad_splits():
         binding.Hisq((4, 4, 4, 8), "fp64", 1, part=(0, 4))       # Lt_loc = 2 < 4
 
 
-def _emulated_cg(L, prec, nranks, nrhs, m, tol, seed):
+def _emulated_cg(L, prec, nranks, nrhs, m, tol, seed, overlap=False):
     """All ranks in lockstep on one GPU: every phase is run for rank 0..G-1 in turn, the cross-rank steps (ring halo
     exchange, all-reduce) are done by hand between the phases -- the same sequence as partition.PartitionedCG.solve."""
     dev = torch.device("cuda:0")
@@ -116,13 +163,15 @@ def _emulated_cg(L, prec, nranks, nrhs, m, tol, seed):
         for t in ts:
             t.copy_(tot)
 
-    def halo(which):
+    def halo(which, between=None):
         fields = [c.cgp_tensor(which, nrhs) for c in ctxs]
         bufs = []
         for c, f in zip(ctxs, fields):
             slo, shi = c.halo_buffers(nrhs)
             c.halo_pack(f, slo, shi)
             bufs.append((slo, shi))
+        if between is not None:      # what a rank computes while its halo is in flight
+            for c in ctxs: c.cgp_phase(between, m)
         for r, (c, f) in enumerate(zip(ctxs, fields)):
             c.halo_unpack(f, bufs[(r - 1) % nranks][1], bufs[(r + 1) % nranks][0])
 
@@ -133,10 +182,16 @@ def _emulated_cg(L, prec, nranks, nrhs, m, tol, seed):
     while not st["done"] and st["iterations"] < 5000:
         for _ in range(16):
             for c in ctxs: c.cgp_phase(1, m)
-            halo(0)
-            for c in ctxs: c.cgp_phase(2, m)
-            halo(1)
-            for c in ctxs: c.cgp_phase(3, m)
+            if overlap:
+                halo(0, between=20)
+                for c in ctxs: c.cgp_phase(21, m)
+                halo(1, between=30)
+                for c in ctxs: c.cgp_phase(31, m)
+            else:
+                halo(0)
+                for c in ctxs: c.cgp_phase(2, m)
+                halo(1)
+                for c in ctxs: c.cgp_phase(3, m)
             allreduce(3)
             for c in ctxs: c.cgp_phase(4, m)
             allreduce(4)
@@ -171,6 +226,9 @@ def test_partitioned_cg_matches_oracle_and_single_lattice(nranks):
     xo, it_o, _, ok, _ = oracle.cg(L, X, W, m, tol, b)
     assert ok == 0 and rel_l2(x, xo) <= 10 * tol
     assert abs(st["iterations"] - int(it_o.max())) <= 16 + 3      # status is polled every 16 iterations
+    # Dslashes split around the halo exchange (phases 20/21, 30/31): same sums in the same order -> the same iterates
+    x2, st2 = _emulated_cg(L, "fp64", nranks, nrhs, m, tol, seed, overlap=True)
+    assert st2["iterations"] == st["iterations"] and np.array_equal(x2, x)
 
 
 def test_partitioned_cg_driver_single_rank_equals_hisq_cg():
