@@ -157,13 +157,36 @@ int hisq_dslash_slices(hisq_ctx *h, void *out, const void *in, int parity, int n
 /* The first `width` and the last `width` owned slices in ONE launch (all owned slices if 2*width >= their number):
  * with width = 3, what is left to do once the halo has arrived. */
 int hisq_dslash_edges(hisq_ctx *h, void *out, const void *in, int parity, int nrhs, int width);
-/* Bytes of ONE halo buffer (4 slices, nrhs fields); 0 for a non-partitioned context. */
+/* Bytes of ONE halo buffer (3 slices, nrhs fields: of the 4 halo slices on a side only the 3 nearest are ever read);
+ * 0 for a non-partitioned context. */
 size_t hisq_halo_bytes(const hisq_ctx *h, int nrhs);
-/* send_lo <- the 4 lowest interior slices (for the previous rank's upper halo), send_hi <- the 4 highest (for the next
- * rank's lower halo); buffers are device memory of hisq_halo_bytes each, layout [k][c][4*S] complex.  Asynchronous. */
+/* send_lo <- the 3 lowest interior slices (for the previous rank's upper halo), send_hi <- the 3 highest (for the next
+ * rank's lower halo); buffers are device memory of hisq_halo_bytes each, layout [k][c][3*S] complex.  Asynchronous. */
 int hisq_halo_pack(hisq_ctx *h, void *send_lo, void *send_hi, const void *field, int nrhs);
 /* lower halo <- recv_lo (what the previous rank packed as send_hi), upper halo <- recv_hi (the next rank's send_lo). */
 int hisq_halo_unpack(hisq_ctx *h, void *field, const void *recv_lo, const void *recv_hi, int nrhs);
+
+/* Halo transport through peer-mapped memory, without a communication library (the exchange of PAPER.md:340-348 done
+ * by the packing kernel's own stores over NVLink).  Every rank owns a MAILBOX of hisq_peer_bytes(h, nrhs) bytes of
+ * device memory (256-byte aligned, ZEROED by the caller before any neighbour attaches) that its t-neighbours can
+ * address: cudaDeviceEnablePeerAccess within a process, a CUDA IPC mapping between processes -- obtaining those
+ * pointers is the caller's plumbing.  hisq_peer_attach(h, mine, up, down, nrhs): mailboxes of this rank, of rank+1
+ * and of rank-1 (periodic; all three the same pointer for a single rank, up == down for two ranks); nrhs = the
+ * capacity the mailboxes were sized for.  Then, per exchange and in this order on every rank:
+ *   hisq_halo_send(h, field, nrhs)   packs the 3 lowest / highest owned slices of `field` straight into the
+ *                                     neighbours' mailboxes and raises their "ready" flags;
+ *   hisq_halo_recv(h, field, nrhs)   waits for this rank's "ready" flags, unpacks its mailbox into the halo slices of
+ *                                     `field`, and raises the neighbours' "free" flags.
+ * Both are asynchronous on the context's stream; waiting and signalling are stream memory operations
+ * (cuStreamWaitValue32 / cuStreamWriteValue32), so no kernel spins and work enqueued between send and recv (the
+ * interior slices, hisq_dslash_slices) overlaps the transfer.  Mailboxes are double-buffered: send number e waits
+ * until both neighbours have unpacked exchange e-2.  Every rank must issue the same sequence of send / recv calls;
+ * a recv without a matching earlier send on the same rank is refused (HISQ_EINVAL).  HISQ_ECUDA if the driver lacks
+ * stream memory operations. */
+size_t hisq_peer_bytes(const hisq_ctx *h, int nrhs);
+int hisq_peer_attach(hisq_ctx *h, void *mine, void *up, void *down, int nrhs);
+int hisq_halo_send(hisq_ctx *h, const void *field, int nrhs);
+int hisq_halo_recv(hisq_ctx *h, void *field, int nrhs);
 
 /* CG on a t-partitioned lattice, phase by phase.  The solver's reductions span all ranks, so the iteration is cut where
  * a cross-rank step is due and the CALLER performs it between the calls (halo exchange of a field through

@@ -25,7 +25,7 @@ EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
     "hisq_set_links", "hisq_dslash", "hisq_apply_A", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
     "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count",
-    "hisq_create_part", "hisq_dslash_slices", "hisq_dslash_edges", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
+    "hisq_create_part", "hisq_peer_bytes", "hisq_peer_attach", "hisq_halo_send", "hisq_halo_recv", "hisq_dslash_slices", "hisq_dslash_edges", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
     "hisq_cgp_begin", "hisq_cgp_phase", "hisq_cgp_ptr", "hisq_cgp_status", "hisq_strerror",
     "hisq_last_error",
 ]
@@ -72,6 +72,11 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_create_part.argtypes = [ctypes.POINTER(vp), i, i, i, i, i, i, i]
     lib.hisq_halo_bytes.argtypes = [vp, i]
     lib.hisq_halo_bytes.restype = sz
+    lib.hisq_peer_bytes.argtypes = [vp, i]
+    lib.hisq_peer_bytes.restype = sz
+    lib.hisq_peer_attach.argtypes = [vp, vp, vp, vp, i]
+    lib.hisq_halo_send.argtypes = [vp, vp, i]
+    lib.hisq_halo_recv.argtypes = [vp, vp, i]
     lib.hisq_halo_pack.argtypes = [vp, vp, vp, vp, i]
     lib.hisq_halo_unpack.argtypes = [vp, vp, vp, vp, i]
     lib.hisq_cgp_begin.argtypes = [vp, vp, vp, d, i]
@@ -279,7 +284,7 @@ class Hisq:
         if nb == 0:
             raise HisqError(-1, "not a partitioned context")
         S = self.Vh // self.L[3]
-        mk = lambda: torch.empty((nrhs, 3, 4 * S), dtype=self.cdtype, device=self.device)
+        mk = lambda: torch.empty((nrhs, 3, 3 * S), dtype=self.cdtype, device=self.device)
         return mk(), mk()
 
     def halo_pack(self, field: torch.Tensor, lo: torch.Tensor, hi: torch.Tensor):
@@ -287,6 +292,24 @@ class Hisq:
 
     def halo_unpack(self, field: torch.Tensor, lo: torch.Tensor, hi: torch.Tensor):
         self._check(self.lib.hisq_halo_unpack(self._h, self._ptr(field), self._ptr(lo), self._ptr(hi), field.shape[0]))
+
+    # -- halo transport through peer-mapped mailboxes ------------------------------------------------
+    def peer_mailbox(self, nrhs: int) -> torch.Tensor:
+        """A zeroed mailbox of hisq_peer_bytes (uint8 device tensor) for this rank; share it with the neighbours."""
+        nb = self.lib.hisq_peer_bytes(self._h, nrhs)
+        if nb == 0:
+            raise HisqError(-1, "not a partitioned context")
+        return torch.zeros(nb, dtype=torch.uint8, device=self.device)
+
+    def peer_attach(self, mine: torch.Tensor, up: torch.Tensor, down: torch.Tensor, nrhs: int):
+        self._mailboxes = (mine, up, down)     # keep the mappings alive as long as the context uses them
+        self._check(self.lib.hisq_peer_attach(self._h, mine.data_ptr(), up.data_ptr(), down.data_ptr(), int(nrhs)))
+
+    def halo_send(self, field: torch.Tensor):
+        self._check(self.lib.hisq_halo_send(self._h, self._ptr(field), field.shape[0]))
+
+    def halo_recv(self, field: torch.Tensor):
+        self._check(self.lib.hisq_halo_recv(self._h, self._ptr(field), field.shape[0]))
 
     # -- phase-wise CG (partitioned lattices) ------------------------------------------------------
     def cgp_begin(self, x: torch.Tensor, b: torch.Tensor, tol: float):

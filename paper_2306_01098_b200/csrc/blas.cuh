@@ -415,6 +415,7 @@ __global__ void __launch_bounds__(256) spinor_layout_kernel(T* __restrict__ dst,
 }
 
 // ---- t-halo pack / unpack (row f3): native field [k][c][slice][S] complex, S = sites of one parity per time slice.
+// H = 3 slices move (the reach of the stencil); the 4th halo slice on each side only keeps parities aligned, never read.
 // PACK:   lo <- interior slices [t_lo, t_lo+H)            (goes to the previous rank's UPPER halo)
 //         hi <- interior slices [t_lo+t_cnt-H, t_lo+t_cnt) (goes to the next rank's LOWER halo)
 // UNPACK: lower halo [t_lo-H, t_lo) <- lo (received from the previous rank), upper halo [t_lo+t_cnt, +H) <- hi.

@@ -2,6 +2,8 @@
 // multi-RHS CG drivers (fp32 / fp64 / mixed with fp64 reliable updates).  sm_100a only; no CPU path.
 #include "../../include/hisq.h"
 
+#include <cuda.h>   // types of the stream memory operations only: the entry points are looked up at run time, libcuda is not linked
+
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -35,6 +37,11 @@ struct hisq_ctx {
     int naik_compress;     // option: try to compress at the next hisq_set_links
     int fused_blas;        // option: cooperative fused x/r/p update for small fields
     void* cgp_x; int cgp_nrhs; double cgp_tol;   // phase-wise CG on partitioned lattices
+    // peer-memory halo transport (hisq_peer_attach): mailboxes of this rank and of its t-neighbours, exchange counters
+    char *mbox, *mbox_up, *mbox_down;
+    size_t mbox_buf;       // bytes of one halo buffer inside a mailbox
+    int mbox_nrhs;
+    unsigned seq_send, seq_recv;
     int num_sms;
     unsigned long long* bad_count;  // device counter used by the compression check
     // options
@@ -1015,7 +1022,7 @@ extern "C" int hisq_cgp_status(hisq_ctx* h, int* iterations, int* done, int* bre
 extern "C" size_t hisq_halo_bytes(const hisq_ctx* h, int nrhs)
 {
     if (!h || !h->g.part || nrhs < 1 || nrhs > HISQ_MAX_NRHS) return 0;
-    return (size_t)nrhs * 3 * kHaloT * (h->g.Vh / h->g.L[3]) * 2 * elem_size(h->prec);
+    return (size_t)nrhs * 3 * kHopMax * (h->g.Vh / h->g.L[3]) * 2 * elem_size(h->prec);   // only 3 of the 4 halo slices are ever read
 }
 
 template <bool PACK>
@@ -1023,13 +1030,13 @@ static int halo_move(hisq_ctx* h, void* field, void* lo, void* hi, int nrhs)
 {
     if (!h || !field || !lo || !hi || nrhs < 1 || nrhs > HISQ_MAX_NRHS || !h->g.part) return HISQ_EINVAL;
     const int S = h->g.Vh / h->g.L[3];
-    const size_t total = (size_t)nrhs * 3 * kHaloT * S;
+    const size_t total = (size_t)nrhs * 3 * kHopMax * S;
     unsigned grid = (unsigned)((total + 255) / 256);
     if (grid > 148 * 8) grid = 148 * 8;
     if (h->prec == HISQ_FP32)
-        halo_kernel<float, PACK><<<grid, 256, 0, h->stream>>>((float*)field, (float*)lo, (float*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHaloT, nrhs);
+        halo_kernel<float, PACK><<<grid, 256, 0, h->stream>>>((float*)field, (float*)lo, (float*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHopMax, nrhs);
     else
-        halo_kernel<double, PACK><<<grid, 256, 0, h->stream>>>((double*)field, (double*)lo, (double*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHaloT, nrhs);
+        halo_kernel<double, PACK><<<grid, 256, 0, h->stream>>>((double*)field, (double*)lo, (double*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHopMax, nrhs);
     h->stats.launches++;
     CK(cudaGetLastError());
     return HISQ_OK;
@@ -1041,6 +1048,85 @@ extern "C" int hisq_halo_pack(hisq_ctx* h, void* send_lo, void* send_hi, const v
 extern "C" int hisq_halo_unpack(hisq_ctx* h, void* field, const void* recv_lo, const void* recv_hi, int nrhs)
 {
     return halo_move<false>(h, field, const_cast<void*>(recv_lo), const_cast<void*>(recv_hi), nrhs);
+}
+
+// ---- halo transport through peer-mapped memory (no library collective) ----------------------------------------
+// Mailbox = [16 flags (u32), 256 B][slot 0: lo, hi][slot 1: lo, hi].  Flags, all exchange numbers e = 1, 2, ...:
+//   ready_lo[s] (0+s): my lower-halo buffer of slot s holds exchange e      (written by the previous rank)
+//   ready_hi[s] (2+s): my upper-halo buffer of slot s holds exchange e      (written by the next rank)
+//   free_up[s]  (4+s): the next rank has unpacked what I put in ITS lo buffer of slot s for exchange e
+//   free_down[s](6+s): the previous rank has unpacked what I put in ITS hi buffer of slot s
+// Waiting and signalling are stream memory operations (cuStreamWaitValue32 / cuStreamWriteValue32): no kernel spins.
+static const size_t kMboxFlags = 256;
+typedef CUresult (*StreamMemOp32)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
+static StreamMemOp32 g_wait32 = nullptr, g_write32 = nullptr;
+static bool load_memops()
+{
+    if (g_wait32 && g_write32) return true;
+    void *w = nullptr, *r = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &w, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) return false;
+    if (cudaGetDriverEntryPoint("cuStreamWriteValue32", &r, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) return false;
+    g_wait32 = (StreamMemOp32)w; g_write32 = (StreamMemOp32)r;
+    return true;
+}
+static char* mbox_buffer(char* box, size_t buf, int slot, int hi) { return box + kMboxFlags + (size_t)(2 * slot + hi) * buf; }
+static CUdeviceptr mbox_flag(char* box, int which, int slot) { return (CUdeviceptr)(uintptr_t)(box + 4 * (which * 2 + slot)); }
+
+extern "C" size_t hisq_peer_bytes(const hisq_ctx* h, int nrhs)
+{
+    const size_t b = hisq_halo_bytes(h, nrhs);
+    return b ? kMboxFlags + 4 * align_up(b) : 0;
+}
+extern "C" int hisq_peer_attach(hisq_ctx* h, void* mine, void* up, void* down, int nrhs)
+{
+    if (!h || !h->g.part || !mine || !up || !down || nrhs < 1 || nrhs > HISQ_MAX_NRHS) return HISQ_EINVAL;
+    if (((uintptr_t)mine & 255) || ((uintptr_t)up & 255) || ((uintptr_t)down & 255)) return HISQ_EINVAL;
+    if (!load_memops()) { h->last_error = "stream memory operations (cuStreamWaitValue32) are not available"; return HISQ_ECUDA; }
+    h->mbox = (char*)mine; h->mbox_up = (char*)up; h->mbox_down = (char*)down;
+    h->mbox_buf = align_up(hisq_halo_bytes(h, nrhs));
+    h->mbox_nrhs = nrhs;
+    h->seq_send = h->seq_recv = 0;
+    return HISQ_OK;
+}
+#define CKU(call)                                                                                         \
+    do {                                                                                                  \
+        CUresult r_ = (call);                                                                             \
+        if (r_ != CUDA_SUCCESS) { h->last_error = std::string(#call) + ": CUresult " + std::to_string((int)r_); return HISQ_ECUDA; } \
+    } while (0)
+extern "C" int hisq_halo_send(hisq_ctx* h, const void* field, int nrhs)
+{
+    if (!h || !field || !h->mbox || nrhs < 1 || nrhs > h->mbox_nrhs) return HISQ_EINVAL;
+    const unsigned e = ++h->seq_send;
+    const int s = (int)(e & 1u);
+    CUstream st = (CUstream)h->stream;
+    if (e > 2) {   // the buffers of this slot were last used by exchange e - 2: both neighbours must have unpacked them
+        CKU(g_wait32(st, mbox_flag(h->mbox, 2, s), e - 2, CU_STREAM_WAIT_VALUE_GEQ));
+        CKU(g_wait32(st, mbox_flag(h->mbox, 3, s), e - 2, CU_STREAM_WAIT_VALUE_GEQ));
+    }
+    // my lowest slices -> the previous rank's UPPER halo buffer, my highest -> the next rank's LOWER halo buffer
+    int rc = halo_move<true>(h, const_cast<void*>(field), mbox_buffer(h->mbox_down, h->mbox_buf, s, 1),
+                             mbox_buffer(h->mbox_up, h->mbox_buf, s, 0), nrhs);
+    if (rc) return rc;
+    CKU(g_write32(st, mbox_flag(h->mbox_up, 0, s), e, CU_STREAM_WRITE_VALUE_DEFAULT));
+    CKU(g_write32(st, mbox_flag(h->mbox_down, 1, s), e, CU_STREAM_WRITE_VALUE_DEFAULT));
+    return HISQ_OK;
+}
+extern "C" int hisq_halo_recv(hisq_ctx* h, void* field, int nrhs)
+{
+    if (!h || !field || !h->mbox || nrhs < 1 || nrhs > h->mbox_nrhs) return HISQ_EINVAL;
+    if (h->seq_recv >= h->seq_send) return HISQ_EINVAL;   // nothing sent for this exchange: the neighbours would wait for ever
+    const unsigned e = ++h->seq_recv;
+    const int s = (int)(e & 1u);
+    CUstream st = (CUstream)h->stream;
+    CKU(g_wait32(st, mbox_flag(h->mbox, 0, s), e, CU_STREAM_WAIT_VALUE_GEQ));
+    CKU(g_wait32(st, mbox_flag(h->mbox, 1, s), e, CU_STREAM_WAIT_VALUE_GEQ));
+    int rc = halo_move<false>(h, field, mbox_buffer(h->mbox, h->mbox_buf, s, 0), mbox_buffer(h->mbox, h->mbox_buf, s, 1), nrhs);
+    if (rc) return rc;
+    // I am the previous rank's "up" neighbour and the next rank's "down" neighbour
+    CKU(g_write32(st, mbox_flag(h->mbox_down, 2, s), e, CU_STREAM_WRITE_VALUE_DEFAULT));
+    CKU(g_write32(st, mbox_flag(h->mbox_up, 3, s), e, CU_STREAM_WRITE_VALUE_DEFAULT));
+    return HISQ_OK;
 }
 
 extern "C" int hisq_naik_compressed(const hisq_ctx* h) { return h && h->naik_c13 ? 1 : 0; }

@@ -115,27 +115,79 @@ def exchange_halos(send_lo, send_hi, recv_lo, recv_hi, rank: int, nranks: int, d
 
 
 def dslash_partitioned(ctx, field_in: torch.Tensor, parity: int, rank: int, nranks: int, dist=None, out=None,
-                       overlap: bool = True):
+                       overlap: bool = True, peer=None):
     """What one rank does per Dslash application: pack the halo of `field_in`, exchange it, compute.  overlap: the owned
     slices that read no halo are computed while the exchange is in flight, the first and last 3 afterwards
     (hisq_dslash_slices; PAPER.md:340-348 'communication hidden behind computation')."""
     n = field_in.shape[0]
-    slo, shi = ctx.halo_buffers(n)
-    rlo, rhi = ctx.halo_buffers(n)
-    ctx.halo_pack(field_in, slo, shi)
-    ex = begin_exchange(slo, shi, rlo, rhi, rank, nranks, dist)
+    if peer is not None:             # PeerHalo: the pack kernel writes into the neighbours' mailboxes
+        peer.send(field_in)
+        arrive = lambda: peer.recv(field_in)
+    else:
+        slo, shi = ctx.halo_buffers(n)
+        rlo, rhi = ctx.halo_buffers(n)
+        ctx.halo_pack(field_in, slo, shi)
+        ex = begin_exchange(slo, shi, rlo, rhi, rank, nranks, dist)
+
+        def arrive():
+            ex.finish()
+            ctx.halo_unpack(field_in, rlo, rhi)
     nt = ctx.L[3] - 2 * HALO_T
     if not overlap or nt <= 2 * HOP_MAX:
-        ex.finish()
-        ctx.halo_unpack(field_in, rlo, rhi)
+        arrive()
         return ctx.dslash(field_in, parity, out=out)
     if out is None:
         out = ctx.new_field(n)
     ctx.dslash_slices(field_in, parity, out, HOP_MAX, nt - 2 * HOP_MAX)
-    ex.finish()
-    ctx.halo_unpack(field_in, rlo, rhi)
+    arrive()
     ctx.dslash_edges(field_in, parity, out, HOP_MAX)
     return out
+
+
+class PeerHalo:
+    """Halo exchange through mailboxes in peer-mapped device memory (include/hisq.h, hisq_peer_*): the packing kernel
+    stores straight into the neighbours' memory over NVLink and stream memory operations do the signalling -- no
+    communication-library call on the data path.  This class is the plumbing: it allocates this rank's mailbox,
+    hands a CUDA IPC mapping of it to the other ranks of the node (through `dist`'s object collectives; one process per
+    GPU) and attaches the neighbours' mappings to the context.  dist = None or one rank: the ring closes on itself."""
+
+    def __init__(self, ctx, rank: int, nranks: int, nrhs: int, dist=None):
+        self.ctx, self.dist, self.nranks = ctx, dist, nranks
+        self.mine = ctx.peer_mailbox(nrhs)
+        torch.cuda.synchronize(ctx.device)          # zeroed before anybody can see it
+        if nranks == 1 or dist is None:
+            up = down = self.mine
+        else:
+            from torch.multiprocessing.reductions import reduce_tensor
+            shared = [None] * nranks
+            dist.all_gather_object(shared, reduce_tensor(self.mine))
+            boxes = {}
+            for r in {(rank + 1) % nranks, (rank - 1) % nranks}:
+                rebuild, args = shared[r]
+                boxes[r] = rebuild(*args)
+                if boxes[r].device != ctx.device:
+                    # a first copy makes torch enable peer access from this GPU to the owner's (kernels need it too)
+                    torch.empty(1, dtype=torch.uint8, device=ctx.device).copy_(boxes[r][:1])
+            up, down = boxes[(rank + 1) % nranks], boxes[(rank - 1) % nranks]
+        ctx.peer_attach(self.mine, up, down, nrhs)
+        self._barrier()
+
+    def _barrier(self):
+        torch.cuda.synchronize(self.ctx.device)
+        if self.dist is not None and self.nranks > 1:
+            self.dist.barrier()
+
+    def send(self, field):
+        self.ctx.halo_send(field)
+
+    def recv(self, field):
+        self.ctx.halo_recv(field)
+
+    def close(self):
+        """Collective: nobody frees a mailbox a neighbour may still be writing to."""
+        self._barrier()
+        self.ctx._mailboxes = None
+        self.mine = None
 
 
 class PartitionedCG:
@@ -143,10 +195,15 @@ class PartitionedCG:
     library's; this class only sequences the phases and performs the two cross-rank steps between them -- halo
     exchange of a field and all-reduce of nrhs doubles -- through `dist` (torch.distributed: NCCL between GPUs)."""
 
-    def __init__(self, ctx, rank: int, nranks: int, dist=None):
-        self.ctx, self.rank, self.nranks, self.dist = ctx, rank, nranks, dist
+    def __init__(self, ctx, rank: int, nranks: int, dist=None, peer: "PeerHalo | None" = None):
+        """peer: move the halos through peer-mapped mailboxes (PeerHalo) instead of `dist` send / recv; the all-reduces
+        of the scalar products still go through `dist`."""
+        self.ctx, self.rank, self.nranks, self.dist, self.peer = ctx, rank, nranks, dist, peer
 
     def _halo_begin(self, field):
+        if self.peer is not None:
+            self.peer.send(field)
+            return None
         n = field.shape[0]
         slo, shi = self.ctx.halo_buffers(n)
         rlo, rhi = self.ctx.halo_buffers(n)
@@ -154,6 +211,9 @@ class PartitionedCG:
         return begin_exchange(slo, shi, rlo, rhi, self.rank, self.nranks, self.dist), rlo, rhi
 
     def _halo_end(self, field, pending):
+        if self.peer is not None:
+            self.peer.recv(field)
+            return
         ex, rlo, rhi = pending
         ex.finish()
         self.ctx.halo_unpack(field, rlo, rhi)

@@ -14,7 +14,7 @@ from tests.helpers import oracle_field, oracle_links
 pytestmark = pytest.mark.gpu
 
 
-def _run(L, prec, nranks, nrhs, parity, seed, overlap=False):
+def _run(L, prec, nranks, nrhs, parity, seed, overlap=False, peer=False):
     dev = torch.device("cuda:0")
     ctxs, fields, bufs = [], [], []
     for r in range(nranks):
@@ -24,8 +24,16 @@ def _run(L, prec, nranks, nrhs, parity, seed, overlap=False):
         src = partition.make_sources_part(L, seed + 1, nrhs, 1 - parity, r, nranks, dev, ctx.cdtype)
         f = ctx.pack(src)
         slo, shi = ctx.halo_buffers(nrhs)
-        ctx.halo_pack(f, slo, shi)
+        if not peer:
+            ctx.halo_pack(f, slo, shi)
         ctxs.append(ctx); fields.append(f); bufs.append((slo, shi))
+    if peer:
+        # mailboxes in the one process: plain device pointers.  All sends are enqueued before any recv (one stream).
+        boxes = [c.peer_mailbox(nrhs) for c in ctxs]
+        for r, c in enumerate(ctxs):
+            c.peer_attach(boxes[r], boxes[(r + 1) % nranks], boxes[(r - 1) % nranks], nrhs)
+        for c, f in zip(ctxs, fields):
+            c.halo_send(f)
     outs = []
     nt, w = L[3] // nranks, partition.HOP_MAX
     for r, ctx in enumerate(ctxs):
@@ -40,10 +48,10 @@ def _run(L, prec, nranks, nrhs, parity, seed, overlap=False):
             v[:, :, :partition.HALO_T] = float("nan")
             v[:, :, ctx.L[3] - partition.HALO_T:] = float("nan")
             ctx.dslash_slices(fields[r], parity, out, w, nt - 2 * w)
-            ctx.halo_unpack(fields[r], rlo, rhi)
+            ctx.halo_recv(fields[r]) if peer else ctx.halo_unpack(fields[r], rlo, rhi)
             ctx.dslash_edges(fields[r], parity, out, w)
         else:
-            ctx.halo_unpack(fields[r], rlo, rhi)
+            ctx.halo_recv(fields[r]) if peer else ctx.halo_unpack(fields[r], rlo, rhi)
             ctx.dslash(fields[r], parity, out=out)
         outs.append(ctx.unpack(out).cpu().numpy().astype(np.complex128))
     # gather the interiors into a global full-lattice field
@@ -93,6 +101,9 @@ def test_partitioned_dslash_equals_single_lattice_and_oracle(nranks, prec):
         # interior / boundary split around the exchange (hisq_dslash_slices): the same bits
         full_o, seen_o = _run(L, prec, nranks, nrhs, parity, seed, overlap=True)
         assert np.array_equal(seen_o, seen) and np.array_equal(full_o, full)
+        # halos moved through the mailboxes (hisq_halo_send / recv) instead of pack / copy / unpack: the same bits
+        full_p, seen_p = _run(L, prec, nranks, nrhs, parity, seed, overlap=(parity == 0), peer=True)
+        assert np.array_equal(seen_p, seen) and np.array_equal(full_p, full)
 
 
 @pytest.mark.parametrize("prec", ["fp64", "fp32"])
@@ -143,7 +154,7 @@ def test_partitioned_context_rejects_solvers_and_bad_splits():
         binding.Hisq((4, 4, 4, 8), "fp64", 1, part=(0, 4))       # Lt_loc = 2 < 4
 
 
-def _emulated_cg(L, prec, nranks, nrhs, m, tol, seed, overlap=False):
+def _emulated_cg(L, prec, nranks, nrhs, m, tol, seed, overlap=False, peer=False):
     """All ranks in lockstep on one GPU: every phase is run for rank 0..G-1 in turn, the cross-rank steps (ring halo
     exchange, all-reduce) are done by hand between the phases -- the same sequence as partition.PartitionedCG.solve."""
     dev = torch.device("cuda:0")
@@ -163,8 +174,19 @@ def _emulated_cg(L, prec, nranks, nrhs, m, tol, seed, overlap=False):
         for t in ts:
             t.copy_(tot)
 
+    if peer:
+        boxes = [c.peer_mailbox(nrhs) for c in ctxs]
+        for r, c in enumerate(ctxs):
+            c.peer_attach(boxes[r], boxes[(r + 1) % nranks], boxes[(r - 1) % nranks], nrhs)
+
     def halo(which, between=None):
         fields = [c.cgp_tensor(which, nrhs) for c in ctxs]
+        if peer:
+            for c, f in zip(ctxs, fields): c.halo_send(f)
+            if between is not None:
+                for c in ctxs: c.cgp_phase(between, m)
+            for c, f in zip(ctxs, fields): c.halo_recv(f)
+            return
         bufs = []
         for c, f in zip(ctxs, fields):
             slo, shi = c.halo_buffers(nrhs)
@@ -229,6 +251,9 @@ def test_partitioned_cg_matches_oracle_and_single_lattice(nranks):
     # Dslashes split around the halo exchange (phases 20/21, 30/31): same sums in the same order -> the same iterates
     x2, st2 = _emulated_cg(L, "fp64", nranks, nrhs, m, tol, seed, overlap=True)
     assert st2["iterations"] == st["iterations"] and np.array_equal(x2, x)
+    # ... and with the halos moved through peer mailboxes (double-buffered: hundreds of exchanges reuse two slots)
+    x3, st3 = _emulated_cg(L, "fp64", nranks, nrhs, m, tol, seed, overlap=True, peer=True)
+    assert st3["iterations"] == st["iterations"] and np.array_equal(x3, x)
 
 
 def test_partitioned_cg_driver_single_rank_equals_hisq_cg():
@@ -254,7 +279,7 @@ def test_partitioned_cg_driver_single_rank_equals_hisq_cg():
     ctx.close(); ref.close()
 
 
-def _mp_worker(rank, world, port, L, m, tol, seed, q):
+def _mp_worker(rank, world, port, L, m, tol, seed, q, transport):
     import os, sys
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     import torch.distributed as dist
@@ -264,7 +289,10 @@ def _mp_worker(rank, world, port, L, m, tol, seed, q):
     fat, naik = partition.make_links_part(L, seed, rank, world, dev)
     ctx.set_links(fat, naik)
     b = ctx.pack(partition.make_sources_part(L, seed + 1, 1, 0, rank, world, dev))
-    x, st = partition.PartitionedCG(ctx, rank, world, dist).solve(b, m, tol, check_every=8)
+    peer = partition.PeerHalo(ctx, rank, world, 1, dist) if transport == "peer" else None
+    x, st = partition.PartitionedCG(ctx, rank, world, dist, peer=peer).solve(b, m, tol, check_every=8)
+    if peer is not None:
+        peer.close()
     Le = partition.extended_lattice(L, world)
     S = ctx.Vh // Le[3]
     xi = ctx.unpack(x).view(1, Le[3], S, 3)[:, partition.HALO_T:Le[3] - partition.HALO_T].reshape(1, -1, 3).cpu()
@@ -278,21 +306,30 @@ def _mp_worker(rank, world, port, L, m, tol, seed, q):
     dist.destroy_process_group()
 
 
-def test_partitioned_cg_two_processes_gloo_on_one_gpu():
+@pytest.mark.parametrize("transport", ["dist", "peer"])
+def test_partitioned_cg_two_processes_gloo_on_one_gpu(transport):
     """The real thing minus the second GPU: two PROCESSES, each with its own context, exchanging halos and all-reducing
-    through torch.distributed (gloo here, NCCL between GPUs), run partition.PartitionedCG.solve."""
+    through torch.distributed (gloo here, NCCL between GPUs), run partition.PartitionedCG.solve.
+    transport = "peer": the halos go through mailboxes mapped into the other process by CUDA IPC (partition.PeerHalo;
+    the packing kernel stores into the neighbour's memory, stream memory operations signal) -- no kernel waits on
+    another one, the streams do."""
     import torch.multiprocessing as mp
     L, m, tol, seed, world = (4, 4, 6, 16), 0.15, 1e-9, 8, 2
     ctxmp = mp.get_context("spawn")
     q = ctxmp.Queue()
-    port = 33500 + __import__("os").getpid() % 2000
-    ps = [ctxmp.Process(target=_mp_worker, args=(r, world, port, L, m, tol, seed, q)) for r in range(world)]
+    port = 33500 + __import__("os").getpid() % 2000 + (17 if transport == "peer" else 0)
+    ps = [ctxmp.Process(target=_mp_worker, args=(r, world, port, L, m, tol, seed, q, transport)) for r in range(world)]
     for p in ps:
         p.start()
-    st, parts = q.get(timeout=150)
-    for p in ps:
-        p.join(timeout=120)
-        assert p.exitcode == 0
+    try:
+        st, parts = q.get(timeout=150)
+        for p in ps:
+            p.join(timeout=120)
+            assert p.exitcode == 0
+    finally:
+        for p in ps:          # exactly the processes started above
+            if p.is_alive():
+                p.kill()
     assert st["done"] and not st["breakdown"]
     # rank r's interior = global even sites with t in [r*Lt_loc, (r+1)*Lt_loc), in global half-index order
     xh = np.concatenate(parts, axis=1).astype(np.complex128)
