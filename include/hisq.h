@@ -119,7 +119,8 @@ int hisq_cg_multishift(hisq_ctx *h, void *x, const void *b, double mass, const d
  * "tile_y", "tile_z" (CTA sweep order blocking in y,z; 0 = auto),
  * "naik_compress" (see hisq_naik_compressed; default 0), "fused_blas" (1: cooperative fused x/r/p update kernel when the
  * fields are small enough to stay in registers across a grid barrier, default 1), "window_mb" (L2 budget of the CTA sweep
- * order, default 20). */
+ * order, default 20), "overlap" (hisq_cg on a partitioned context: compute the slices that read no halo while the halo is
+ * in flight; -1 = when at least half of the owned slices qualify (Lt_loc >= 12), 0 never, 1 always; default -1). */
 int hisq_set_option(hisq_ctx *h, const char *key, double value);
 
 /* After hisq_cg: iterations done, number of fp64 true-residual recomputations, and per RHS the true
@@ -145,8 +146,10 @@ int hisq_cg_host(hisq_ctx *h, void *x_host, const void *b_host, double mass, dou
  * hisq_dslash computes the interior slices only, reads t-neighbours from the halo slices of `in` (which the caller
  * must have filled: hisq_halo_pack -> exchange with the neighbouring ranks -> hisq_halo_unpack), and applies the
  * antiperiodic sign only on the ranks that own the global t boundary.  Halo slices of `out` are left untouched.
- * Lt_loc must be even and >= 4.  hisq_cg / hisq_cg_multishift are not available on partitioned contexts (they would
- * need a cross-rank reduction): HISQ_EINVAL. */
+ * Lt_loc must be even and >= 4.  hisq_cg on a partitioned context (fp32 or fp64) solves across the ranks once the peer
+ * mailboxes are attached (hisq_peer_attach, below; HISQ_EINVAL before): every rank calls it with its slab of b and
+ * gets its slab of x; same arithmetic and stopping rule as on one GPU except that the final true-residual check is
+ * left out (hisq_get_info reports the recursive residuals).  hisq_cg_multishift and HISQ_MIXED: HISQ_EINVAL. */
 int hisq_create_part(hisq_ctx **h, int Lx, int Ly, int Lz, int Lt_global, int prec, int rank, int nranks);
 /* hisq_dslash restricted to the OWNED time slices [t_first, t_first + t_count) (0 <= t_first, t_first + t_count <= the
  * number of owned slices: Lt_loc on a partitioned context, Lt otherwise); all other slices of `out` are left untouched.
@@ -166,27 +169,36 @@ int hisq_halo_pack(hisq_ctx *h, void *send_lo, void *send_hi, const void *field,
 /* lower halo <- recv_lo (what the previous rank packed as send_hi), upper halo <- recv_hi (the next rank's send_lo). */
 int hisq_halo_unpack(hisq_ctx *h, void *field, const void *recv_lo, const void *recv_hi, int nrhs);
 
-/* Halo transport through peer-mapped memory, without a communication library (the exchange of PAPER.md:340-348 done
- * by the packing kernel's own stores over NVLink).  Every rank owns a MAILBOX of hisq_peer_bytes(h, nrhs) bytes of
- * device memory (256-byte aligned, ZEROED by the caller before any neighbour attaches) that its t-neighbours can
- * address: cudaDeviceEnablePeerAccess within a process, a CUDA IPC mapping between processes -- obtaining those
- * pointers is the caller's plumbing.  hisq_peer_attach(h, mine, up, down, nrhs): mailboxes of this rank, of rank+1
- * and of rank-1 (periodic; all three the same pointer for a single rank, up == down for two ranks); nrhs = the
- * capacity the mailboxes were sized for.  Then, per exchange and in this order on every rank:
+/* Halo transport and all-reduce through peer-mapped memory, without a communication library (the exchange of
+ * PAPER.md:340-348 done by the packing kernel's own stores over NVLink).  Every rank owns a MAILBOX of
+ * hisq_peer_bytes(h, nrhs) bytes of device memory (256-byte aligned, ZEROED by the caller before any other rank
+ * attaches) that the other ranks can address: cudaDeviceEnablePeerAccess within a process, a CUDA IPC mapping between
+ * processes -- obtaining those pointers is the caller's plumbing.
+ * hisq_peer_attach(h, boxes, nboxes, nrhs): boxes[r] = mailbox of rank r as addressable from this device (boxes[own
+ * rank] = this rank's), nboxes = nranks of hisq_create_part (<= 16); nrhs = the capacity the mailboxes were sized for.
+ * Then, per halo exchange and in this order on every rank:
  *   hisq_halo_send(h, field, nrhs)   packs the 3 lowest / highest owned slices of `field` straight into the
- *                                     neighbours' mailboxes and raises their "ready" flags;
- *   hisq_halo_recv(h, field, nrhs)   waits for this rank's "ready" flags, unpacks its mailbox into the halo slices of
- *                                     `field`, and raises the neighbours' "free" flags.
- * Both are asynchronous on the context's stream; waiting and signalling are stream memory operations
- * (cuStreamWaitValue32 / cuStreamWriteValue32), so no kernel spins and work enqueued between send and recv (the
- * interior slices, hisq_dslash_slices) overlaps the transfer.  Mailboxes are double-buffered: send number e waits
- * until both neighbours have unpacked exchange e-2.  Every rank must issue the same sequence of send / recv calls;
- * a recv without a matching earlier send on the same rank is refused (HISQ_EINVAL).  HISQ_ECUDA if the driver lacks
+ *                                     t-neighbours' mailboxes; the kernel's last CTA bumps their arrival counters;
+ *   hisq_halo_recv(h, field, nrhs)   waits (stream memory operation) until both neighbours' halos have arrived and
+ *                                     unpacks its mailbox into the halo slices of `field`.
+ * and per all-reduce (sum over ranks of the first nrhs doubles of a CG state array; which = 2 rho, 3 pq, 4 sums as in
+ * hisq_cgp_ptr; in place):
+ *   hisq_peer_reduce_send(h, which, nrhs)   stores the local values into every rank's mailbox, bumps its counter;
+ *   hisq_peer_reduce_recv(h, which, nrhs)   waits until all ranks' values have arrived and adds them in rank order
+ *                                            (the same order on every rank: all ranks end up with the same bits).
+ * All four are asynchronous on the context's stream.  Signalling = system-scope atomics issued by the sending kernel
+ * after fencing its stores; waiting = cuStreamWaitValue32 on the receiver's stream: no kernel spins, and work enqueued
+ * between send and recv (the interior slices, hisq_dslash_slices) overlaps the transfer.  Mailboxes hold two slots
+ * used in turn.  Every rank must issue the same sequence of calls, sends and recvs strictly alternating (send e,
+ * recv e, send e+1, ...; likewise for reduces) -- that order is what makes a slot safe to overwrite two exchanges
+ * later without any acknowledgement; a call out of order is refused (HISQ_EINVAL).  HISQ_ECUDA if the driver lacks
  * stream memory operations. */
 size_t hisq_peer_bytes(const hisq_ctx *h, int nrhs);
-int hisq_peer_attach(hisq_ctx *h, void *mine, void *up, void *down, int nrhs);
+int hisq_peer_attach(hisq_ctx *h, void *const *boxes, int nboxes, int nrhs);
 int hisq_halo_send(hisq_ctx *h, const void *field, int nrhs);
 int hisq_halo_recv(hisq_ctx *h, void *field, int nrhs);
+int hisq_peer_reduce_send(hisq_ctx *h, int which, int nrhs);
+int hisq_peer_reduce_recv(hisq_ctx *h, int which, int nrhs);
 
 /* CG on a t-partitioned lattice, phase by phase.  The solver's reductions span all ranks, so the iteration is cut where
  * a cross-rank step is due and the CALLER performs it between the calls (halo exchange of a field through

@@ -25,7 +25,7 @@ EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
     "hisq_set_links", "hisq_dslash", "hisq_apply_A", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
     "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count",
-    "hisq_create_part", "hisq_peer_bytes", "hisq_peer_attach", "hisq_halo_send", "hisq_halo_recv", "hisq_dslash_slices", "hisq_dslash_edges", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
+    "hisq_create_part", "hisq_peer_bytes", "hisq_peer_attach", "hisq_halo_send", "hisq_halo_recv", "hisq_peer_reduce_send", "hisq_peer_reduce_recv", "hisq_dslash_slices", "hisq_dslash_edges", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
     "hisq_cgp_begin", "hisq_cgp_phase", "hisq_cgp_ptr", "hisq_cgp_status", "hisq_strerror",
     "hisq_last_error",
 ]
@@ -74,7 +74,9 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_halo_bytes.restype = sz
     lib.hisq_peer_bytes.argtypes = [vp, i]
     lib.hisq_peer_bytes.restype = sz
-    lib.hisq_peer_attach.argtypes = [vp, vp, vp, vp, i]
+    lib.hisq_peer_attach.argtypes = [vp, ctypes.POINTER(vp), i, i]
+    lib.hisq_peer_reduce_send.argtypes = [vp, i, i]
+    lib.hisq_peer_reduce_recv.argtypes = [vp, i, i]
     lib.hisq_halo_send.argtypes = [vp, vp, i]
     lib.hisq_halo_recv.argtypes = [vp, vp, i]
     lib.hisq_halo_pack.argtypes = [vp, vp, vp, vp, i]
@@ -301,9 +303,17 @@ class Hisq:
             raise HisqError(-1, "not a partitioned context")
         return torch.zeros(nb, dtype=torch.uint8, device=self.device)
 
-    def peer_attach(self, mine: torch.Tensor, up: torch.Tensor, down: torch.Tensor, nrhs: int):
-        self._mailboxes = (mine, up, down)     # keep the mappings alive as long as the context uses them
-        self._check(self.lib.hisq_peer_attach(self._h, mine.data_ptr(), up.data_ptr(), down.data_ptr(), int(nrhs)))
+    def peer_attach(self, boxes, nrhs: int):
+        """boxes[r]: rank r's mailbox as a tensor addressable from this device (own rank: this context's)."""
+        self._mailboxes = list(boxes)          # keep the mappings alive as long as the context uses them
+        arr = (ctypes.c_void_p * len(boxes))(*[b.data_ptr() for b in boxes])
+        self._check(self.lib.hisq_peer_attach(self._h, arr, len(boxes), int(nrhs)))
+
+    def peer_reduce_send(self, which: int, nrhs: int):
+        self._check(self.lib.hisq_peer_reduce_send(self._h, int(which), int(nrhs)))
+
+    def peer_reduce_recv(self, which: int, nrhs: int):
+        self._check(self.lib.hisq_peer_reduce_recv(self._h, int(which), int(nrhs)))
 
     def halo_send(self, field: torch.Tensor):
         self._check(self.lib.hisq_halo_send(self._h, self._ptr(field), field.shape[0]))

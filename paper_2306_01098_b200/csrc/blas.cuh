@@ -110,15 +110,21 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_p_kernel(T* __restrict__
 template <typename T>
 __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict__ x, T* __restrict__ r, const T* __restrict__ p,
                                                                   const T* __restrict__ q, size_t nreal, CgState* st,
-                                                                  double* partial, int defer = 0)
+                                                                  double* partial, int defer = 0, PeerPush push = PeerPush(),
+                                                                  const double* red_pq = nullptr)
 {
-    if (st->done) return;
+    // defer = 1 (partitioned lattice).  red_pq: <p,q> is not in st->pq yet but, rank by rank, in this slot of the
+    // mailbox (every block adds them up itself); push: the last block hands the local ||r||^2 to all ranks.
+    if (st->done) {   // finished: keep the other ranks' arrival count right (see dslash_kernel)
+        if (push.boxes != nullptr && blockIdx.x == 0 && blockIdx.y == 0) peer_push(push, st->sums, gridDim.y);
+        return;
+    }
     using V = typename V16<T>::type;
     constexpr int N = V16<T>::n;
     const int k = blockIdx.y;
     double alpha_d = 0.0;
     if (st->active[k]) {
-        const double pq = st->pq[k];
+        const double pq = red_pq ? peer_sum(red_pq, push.nranks, k) : st->pq[k];
         alpha_d = (pq > 0.0 && isfinite(pq)) ? st->rho[k] / pq : 0.0;
     }
     const T alpha = (T)alpha_d;
@@ -157,7 +163,11 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict_
                                    totals)) {
         const int n = gridDim.y;
         if (defer) {   // partitioned lattice: only the LOCAL sums; the scalar update runs after the cross-rank all-reduce
-            if (threadIdx.x < n) st->sums[threadIdx.x] = totals[threadIdx.x];
+            if (threadIdx.x < n) {
+                st->sums[threadIdx.x] = totals[threadIdx.x];
+                if (red_pq) st->pq[threadIdx.x] = peer_sum(red_pq, push.nranks, threadIdx.x);   // for the scalar update
+            }
+            if (push.boxes) peer_push(push, totals, n);
             return;
         }
         if (threadIdx.x < n) {
@@ -299,11 +309,12 @@ __global__ void __launch_bounds__(kBlasBlock) cg_fused_update_kernel(T* __restri
 }
 
 // ---- partitioned-lattice CG (row f3): scalar updates that consume GLOBAL (all-reduced) sums ------------------------
-__global__ void cgp_finalize_init_kernel(CgState* st, int n, double tol, int max_iter)
+__global__ void cgp_finalize_init_kernel(CgState* st, int n, double tol, int max_iter, const double* red = nullptr, int nranks = 0)
 {
     int any = 0;
     for (int k = 0; k < n; ++k) {
-        const double bb = st->rho[k];       // all-reduced ||b_k||^2
+        const double bb = red ? peer_sum(red, nranks, k) : st->rho[k];       // all-reduced ||b_k||^2
+        st->rho[k] = bb;
         st->rho_prev[k] = bb; st->bnorm2[k] = bb; st->pq[k] = 1.0; st->beta[k] = 0.0; st->sums[k] = 0.0;
         st->active[k] = bb > 0.0 ? 1 : 0;
         any |= st->active[k];
@@ -312,13 +323,13 @@ __global__ void cgp_finalize_init_kernel(CgState* st, int n, double tol, int max
     st->done = any ? 0 : 1;
 }
 
-__global__ void cgp_finalize_xr_kernel(CgState* st, int n)
+__global__ void cgp_finalize_xr_kernel(CgState* st, int n, const double* red_sums = nullptr, int nranks = 0)
 {
     if (st->done) return;
     int any = 0;
     for (int k = 0; k < n; ++k) {
         if (st->active[k]) {
-            const double rn = st->sums[k], pq = st->pq[k];   // both all-reduced
+            const double rn = red_sums ? peer_sum(red_sums, nranks, k) : st->sums[k], pq = st->pq[k];   // both all-reduced
             if (!(pq > 0.0) || !isfinite(pq) || !isfinite(rn)) st->breakdown = 1;
             st->rho_prev[k] = st->rho[k];
             st->beta[k] = rn / st->rho[k];
@@ -420,9 +431,12 @@ __global__ void __launch_bounds__(256) spinor_layout_kernel(T* __restrict__ dst,
 //         hi <- interior slices [t_lo+t_cnt-H, t_lo+t_cnt) (goes to the next rank's LOWER halo)
 // UNPACK: lower halo [t_lo-H, t_lo) <- lo (received from the previous rank), upper halo [t_lo+t_cnt, +H) <- hi.
 // Buffers are [k][c][H*S] complex.
+// sig_a / sig_b (PACK into peer mailboxes only, else null): arrival counters in the two neighbours' mailboxes, bumped
+// once by the last CTA after every CTA's stores have been fenced at system scope -- the kernel signals, nothing waits.
 template <typename T, bool PACK>
 __global__ void __launch_bounds__(256) halo_kernel(T* __restrict__ field, T* __restrict__ lo, T* __restrict__ hi, int S, int Lt_ext,
-                                                   int t_lo, int t_cnt, int H, int nrhs)
+                                                   int t_lo, int t_cnt, int H, int nrhs, unsigned* ticket, unsigned* sig_a,
+                                                   unsigned* sig_b)
 {
     using C = typename Vec<T>::c1;
     C* f = reinterpret_cast<C*>(field);
@@ -439,6 +453,48 @@ __global__ void __launch_bounds__(256) halo_kernel(T* __restrict__ field, T* __r
             f[plane + (size_t)(t_lo - H) * S + j] = l[i];
             f[plane + (size_t)(t_lo + t_cnt) * S + j] = u[i];
         }
+    }
+    if (PACK && sig_a != nullptr) {
+        // the barrier orders the CTA's stores before thread 0's fence, which is cumulative (the grid.sync idiom):
+        // one system-scope fence per CTA instead of one per thread
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence_system();
+            const unsigned done = atomicAdd(ticket, 1u);
+            if (done == gridDim.x - 1) {
+                *ticket = 0;
+                __threadfence_system();
+                atomicAdd_system(sig_a, 1u);
+                atomicAdd_system(sig_b, 1u);
+            }
+        }
+    }
+}
+
+// ---- all-reduce of nrhs doubles through peer-mapped mailboxes (row f3): every rank stores its local sums into EVERY
+// rank's mailbox (slot, source rank) and bumps that mailbox's arrival counter; after a stream wait on its own counter
+// each rank adds the contributions in rank order -- the same order everywhere, so all ranks hold the same bits.
+__global__ void __launch_bounds__(32) peer_reduce_send_kernel(const double* __restrict__ src, PeerBoxes pb, int rank, int slot, int n,
+                                                               size_t data_off, size_t counter_off)
+{
+    char* box = pb.box[blockIdx.x];       // one CTA per destination rank (my own mailbox included)
+    double* dst = reinterpret_cast<double*>(box + data_off) + ((size_t)slot * kMaxRanks + rank) * kMaxNrhs;
+    if (threadIdx.x < n) {
+        dst[threadIdx.x] = src[threadIdx.x];
+        __threadfence_system();
+    }
+    __syncwarp();
+    if (threadIdx.x == 0) atomicAdd_system(reinterpret_cast<unsigned*>(box + counter_off) + slot, 1u);
+}
+
+__global__ void __launch_bounds__(32) peer_reduce_sum_kernel(double* __restrict__ dst, const char* __restrict__ mybox, int nranks, int slot,
+                                                              int n, size_t data_off)
+{
+    const volatile double* d = reinterpret_cast<const volatile double*>(mybox + data_off) + (size_t)slot * kMaxRanks * kMaxNrhs;
+    if (threadIdx.x < n) {
+        double s = 0.0;
+        for (int r = 0; r < nranks; ++r) s += d[(size_t)r * kMaxNrhs + threadIdx.x];
+        dst[threadIdx.x] = s;
     }
 }
 

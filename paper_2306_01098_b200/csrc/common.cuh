@@ -124,6 +124,41 @@ struct CgState {
     int ms_nshift;
 };
 
+// ---- all-reduce through peer-mapped mailboxes (row f3; layout and protocol: hisq.cu, "halo transport") ----------
+constexpr int kMaxRanks = 16;
+constexpr size_t kMboxCounterOff = 8 * sizeof(unsigned);   // reduce arrival counters (one per slot)
+constexpr size_t kMboxDataOff = 256;                        // reduce data [2 slots][kMaxRanks][kMaxNrhs] doubles
+struct PeerBoxes { char* box[kMaxRanks]; };                 // every rank's mailbox as addressable from this device
+struct PeerPush {                                           // boxes == nullptr: off
+    const PeerBoxes* boxes;
+    int nranks, rank, slot;
+};
+
+// The LAST block of a reducing kernel hands its n local sums (vals: shared memory, written before a barrier) to every
+// rank: stores into each mailbox [slot][my rank][k], barrier, then one thread per destination fences at system scope
+// (cumulative over the CTA's stores, the grid.sync idiom) and bumps that mailbox's counter.  Call block-uniformly.
+__device__ __forceinline__ void peer_push(const PeerPush& pp, const double* vals, int n)
+{
+    for (int idx = threadIdx.x; idx < pp.nranks * n; idx += blockDim.x) {
+        const int r = idx / n, k = idx - r * n;
+        double* dst = reinterpret_cast<double*>(pp.boxes->box[r] + kMboxDataOff) + ((size_t)pp.slot * kMaxRanks + pp.rank) * kMaxNrhs;
+        dst[k] = vals[k];
+    }
+    __syncthreads();
+    if ((int)threadIdx.x < pp.nranks) {
+        __threadfence_system();
+        atomicAdd_system(reinterpret_cast<unsigned*>(pp.boxes->box[threadIdx.x] + kMboxCounterOff) + pp.slot, 1u);
+    }
+}
+// Sum over ranks, in rank order (the same bits on every rank), of entry k of one slot of this rank's own mailbox.
+__device__ __forceinline__ double peer_sum(const double* slot_data, int nranks, int k)
+{
+    const volatile double* d = slot_data;
+    double s = 0.0;
+    for (int r = 0; r < nranks; ++r) s += d[(size_t)r * kMaxNrhs + k];
+    return s;
+}
+
 // ---- deterministic two-stage reduction: block partials, then the last block to finish sums them ---
 // vals[NR] are this thread's contributions to right-hand sides k0 .. k0+NR-1.  partial is
 // [nrhs_total][ncols]; this block owns column `col` of rows k0..k0+NR-1.  Returns true in the LAST of

@@ -45,6 +45,7 @@ template <typename T> struct DslashArgs {
     unsigned total_blocks; // CTAs of the whole launch group (epilogue ticket)
     int naik_c13;        // 1: Naik links are stored compressed (13 reals, row f2)
     int t0, tn;          // this launch covers tn owned slices: blockIdx.y = j is slice g.t_lo + t0 + j, plus t_skip for
+    PeerPush push;       // MODE_APPLY_A on a partitioned lattice: the last CTA also hands the sums to every rank's mailbox
     int t_skip_at, t_skip;  // j >= t_skip_at (two ranges in one launch: the first and last slices around an interior).
                          // A launch GROUP (the launches that share one ticket) covers every owned slice exactly once
 };
@@ -311,7 +312,14 @@ template <typename T, int NR, int MODE = 0> struct KernelShape {
 template <typename T, int NR, int MODE, int BLOCK, bool NC>
 __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR, MODE>::minb) dslash_kernel(const DslashArgs<T> a)
 {
-    if (a.done != nullptr && *a.done != 0) return;
+    if (a.done != nullptr && *a.done != 0) {
+        // solver finished: nothing to compute, but the other ranks' streams still wait for this rank's arrival in
+        // the all-reduce of this iteration -- one designated CTA of the launch group keeps the count right
+        if (MODE == MODE_APPLY_A && a.push.boxes != nullptr && blockIdx.x == 0 && blockIdx.z == 0 && a.k0 == 0 &&
+            (int)blockIdx.y + a.t0 + ((int)blockIdx.y >= a.t_skip_at ? a.t_skip : 0) == a.g.t_cnt - 1)
+            peer_push(a.push, a.result, a.nrhs_total);
+        return;
+    }
     const Geom& g = a.g;
     const int Vh = g.Vh, H = g.H;
     const int chunk = blockIdx.x % a.nchunks;
@@ -482,6 +490,7 @@ __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR, MODE>::minb) dslash_
         const int ncols = a.slab_blocks * g.t_cnt * g.nty * g.ntz;
         if (grid_reduce<NR, BLOCK>(red, kg0, a.partial, ncols, col, a.ticket, a.total_blocks, a.nrhs_total, totals)) {
             if (threadIdx.x < a.nrhs_total) a.result[threadIdx.x] = totals[threadIdx.x];
+            if (a.push.boxes) peer_push(a.push, totals, a.nrhs_total);
         }
     }
 }

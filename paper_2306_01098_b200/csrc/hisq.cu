@@ -38,14 +38,20 @@ struct hisq_ctx {
     int fused_blas;        // option: cooperative fused x/r/p update for small fields
     void* cgp_x; int cgp_nrhs; double cgp_tol;   // phase-wise CG on partitioned lattices
     // peer-memory halo transport (hisq_peer_attach): mailboxes of this rank and of its t-neighbours, exchange counters
+    int part_rank, part_nranks;
     char *mbox, *mbox_up, *mbox_down;
+    PeerBoxes mbox_all;    // every rank's mailbox (all-reduce)
+    PeerBoxes* d_boxes;    // the same table in device memory (kernels that push their sums themselves)
+    // set by cgp_solve around the phases whose kernels push / read the cross-rank sums themselves; all null otherwise
+    PeerPush fuse_push_pq, fuse_push_sums;
+    const double *fuse_red_pq, *fuse_red_sums;
     size_t mbox_buf;       // bytes of one halo buffer inside a mailbox
     int mbox_nrhs;
-    unsigned seq_send, seq_recv;
+    unsigned seq_send, seq_recv, red_send, red_recv;
     int num_sms;
     unsigned long long* bad_count;  // device counter used by the compression check
     // options
-    int max_iter, reliable_interval, check_interval, use_graph, nrhs_inner, tile_y, tile_z;
+    int max_iter, reliable_interval, check_interval, use_graph, nrhs_inner, tile_y, tile_z, overlap_opt;
     double window_mb;
     // info of the last solve
     int info_iters, info_reliable;
@@ -126,7 +132,7 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     h->use_graph = 1;
     h->nrhs_inner = 0;
     h->naik_c13 = false; h->naik_compress = 0; h->bad_count = nullptr;
-    h->fused_blas = 1; h->num_sms = 0;
+    h->fused_blas = 1; h->num_sms = 0; h->overlap_opt = -1;
     h->cgp_x = nullptr; h->cgp_nrhs = 0; h->cgp_tol = 0.0;
     { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev); }
     h->tile_y = 0; h->tile_z = 0;
@@ -159,6 +165,7 @@ extern "C" int hisq_create_part(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt_g
     Geom& g = (*out)->g;
     g.part = 1; g.t_lo = kHaloT; g.t_cnt = Lt_loc;
     g.flip_lo = rank == 0; g.flip_hi = rank == nranks - 1;
+    (*out)->part_rank = rank; (*out)->part_nranks = nranks;
     return HISQ_OK;
 }
 
@@ -166,6 +173,7 @@ extern "C" int hisq_destroy(hisq_ctx* h)
 {
     if (!h) return HISQ_EINVAL;
     if (h->host_state) cudaFreeHost(h->host_state);
+    if (h->d_boxes) cudaFree(h->d_boxes);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     for (int i = 0; i < 2; ++i) if (h->poll_ev[i]) cudaEventDestroy(h->poll_ev[i]);
     delete h;
@@ -318,6 +326,7 @@ static int run_dslash(hisq_ctx* h, const T* links, T* out, const T* in, int pari
     a.naik_c13 = h->naik_c13 ? 1 : 0;
     a.t0 = t_first; a.tn = t_count < 0 ? h->g.t_cnt - t_first : t_count;
     a.t_skip_at = t_skip_at; a.t_skip = t_skip;
+    a.push = mode == MODE_APPLY_A ? h->fuse_push_pq : PeerPush();
     if (a.tn <= 0) return HISQ_OK;
     int cap = h->nrhs_inner > 0 ? h->nrhs_inner : default_inner_cap((int)sizeof(T));
     int e = launch_dslash<T>(a, mode, nrhs, cap, h->stream, &h->stats);
@@ -784,6 +793,8 @@ extern "C" int hisq_cg_multishift(hisq_ctx* h, void* x, const void* b, double ma
     return ms_solve<double>(h, h->links64, (double*)x, (const double*)b, mass, shifts, nshift, tol);
 }
 
+static int cgp_solve(hisq_ctx* h, void* x, const void* b, double mass, double tol, int nrhs);
+
 extern "C" int hisq_cg(hisq_ctx* h, void* x, const void* b, double mass, double tol, int nrhs)
 {
     if (!h || !x || !b || nrhs < 1 || nrhs > HISQ_MAX_NRHS || !(tol > 0.0) || !std::isfinite(mass)) return HISQ_EINVAL;
@@ -791,9 +802,9 @@ extern "C" int hisq_cg(hisq_ctx* h, void* x, const void* b, double mass, double 
     if (!h->ws) return HISQ_ENOWORKSPACE;
     if (nrhs > h->ws_nrhs) return HISQ_ENOWORKSPACE;
     if (!h->have_links) return HISQ_ENOLINKS;
-    if (h->g.part) return HISQ_EINVAL;   // the solvers need a cross-rank reduction: not built
     const size_t bytes = (size_t)nrhs * 6 * h->g.Vh * elem_size(h->prec);
     if (overlap(x, b, bytes)) return HISQ_EINVAL;
+    if (h->g.part) return cgp_solve(h, x, b, mass, tol, nrhs);   // across ranks: needs the peer mailboxes
     if (h->prec == HISQ_FP32) return cg_solve<float, float>(h, h->links32, nullptr, (float*)x, (const float*)b, mass, tol, nrhs);
     if (h->prec == HISQ_FP64) return cg_solve<double, double>(h, h->links64, nullptr, (double*)x, (const double*)b, mass, tol, nrhs);
     return cg_solve<float, double>(h, h->links32, h->links64, (double*)x, (const double*)b, mass, tol, nrhs);
@@ -811,6 +822,7 @@ extern "C" int hisq_set_option(hisq_ctx* h, const char* key, double value)
     else if (!strcmp(key, "nrhs_inner")) { if (v < 0 || v > 8) return HISQ_EINVAL; h->nrhs_inner = v; }
     else if (!strcmp(key, "naik_compress")) h->naik_compress = v != 0;
     else if (!strcmp(key, "fused_blas")) h->fused_blas = v != 0;
+    else if (!strcmp(key, "overlap")) { if (v < -1 || v > 1) return HISQ_EINVAL; h->overlap_opt = v; }
     else if (!strcmp(key, "tile_y")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[1] % v))) return HISQ_EINVAL; h->tile_y = v; }
     else if (!strcmp(key, "tile_z")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[2] % v))) return HISQ_EINVAL; h->tile_z = v; }
     else if (!strcmp(key, "window_mb")) { if (!(value > 0)) return HISQ_EINVAL; h->window_mb = value; }
@@ -964,11 +976,11 @@ static int cgp_phase(hisq_ctx* h, const T* links, int phase, double mass)
         return HISQ_OK;
     }
     case 4:
-        cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial, 1);
+        cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial, 1, h->fuse_push_sums, h->fuse_red_pq);
         h->stats.launches++;
         break;
     case 5:  // after the all-reduce of sums (= ||r||^2)
-        cgp_finalize_xr_kernel<<<1, 1, 0, h->stream>>>(h->state, nrhs);
+        cgp_finalize_xr_kernel<<<1, 1, 0, h->stream>>>(h->state, nrhs, h->fuse_red_sums, h->part_nranks);
         h->stats.launches++;
         break;
     default: return HISQ_EINVAL;
@@ -1026,17 +1038,19 @@ extern "C" size_t hisq_halo_bytes(const hisq_ctx* h, int nrhs)
 }
 
 template <bool PACK>
-static int halo_move(hisq_ctx* h, void* field, void* lo, void* hi, int nrhs)
+static int halo_move(hisq_ctx* h, void* field, void* lo, void* hi, int nrhs, unsigned* sig_a = nullptr, unsigned* sig_b = nullptr)
 {
     if (!h || !field || !lo || !hi || nrhs < 1 || nrhs > HISQ_MAX_NRHS || !h->g.part) return HISQ_EINVAL;
+    if (!h->ws) return HISQ_ENOWORKSPACE;
     const int S = h->g.Vh / h->g.L[3];
     const size_t total = (size_t)nrhs * 3 * kHopMax * S;
     unsigned grid = (unsigned)((total + 255) / 256);
-    if (grid > 148 * 8) grid = 148 * 8;
+    if (grid > 148 * 4) grid = 148 * 4;
+    unsigned* ticket = &h->state->ticket[3];
     if (h->prec == HISQ_FP32)
-        halo_kernel<float, PACK><<<grid, 256, 0, h->stream>>>((float*)field, (float*)lo, (float*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHopMax, nrhs);
+        halo_kernel<float, PACK><<<grid, 256, 0, h->stream>>>((float*)field, (float*)lo, (float*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHopMax, nrhs, ticket, sig_a, sig_b);
     else
-        halo_kernel<double, PACK><<<grid, 256, 0, h->stream>>>((double*)field, (double*)lo, (double*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHopMax, nrhs);
+        halo_kernel<double, PACK><<<grid, 256, 0, h->stream>>>((double*)field, (double*)lo, (double*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHopMax, nrhs, ticket, sig_a, sig_b);
     h->stats.launches++;
     CK(cudaGetLastError());
     return HISQ_OK;
@@ -1051,42 +1065,61 @@ extern "C" int hisq_halo_unpack(hisq_ctx* h, void* field, const void* recv_lo, c
 }
 
 // ---- halo transport through peer-mapped memory (no library collective) ----------------------------------------
-// Mailbox = [16 flags (u32), 256 B][slot 0: lo, hi][slot 1: lo, hi].  Flags, all exchange numbers e = 1, 2, ...:
-//   ready_lo[s] (0+s): my lower-halo buffer of slot s holds exchange e      (written by the previous rank)
-//   ready_hi[s] (2+s): my upper-halo buffer of slot s holds exchange e      (written by the next rank)
-//   free_up[s]  (4+s): the next rank has unpacked what I put in ITS lo buffer of slot s for exchange e
-//   free_down[s](6+s): the previous rank has unpacked what I put in ITS hi buffer of slot s
-// Waiting and signalling are stream memory operations (cuStreamWaitValue32 / cuStreamWriteValue32): no kernel spins.
+// Mailbox = [16 counters (u32), 256 B][reduce data: [2 slots][16 ranks][16] doubles][slot 0: lo, hi][slot 1: lo, hi].
+// Counters 0, 1: halo arrivals of the two slots (each exchange adds 2: one per neighbour); 8, 9: reduce arrivals (each
+// reduce adds nranks).  The SENDING kernels bump them with system-scope atomics after fencing their stores; the receiver
+// waits with a stream memory operation (cuStreamWaitValue32): no kernel spins.
+// Why two slots and no "free" credits: every rank alternates send e, recv e, send e+1, ...  A rank's send e+2 follows
+// its recv e+1 in stream order, which completes only after BOTH neighbours' send e+1, each of which follows that
+// neighbour's recv e (unpack finished) in its own stream order: the slot of exchange e has been read before it is
+// written again.
 static const size_t kMboxFlags = 256;
+static const size_t kMboxReduce = (size_t)2 * kMaxRanks * kMaxNrhs * sizeof(double);
 typedef CUresult (*StreamMemOp32)(CUstream, CUdeviceptr, cuuint32_t, unsigned int);
-static StreamMemOp32 g_wait32 = nullptr, g_write32 = nullptr;
+static StreamMemOp32 g_wait32 = nullptr;
 static bool load_memops()
 {
-    if (g_wait32 && g_write32) return true;
-    void *w = nullptr, *r = nullptr;
+    if (g_wait32) return true;
+    void* w = nullptr;
     cudaDriverEntryPointQueryResult q;
     if (cudaGetDriverEntryPoint("cuStreamWaitValue32", &w, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) return false;
-    if (cudaGetDriverEntryPoint("cuStreamWriteValue32", &r, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) return false;
-    g_wait32 = (StreamMemOp32)w; g_write32 = (StreamMemOp32)r;
+    g_wait32 = (StreamMemOp32)w;
     return true;
 }
-static char* mbox_buffer(char* box, size_t buf, int slot, int hi) { return box + kMboxFlags + (size_t)(2 * slot + hi) * buf; }
-static CUdeviceptr mbox_flag(char* box, int which, int slot) { return (CUdeviceptr)(uintptr_t)(box + 4 * (which * 2 + slot)); }
+static CUresult stream_wait_geq(hisq_ctx* h, const void* counter, unsigned value)
+{
+#ifdef HISQ_DEBUG_NOWAIT   // timing experiment only (single rank: stream order already guarantees the arrival)
+    (void)h; (void)counter; (void)value;
+    return CUDA_SUCCESS;
+#else
+    return g_wait32((CUstream)h->stream, (CUdeviceptr)(uintptr_t)counter, value, CU_STREAM_WAIT_VALUE_GEQ);
+#endif
+}
+static char* mbox_buffer(char* box, size_t buf, int slot, int hi) { return box + kMboxFlags + kMboxReduce + (size_t)(2 * slot + hi) * buf; }
+static unsigned* mbox_counter(char* box, int slot) { return reinterpret_cast<unsigned*>(box) + slot; }
 
 extern "C" size_t hisq_peer_bytes(const hisq_ctx* h, int nrhs)
 {
     const size_t b = hisq_halo_bytes(h, nrhs);
-    return b ? kMboxFlags + 4 * align_up(b) : 0;
+    return b ? kMboxFlags + kMboxReduce + 4 * align_up(b) : 0;
 }
-extern "C" int hisq_peer_attach(hisq_ctx* h, void* mine, void* up, void* down, int nrhs)
+extern "C" int hisq_peer_attach(hisq_ctx* h, void* const* boxes, int nboxes, int nrhs)
 {
-    if (!h || !h->g.part || !mine || !up || !down || nrhs < 1 || nrhs > HISQ_MAX_NRHS) return HISQ_EINVAL;
-    if (((uintptr_t)mine & 255) || ((uintptr_t)up & 255) || ((uintptr_t)down & 255)) return HISQ_EINVAL;
+    if (!h || !h->g.part || !boxes || nrhs < 1 || nrhs > HISQ_MAX_NRHS) return HISQ_EINVAL;
+    if (nboxes != h->part_nranks || nboxes > kMaxRanks) return HISQ_EINVAL;
+    for (int r = 0; r < nboxes; ++r)
+        if (!boxes[r] || ((uintptr_t)boxes[r] & 255)) return HISQ_EINVAL;
     if (!load_memops()) { h->last_error = "stream memory operations (cuStreamWaitValue32) are not available"; return HISQ_ECUDA; }
-    h->mbox = (char*)mine; h->mbox_up = (char*)up; h->mbox_down = (char*)down;
+    for (int r = 0; r < kMaxRanks; ++r) h->mbox_all.box[r] = r < nboxes ? (char*)boxes[r] : nullptr;
+    h->mbox = (char*)boxes[h->part_rank];
+    h->mbox_up = (char*)boxes[(h->part_rank + 1) % nboxes];
+    h->mbox_down = (char*)boxes[(h->part_rank + nboxes - 1) % nboxes];
     h->mbox_buf = align_up(hisq_halo_bytes(h, nrhs));
     h->mbox_nrhs = nrhs;
-    h->seq_send = h->seq_recv = 0;
+    h->seq_send = h->seq_recv = h->red_send = h->red_recv = 0;
+    if (!h->d_boxes) CK(cudaMalloc(&h->d_boxes, sizeof(PeerBoxes)));
+    CK(cudaMemcpyAsync(h->d_boxes, &h->mbox_all, sizeof(PeerBoxes), cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
     return HISQ_OK;
 }
 #define CKU(call)                                                                                         \
@@ -1097,36 +1130,141 @@ extern "C" int hisq_peer_attach(hisq_ctx* h, void* mine, void* up, void* down, i
 extern "C" int hisq_halo_send(hisq_ctx* h, const void* field, int nrhs)
 {
     if (!h || !field || !h->mbox || nrhs < 1 || nrhs > h->mbox_nrhs) return HISQ_EINVAL;
-    const unsigned e = ++h->seq_send;
+    if (h->seq_send != h->seq_recv) return HISQ_EINVAL;   // strict alternation send / recv (see the slot argument above)
+    const unsigned e = h->seq_send + 1;
     const int s = (int)(e & 1u);
-    CUstream st = (CUstream)h->stream;
-    if (e > 2) {   // the buffers of this slot were last used by exchange e - 2: both neighbours must have unpacked them
-        CKU(g_wait32(st, mbox_flag(h->mbox, 2, s), e - 2, CU_STREAM_WAIT_VALUE_GEQ));
-        CKU(g_wait32(st, mbox_flag(h->mbox, 3, s), e - 2, CU_STREAM_WAIT_VALUE_GEQ));
-    }
     // my lowest slices -> the previous rank's UPPER halo buffer, my highest -> the next rank's LOWER halo buffer
     int rc = halo_move<true>(h, const_cast<void*>(field), mbox_buffer(h->mbox_down, h->mbox_buf, s, 1),
-                             mbox_buffer(h->mbox_up, h->mbox_buf, s, 0), nrhs);
+                             mbox_buffer(h->mbox_up, h->mbox_buf, s, 0), nrhs, mbox_counter(h->mbox_down, s),
+                             mbox_counter(h->mbox_up, s));
     if (rc) return rc;
-    CKU(g_write32(st, mbox_flag(h->mbox_up, 0, s), e, CU_STREAM_WRITE_VALUE_DEFAULT));
-    CKU(g_write32(st, mbox_flag(h->mbox_down, 1, s), e, CU_STREAM_WRITE_VALUE_DEFAULT));
+    h->seq_send = e;
     return HISQ_OK;
 }
 extern "C" int hisq_halo_recv(hisq_ctx* h, void* field, int nrhs)
 {
     if (!h || !field || !h->mbox || nrhs < 1 || nrhs > h->mbox_nrhs) return HISQ_EINVAL;
-    if (h->seq_recv >= h->seq_send) return HISQ_EINVAL;   // nothing sent for this exchange: the neighbours would wait for ever
-    const unsigned e = ++h->seq_recv;
+    if (h->seq_recv + 1 != h->seq_send) return HISQ_EINVAL;   // nothing sent for this exchange: the neighbours would wait for ever
+    const unsigned e = h->seq_recv + 1;
     const int s = (int)(e & 1u);
-    CUstream st = (CUstream)h->stream;
-    CKU(g_wait32(st, mbox_flag(h->mbox, 0, s), e, CU_STREAM_WAIT_VALUE_GEQ));
-    CKU(g_wait32(st, mbox_flag(h->mbox, 1, s), e, CU_STREAM_WAIT_VALUE_GEQ));
+    const unsigned uses = (e + 1) >> 1;   // how often this slot has been used, this exchange included
+    CKU(stream_wait_geq(h, mbox_counter(h->mbox, s), 2u * uses));
     int rc = halo_move<false>(h, field, mbox_buffer(h->mbox, h->mbox_buf, s, 0), mbox_buffer(h->mbox, h->mbox_buf, s, 1), nrhs);
     if (rc) return rc;
-    // I am the previous rank's "up" neighbour and the next rank's "down" neighbour
-    CKU(g_write32(st, mbox_flag(h->mbox_down, 2, s), e, CU_STREAM_WRITE_VALUE_DEFAULT));
-    CKU(g_write32(st, mbox_flag(h->mbox_up, 3, s), e, CU_STREAM_WRITE_VALUE_DEFAULT));
+    h->seq_recv = e;
     return HISQ_OK;
+}
+
+static double* state_array(hisq_ctx* h, int which)
+{
+    switch (which) {
+    case 2: return h->state->rho;
+    case 3: return h->state->pq;
+    case 4: return h->state->sums;
+    default: return nullptr;
+    }
+}
+// Reduce number e uses slot e & 1.  A slot is written again two reduces later; by then every rank has finished reduce
+// e + 1, which needed every rank's contribution, sent after that rank had summed reduce e: no credit flags are needed.
+extern "C" int hisq_peer_reduce_send(hisq_ctx* h, int which, int nrhs)
+{
+    if (!h || !h->mbox || !h->ws || nrhs < 1 || nrhs > kMaxNrhs || !state_array(h, which)) return HISQ_EINVAL;
+    if (h->red_send != h->red_recv) return HISQ_EINVAL;   // one reduce in flight at a time (the slot argument above)
+    const unsigned e = ++h->red_send;
+    peer_reduce_send_kernel<<<h->part_nranks, 32, 0, h->stream>>>(state_array(h, which), h->mbox_all, h->part_rank, (int)(e & 1u), nrhs,
+                                                                  kMboxFlags, kMboxCounterOff);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+extern "C" int hisq_peer_reduce_recv(hisq_ctx* h, int which, int nrhs)
+{
+    if (!h || !h->mbox || !h->ws || nrhs < 1 || nrhs > kMaxNrhs || !state_array(h, which)) return HISQ_EINVAL;
+    if (h->red_recv + 1 != h->red_send) return HISQ_EINVAL;
+    const unsigned e = ++h->red_recv;
+    const int s = (int)(e & 1u);
+    const unsigned uses = (e + 1) >> 1;   // how often this slot has been used, this reduce included
+    CKU(stream_wait_geq(h, h->mbox + kMboxCounterOff + 4 * s, uses * (unsigned)h->part_nranks));
+    peer_reduce_sum_kernel<<<1, 32, 0, h->stream>>>(state_array(h, which), h->mbox, h->part_nranks, s, nrhs, kMboxFlags);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+
+// Fused form of hisq_peer_reduce_send / recv: the producing kernel's last block pushes (PeerPush), the stream waits,
+// the consuming kernels read the slot.  Same counters and slots as the stand-alone calls.
+static PeerPush reduce_next_push(hisq_ctx* h)
+{
+    const unsigned e = ++h->red_send;
+    PeerPush pp;
+    pp.boxes = h->d_boxes; pp.nranks = h->part_nranks; pp.rank = h->part_rank; pp.slot = (int)(e & 1u);
+    return pp;
+}
+static const double* reduce_wait(hisq_ctx* h, int& rc)
+{
+    const unsigned e = ++h->red_recv;
+    const int s = (int)(e & 1u);
+    const unsigned uses = (e + 1) >> 1;
+    CUresult r = stream_wait_geq(h, h->mbox + kMboxCounterOff + 4 * s, uses * (unsigned)h->part_nranks);
+    rc = HISQ_OK;
+    if (r != CUDA_SUCCESS) { h->last_error = "cuStreamWaitValue32: CUresult " + std::to_string((int)r); rc = HISQ_ECUDA; }
+    return reinterpret_cast<const double*>(h->mbox + kMboxFlags) + (size_t)s * kMaxRanks * kMaxNrhs;
+}
+struct FuseGuard {   // the fused pointers never outlive the solve
+    hisq_ctx* h;
+    ~FuseGuard() { h->fuse_push_pq = h->fuse_push_sums = PeerPush(); h->fuse_red_pq = h->fuse_red_sums = nullptr; }
+};
+
+// hisq_cg on a partitioned context: the phase-wise iteration with every cross-rank step done through the mailboxes, all
+// on the stream -- the host only polls the state every check_interval iterations.  The all-reduce gives every rank the
+// same bits, so all ranks take the same decisions (stop, breakdown, iteration count) and issue the same calls.
+static int cgp_solve(hisq_ctx* h, void* x, const void* b, double mass, double tol, int nrhs)
+{
+    if (h->prec == HISQ_MIXED || !h->mbox || nrhs > h->mbox_nrhs) return HISQ_EINVAL;
+    int rc = hisq_cgp_begin(h, x, b, tol, nrhs);
+    if (rc) return rc;
+    if ((rc = hisq_peer_reduce_send(h, 2, nrhs)) || (rc = hisq_peer_reduce_recv(h, 2, nrhs)) || (rc = hisq_cgp_phase(h, 0, mass))) return rc;
+    void* p = hisq_cgp_ptr(h, 0);
+    void* t = hisq_cgp_ptr(h, 1);
+    h->info_reliable = 0;
+    FuseGuard guard{ h };
+    // splitting a Dslash costs a launch tail and some L2 reuse: do it when at least half of the owned
+    // slices can run under the transfer, or when asked to (option "overlap": -1 auto, 0 never, 1 always)
+    const bool split = h->overlap_opt < 0 ? h->g.t_cnt >= 4 * kHopMax : h->overlap_opt != 0;
+    for (;;) {
+        if ((rc = poll_state(h))) return rc;
+        const CgState s = *h->host_state;
+        if (s.done || s.breakdown || s.iter >= h->max_iter) {
+            h->info_iters = s.iter;
+            for (int k = 0; k < nrhs; ++k) h->info_relres[k] = s.bnorm2[k] > 0.0 ? std::sqrt(s.rho[k] / s.bnorm2[k]) : 0.0;
+            if (s.breakdown) return HISQ_EBREAKDOWN;
+            int any = 0;      // done is also raised at max_iter: converged = no system left active
+            for (int k = 0; k < nrhs; ++k) any |= s.active[k];
+            return any ? HISQ_ENOCONV : HISQ_OK;
+        }
+        for (int i = 0; i < h->check_interval; ++i) {
+            if ((rc = hisq_cgp_phase(h, 1, mass))) return rc;
+            // the kernels that produce <p,q> and ||r||^2 push them to all ranks themselves, those that consume them add up
+            // the mailbox entries themselves: no reduction kernel, one stream wait per all-reduce
+            h->fuse_push_pq = reduce_next_push(h);
+            if (split) {   // interior slices while the halo is in flight, edge slices once it has arrived
+                if ((rc = hisq_halo_send(h, p, nrhs)) || (rc = hisq_cgp_phase(h, 20, mass))) return rc;
+                if ((rc = hisq_halo_recv(h, p, nrhs)) || (rc = hisq_cgp_phase(h, 21, mass))) return rc;
+                if ((rc = hisq_halo_send(h, t, nrhs)) || (rc = hisq_cgp_phase(h, 30, mass))) return rc;
+                if ((rc = hisq_halo_recv(h, t, nrhs)) || (rc = hisq_cgp_phase(h, 31, mass))) return rc;
+            } else {
+                if ((rc = hisq_halo_send(h, p, nrhs)) || (rc = hisq_halo_recv(h, p, nrhs)) || (rc = hisq_cgp_phase(h, 2, mass))) return rc;
+                if ((rc = hisq_halo_send(h, t, nrhs)) || (rc = hisq_halo_recv(h, t, nrhs)) || (rc = hisq_cgp_phase(h, 3, mass))) return rc;
+            }
+            h->fuse_red_pq = reduce_wait(h, rc);            // <p,q> of all ranks have arrived
+            if (rc) return rc;
+            h->fuse_push_sums = reduce_next_push(h);
+            if ((rc = hisq_cgp_phase(h, 4, mass))) return rc;
+            h->fuse_red_sums = reduce_wait(h, rc);          // ||r||^2 of all ranks have arrived
+            if (rc) return rc;
+            if ((rc = hisq_cgp_phase(h, 5, mass))) return rc;
+        }
+    }
 }
 
 extern "C" int hisq_naik_compressed(const hisq_ctx* h) { return h && h->naik_c13 ? 1 : 0; }

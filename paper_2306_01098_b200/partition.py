@@ -149,27 +149,26 @@ class PeerHalo:
     stores straight into the neighbours' memory over NVLink and stream memory operations do the signalling -- no
     communication-library call on the data path.  This class is the plumbing: it allocates this rank's mailbox,
     hands a CUDA IPC mapping of it to the other ranks of the node (through `dist`'s object collectives; one process per
-    GPU) and attaches the neighbours' mappings to the context.  dist = None or one rank: the ring closes on itself."""
+    GPU) and attaches all ranks' mappings to the context (t-neighbours for the halos, everybody for the all-reduce).  dist = None or one rank: the ring closes on itself."""
 
     def __init__(self, ctx, rank: int, nranks: int, nrhs: int, dist=None):
         self.ctx, self.dist, self.nranks = ctx, dist, nranks
         self.mine = ctx.peer_mailbox(nrhs)
         torch.cuda.synchronize(ctx.device)          # zeroed before anybody can see it
-        if nranks == 1 or dist is None:
-            up = down = self.mine
-        else:
+        boxes = [self.mine] * nranks
+        if nranks > 1 and dist is not None:
             from torch.multiprocessing.reductions import reduce_tensor
             shared = [None] * nranks
             dist.all_gather_object(shared, reduce_tensor(self.mine))
-            boxes = {}
-            for r in {(rank + 1) % nranks, (rank - 1) % nranks}:
+            for r in range(nranks):
+                if r == rank:
+                    continue
                 rebuild, args = shared[r]
                 boxes[r] = rebuild(*args)
                 if boxes[r].device != ctx.device:
                     # a first copy makes torch enable peer access from this GPU to the owner's (kernels need it too)
                     torch.empty(1, dtype=torch.uint8, device=ctx.device).copy_(boxes[r][:1])
-            up, down = boxes[(rank + 1) % nranks], boxes[(rank - 1) % nranks]
-        ctx.peer_attach(self.mine, up, down, nrhs)
+        ctx.peer_attach(boxes, nrhs)
         self._barrier()
 
     def _barrier(self):
@@ -182,6 +181,11 @@ class PeerHalo:
 
     def recv(self, field):
         self.ctx.halo_recv(field)
+
+    def allreduce(self, which: int, nrhs: int):
+        """Sum over ranks of a CG state array (hisq_cgp_ptr numbering), in place, on the context's stream."""
+        self.ctx.peer_reduce_send(which, nrhs)
+        self.ctx.peer_reduce_recv(which, nrhs)
 
     def close(self):
         """Collective: nobody frees a mailbox a neighbour may still be writing to."""
@@ -196,8 +200,9 @@ class PartitionedCG:
     exchange of a field and all-reduce of nrhs doubles -- through `dist` (torch.distributed: NCCL between GPUs)."""
 
     def __init__(self, ctx, rank: int, nranks: int, dist=None, peer: "PeerHalo | None" = None):
-        """peer: move the halos through peer-mapped mailboxes (PeerHalo) instead of `dist` send / recv; the all-reduces
-        of the scalar products still go through `dist`."""
+        """peer: move the halos AND the all-reduces of the scalar products through peer-mapped mailboxes (PeerHalo)
+        instead of `dist`: the iteration then runs without a communication-library call and without a host sync
+        between status polls."""
         self.ctx, self.rank, self.nranks, self.dist, self.peer = ctx, rank, nranks, dist, peer
 
     def _halo_begin(self, field):
@@ -218,8 +223,10 @@ class PartitionedCG:
         ex.finish()
         self.ctx.halo_unpack(field, rlo, rhi)
 
-    def _allreduce(self, t):
-        if self.dist is not None and self.nranks > 1:
+    def _allreduce(self, t, which=None):
+        if self.peer is not None and which is not None:
+            self.peer.allreduce(which, t.shape[0])
+        elif self.dist is not None and self.nranks > 1:
             if t.is_cuda and self.dist.get_backend() != "nccl":
                 h = t.cpu()
                 self.dist.all_reduce(h, op=self.dist.ReduceOp.SUM)
@@ -238,7 +245,7 @@ class PartitionedCG:
         p, t = c.cgp_tensor(0, n), c.cgp_tensor(1, n)
         rho, pq, sums = c.cgp_tensor(2, n), c.cgp_tensor(3, n), c.cgp_tensor(4, n)
         c.cgp_begin(x, b, tol)
-        self._allreduce(rho)
+        self._allreduce(rho, 2)
         c.cgp_phase(0, mass)
         st = c.cgp_status(n)
         while not st["done"] and st["iterations"] < max_iter:
@@ -260,9 +267,9 @@ class PartitionedCG:
                 else:
                     self._halo_end(t, pend)
                     c.cgp_phase(3, mass)
-                self._allreduce(pq)
+                self._allreduce(pq, 3)
                 c.cgp_phase(4, mass)
-                self._allreduce(sums)
+                self._allreduce(sums, 4)
                 c.cgp_phase(5, mass)
             st = c.cgp_status(n)
         return x, st

@@ -31,7 +31,7 @@ def _run(L, prec, nranks, nrhs, parity, seed, overlap=False, peer=False):
         # mailboxes in the one process: plain device pointers.  All sends are enqueued before any recv (one stream).
         boxes = [c.peer_mailbox(nrhs) for c in ctxs]
         for r, c in enumerate(ctxs):
-            c.peer_attach(boxes[r], boxes[(r + 1) % nranks], boxes[(r - 1) % nranks], nrhs)
+            c.peer_attach(boxes, nrhs)
         for c, f in zip(ctxs, fields):
             c.halo_send(f)
     outs = []
@@ -169,15 +169,21 @@ def _emulated_cg(L, prec, nranks, nrhs, m, tol, seed, overlap=False, peer=False)
         ctxs.append(ctx); bs.append(b); xs.append(x)
 
     def allreduce(which):
+        if peer:      # every rank stores into every mailbox, then every rank sums in rank order
+            for c in ctxs: c.peer_reduce_send(which, nrhs)
+            for c in ctxs: c.peer_reduce_recv(which, nrhs)
+            return
         ts = [c.cgp_tensor(which, nrhs) for c in ctxs]
-        tot = torch.stack(ts).sum(0)
+        tot = ts[0].clone()
+        for t in ts[1:]:      # rank order, as the mailbox all-reduce adds
+            tot += t
         for t in ts:
             t.copy_(tot)
 
     if peer:
         boxes = [c.peer_mailbox(nrhs) for c in ctxs]
         for r, c in enumerate(ctxs):
-            c.peer_attach(boxes[r], boxes[(r + 1) % nranks], boxes[(r - 1) % nranks], nrhs)
+            c.peer_attach(boxes, nrhs)
 
     def halo(which, between=None):
         fields = [c.cgp_tensor(which, nrhs) for c in ctxs]
@@ -279,6 +285,38 @@ def test_partitioned_cg_driver_single_rank_equals_hisq_cg():
     ctx.close(); ref.close()
 
 
+def test_hisq_cg_on_a_partitioned_context_single_rank_ring():
+    """hisq_cg itself on a partitioned context (mailboxes attached; one rank, the ring closes on itself): the whole
+    iteration, halos and all-reduces included, runs on the stream.  Against hisq_cg on the plain lattice."""
+    L, m, tol, seed, n = (4, 4, 6, 12), 0.2, 1e-10, 16, 3
+    dev = torch.device("cuda:0")
+    ctx = binding.Hisq(L, "fp64", n, dev, part=(0, 1))
+    fat, naik = partition.make_links_part(L, seed, 0, 1, dev)
+    ctx.set_links(fat, naik)
+    b = ctx.pack(partition.make_sources_part(L, seed + 1, n, 0, 0, 1, dev))
+    with pytest.raises(binding.HisqError):
+        ctx.cg(b, m, tol)                         # no mailboxes yet
+    peer = partition.PeerHalo(ctx, 0, 1, n)
+    x, info = ctx.cg(b, m, tol)
+    assert max(info["true_rel_resid"]) <= tol
+    ref = binding.Hisq(L, "fp64", n, dev)
+    f2, n2 = binding.make_links(L, seed, dev)
+    ref.set_links(f2, n2)
+    xr, iref = ref.cg(ref.pack(binding.make_sources(L, seed + 1, n, 0, dev)), m, tol)
+    Le = partition.extended_lattice(L, 1)
+    S = ctx.Vh // Le[3]
+    xi = ctx.unpack(x).view(n, Le[3], S, 3)[:, partition.HALO_T:Le[3] - partition.HALO_T].reshape(n, -1, 3)
+    assert rel_l2(xi.cpu().numpy(), ref.unpack(xr).cpu().numpy()) <= 1e-9
+    assert abs(info["iterations"] - iref["iterations"]) <= 32 + 2          # polled every check_interval iterations
+    # max_iter on the partitioned path: not converged is reported as such
+    ctx.set_option("max_iter", 3)
+    with pytest.raises(binding.HisqError) as e:
+        ctx.cg(b, m, 1e-14)
+    assert e.value.code == -5
+    peer.close()
+    ctx.close(); ref.close()
+
+
 def _mp_worker(rank, world, port, L, m, tol, seed, q, transport):
     import os, sys
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
@@ -289,8 +327,12 @@ def _mp_worker(rank, world, port, L, m, tol, seed, q, transport):
     fat, naik = partition.make_links_part(L, seed, rank, world, dev)
     ctx.set_links(fat, naik)
     b = ctx.pack(partition.make_sources_part(L, seed + 1, 1, 0, rank, world, dev))
-    peer = partition.PeerHalo(ctx, rank, world, 1, dist) if transport == "peer" else None
-    x, st = partition.PartitionedCG(ctx, rank, world, dist, peer=peer).solve(b, m, tol, check_every=8)
+    peer = partition.PeerHalo(ctx, rank, world, 1, dist) if transport != "dist" else None
+    if transport == "native":      # hisq_cg drives the iteration itself: no torch.distributed call inside the solve
+        x, info = ctx.cg(b, m, tol)
+        st = dict(done=info["status"] == 0, breakdown=False, iterations=info["iterations"])
+    else:
+        x, st = partition.PartitionedCG(ctx, rank, world, dist, peer=peer).solve(b, m, tol, check_every=8)
     if peer is not None:
         peer.close()
     Le = partition.extended_lattice(L, world)
@@ -306,7 +348,7 @@ def _mp_worker(rank, world, port, L, m, tol, seed, q, transport):
     dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("transport", ["dist", "peer"])
+@pytest.mark.parametrize("transport", ["dist", "peer", "native"])
 def test_partitioned_cg_two_processes_gloo_on_one_gpu(transport):
     """The real thing minus the second GPU: two PROCESSES, each with its own context, exchanging halos and all-reducing
     through torch.distributed (gloo here, NCCL between GPUs), run partition.PartitionedCG.solve.
@@ -317,7 +359,7 @@ def test_partitioned_cg_two_processes_gloo_on_one_gpu(transport):
     L, m, tol, seed, world = (4, 4, 6, 16), 0.15, 1e-9, 8, 2
     ctxmp = mp.get_context("spawn")
     q = ctxmp.Queue()
-    port = 33500 + __import__("os").getpid() % 2000 + (17 if transport == "peer" else 0)
+    port = 33500 + __import__("os").getpid() % 2000 + {"dist": 0, "peer": 17, "native": 31}[transport]
     ps = [ctxmp.Process(target=_mp_worker, args=(r, world, port, L, m, tol, seed, q, transport)) for r in range(world)]
     for p in ps:
         p.start()
