@@ -148,8 +148,9 @@ int hisq_cg_host(hisq_ctx *h, void *x_host, const void *b_host, double mass, dou
  * antiperiodic sign only on the ranks that own the global t boundary.  Halo slices of `out` are left untouched.
  * Lt_loc must be even and >= 4.  hisq_cg on a partitioned context (fp32 or fp64) solves across the ranks once the peer
  * mailboxes are attached (hisq_peer_attach, below; HISQ_EINVAL before): every rank calls it with its slab of b and
- * gets its slab of x; same arithmetic and stopping rule as on one GPU except that the final true-residual check is
- * left out (hisq_get_info reports the recursive residuals).  hisq_cg_multishift and HISQ_MIXED: HISQ_EINVAL. */
+ * gets its slab of x (halo slices of x are overwritten); same arithmetic and stopping rule as on one GPU, including
+ * the true-residual confirmation b - A x (over all ranks) and the resume if it fails; hisq_get_info reports the
+ * global true residuals, identical on every rank.  hisq_cg_multishift and HISQ_MIXED: HISQ_EINVAL. */
 int hisq_create_part(hisq_ctx **h, int Lx, int Ly, int Lz, int Lt_global, int prec, int rank, int nranks);
 /* hisq_dslash restricted to the OWNED time slices [t_first, t_first + t_count) (0 <= t_first, t_first + t_count <= the
  * number of owned slices: Lt_loc on a partitioned context, Lt otherwise); all other slices of `out` are left untouched.

@@ -1215,6 +1215,29 @@ struct FuseGuard {   // the fused pointers never outlive the solve
     ~FuseGuard() { h->fuse_push_pq = h->fuse_push_sums = PeerPush(); h->fuse_red_pq = h->fuse_red_sums = nullptr; }
 };
 
+// r := b - A x over all ranks, sums := global ||r_k||^2, then the reliable-update bookkeeping (rho := true value, systems
+// above tol become active again, done re-evaluated).  Stand-alone reduce kernels: this runs once or twice per solve.
+template <typename T>
+static int cgp_true_residual_t(hisq_ctx* h, const T* links, T* x, const T* b, double mass, int nrhs)
+{
+    CgpFields f = cgp_fields(h);
+    int rc;
+    if ((rc = hisq_halo_send(h, x, nrhs)) || (rc = hisq_halo_recv(h, x, nrhs))) return rc;
+    if ((rc = run_dslash<T>(h, links, (T*)f.t, x, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, nullptr, 2))) return rc;
+    if ((rc = hisq_halo_send(h, f.t, nrhs)) || (rc = hisq_halo_recv(h, f.t, nrhs))) return rc;
+    if ((rc = run_dslash<T>(h, links, (T*)f.r, (const T*)f.t, HISQ_EVEN, nrhs, MODE_RESID, x, b, mass * mass, h->state->sums, nullptr, 2))) return rc;
+    if ((rc = hisq_peer_reduce_send(h, 4, nrhs)) || (rc = hisq_peer_reduce_recv(h, 4, nrhs))) return rc;
+    cg_after_residual_kernel<<<1, 1, 0, h->stream>>>(h->state, h->true_rr);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+static int cgp_true_residual(hisq_ctx* h, void* x, const void* b, double mass, int nrhs)
+{
+    return h->prec == HISQ_FP32 ? cgp_true_residual_t<float>(h, h->links32, (float*)x, (const float*)b, mass, nrhs)
+                                : cgp_true_residual_t<double>(h, h->links64, (double*)x, (const double*)b, mass, nrhs);
+}
+
 // hisq_cg on a partitioned context: the phase-wise iteration with every cross-rank step done through the mailboxes, all
 // on the stream -- the host only polls the state every check_interval iterations.  The all-reduce gives every rank the
 // same bits, so all ranks take the same decisions (stop, breakdown, iteration count) and issue the same calls.
@@ -1231,9 +1254,25 @@ static int cgp_solve(hisq_ctx* h, void* x, const void* b, double mass, double to
     // splitting a Dslash costs a launch tail and some L2 reuse: do it when at least half of the owned
     // slices can run under the transfer, or when asked to (option "overlap": -1 auto, 0 never, 1 always)
     const bool split = h->overlap_opt < 0 ? h->g.t_cnt >= 4 * kHopMax : h->overlap_opt != 0;
+    int confirms = 0;
     for (;;) {
         if ((rc = poll_state(h))) return rc;
-        const CgState s = *h->host_state;
+        CgState s = *h->host_state;
+        if (s.done && !s.breakdown && s.iter < h->max_iter) {
+            if (confirms >= 8) {   // the recursive residual keeps converging, the true one does not: below the attainable accuracy
+                h->info_iters = s.iter;
+                for (int k = 0; k < nrhs; ++k) h->info_relres[k] = s.bnorm2[k] > 0.0 ? std::sqrt(((const double*)((const char*)h->host_state + sizeof(CgState)))[k] / s.bnorm2[k]) : 0.0;
+                return HISQ_ENOCONV;
+            }
+            // converged by the recursive residual: confirm with r = b - A x across the ranks (halo of x, of D_oe x, one
+            // all-reduce); the bookkeeping kernel re-activates the systems whose true residual is above tol and the
+            // iteration resumes from the true residual (the single-GPU rule, a7)
+            ++confirms;
+            h->fuse_push_pq = h->fuse_push_sums = PeerPush(); h->fuse_red_pq = h->fuse_red_sums = nullptr;
+            if ((rc = cgp_true_residual(h, x, b, mass, nrhs)) || (rc = poll_state(h))) return rc;
+            s = *h->host_state;
+            h->info_reliable = confirms;
+        }
         if (s.done || s.breakdown || s.iter >= h->max_iter) {
             h->info_iters = s.iter;
             for (int k = 0; k < nrhs; ++k) h->info_relres[k] = s.bnorm2[k] > 0.0 ? std::sqrt(s.rho[k] / s.bnorm2[k]) : 0.0;
