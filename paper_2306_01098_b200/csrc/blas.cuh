@@ -30,6 +30,17 @@ template <typename T> __device__ __forceinline__ typename V16<T>::type pack16(co
 template <> __device__ __forceinline__ double2 pack16<double>(const double* e) { return make_double2(e[0], e[1]); }
 template <> __device__ __forceinline__ float4 pack16<float>(const float* e) { return make_float4(e[0], e[1], e[2], e[3]); }
 
+// Partitioned lattices: the per-iteration updates touch the OWNED slices only.  A field is 3 planes (colour) per RHS,
+// the owned part of a plane is one contiguous run: vector i' of the 3*seg owned vectors is vector
+// (i'/seg)*plane + off + i'%seg of the field.  seg == 0: the whole field, i' = i.
+struct Span { size_t seg, plane, off; };
+__device__ __forceinline__ size_t span_map(const Span& sp, size_t i)
+{
+    if (sp.seg == 0) return i;
+    const size_t c = i / sp.seg;
+    return c * sp.plane + sp.off + (i - c * sp.seg);
+}
+
 inline int blas_grid_x(size_t nreal, int vec_n) {
     size_t nvec = nreal / vec_n;
     return (int)((nvec + (size_t)kBlasBlock * kBlasItems - 1) / ((size_t)kBlasBlock * kBlasItems));
@@ -76,7 +87,7 @@ inline int init_grid_x(size_t nreal) { return (int)((nreal + (size_t)kBlasBlock 
 // ---- p_k = r_k + beta_k p_k  (first kernel of an iteration; beta = 0 at the start gives p = r) -------
 template <typename T>
 __global__ void __launch_bounds__(kBlasBlock) cg_update_p_kernel(T* __restrict__ p, const T* __restrict__ r, size_t nreal,
-                                                                 const CgState* st)
+                                                                 const CgState* st, Span sp = Span())
 {
     if (st->done) return;
     using V = typename V16<T>::type;
@@ -84,14 +95,14 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_p_kernel(T* __restrict__
     const int k = blockIdx.y;
     if (!st->active[k]) return;  // frozen RHS keep their search direction (needed if they are resumed)
     const T beta = (T)st->beta[k];
-    const size_t nvec = nreal / N;
+    const size_t nvec = sp.seg ? 3 * sp.seg : nreal / N;
     V* pv = reinterpret_cast<V*>(p + (size_t)k * nreal);
     const V* rv = reinterpret_cast<const V*>(r + (size_t)k * nreal);
     V rr[kBlasItems], pp[kBlasItems];
 #pragma unroll
     for (int it = 0; it < kBlasItems; ++it) {
         size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
-        if (i < nvec) { rr[it] = rv[i]; pp[it] = pv[i]; }
+        if (i < nvec) { const size_t j = span_map(sp, i); rr[it] = rv[j]; pp[it] = pv[j]; }
     }
 #pragma unroll
     for (int it = 0; it < kBlasItems; ++it) {
@@ -101,7 +112,7 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_p_kernel(T* __restrict__
             unpack16<T>(rr[it], a); unpack16<T>(pp[it], b);
 #pragma unroll
             for (int e = 0; e < N; ++e) b[e] = fma(beta, b[e], a[e]);
-            pv[i] = pack16<T>(b);
+            pv[span_map(sp, i)] = pack16<T>(b);
         }
     }
 }
@@ -111,7 +122,7 @@ template <typename T>
 __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict__ x, T* __restrict__ r, const T* __restrict__ p,
                                                                   const T* __restrict__ q, size_t nreal, CgState* st,
                                                                   double* partial, int defer = 0, PeerPush push = PeerPush(),
-                                                                  const double* red_pq = nullptr)
+                                                                  const double* red_pq = nullptr, Span sp = Span())
 {
     // defer = 1 (partitioned lattice).  red_pq: <p,q> is not in st->pq yet but, rank by rank, in this slot of the
     // mailbox (every block adds them up itself); push: the last block hands the local ||r||^2 to all ranks.
@@ -128,7 +139,7 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict_
         alpha_d = (pq > 0.0 && isfinite(pq)) ? st->rho[k] / pq : 0.0;
     }
     const T alpha = (T)alpha_d;
-    const size_t nvec = nreal / N;
+    const size_t nvec = sp.seg ? 3 * sp.seg : nreal / N;
     const size_t base = (size_t)k * nreal;
     V* xv = reinterpret_cast<V*>(x + base);
     V* rv = reinterpret_cast<V*>(r + base);
@@ -139,7 +150,7 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict_
 #pragma unroll
     for (int it = 0; it < kBlasItems; ++it) {
         size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
-        if (live && i < nvec) { xx[it] = xv[i]; rr[it] = rv[i]; pp[it] = pv[i]; qq[it] = qv[i]; }
+        if (live && i < nvec) { const size_t j = span_map(sp, i); xx[it] = xv[j]; rr[it] = rv[j]; pp[it] = pv[j]; qq[it] = qv[j]; }
     }
     double sum[1] = { 0.0 };
 #pragma unroll
@@ -154,8 +165,9 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict_
                 b[e] = fma(-alpha, d[e], b[e]);
                 sum[0] += (double)b[e] * (double)b[e];
             }
-            xv[i] = pack16<T>(a);
-            rv[i] = pack16<T>(b);
+            const size_t j = span_map(sp, i);
+            xv[j] = pack16<T>(a);
+            rv[j] = pack16<T>(b);
         }
     }
     __shared__ double totals[kMaxNrhs];

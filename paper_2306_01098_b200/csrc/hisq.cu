@@ -414,12 +414,22 @@ extern "C" int hisq_apply_A(hisq_ctx* h, void* out, const void* in, double mass,
 // ---- CG --------------------------------------------------------------------------------------------
 // One iteration (textbook Hestenes-Stiefel, independent scalars per RHS):
 //   p = r + beta p ; t = D_oe p ; q = m^2 p - D_eo t , <p,q> ; x += alpha p , r -= alpha q , rho' = ||r||^2
+static Span owned_span(const hisq_ctx* h, int vec_n)
+{
+    Span sp = { 0, 0, 0 };
+    if (h->g.part) {   // vectors of vec_n reals; a plane is [Lt_ext][S] complex, the owned run starts at slice t_lo
+        const size_t S = (size_t)h->g.Vh / h->g.L[3];
+        sp.seg = 2 * S * h->g.t_cnt / vec_n; sp.plane = 2 * S * h->g.L[3] / vec_n; sp.off = 2 * S * h->g.t_lo / vec_n;
+    }
+    return sp;
+}
 template <typename T>
 static int enqueue_p_update(hisq_ctx* h, T* p, const T* r, int nrhs)
 {
     const size_t nreal = (size_t)6 * h->g.Vh;
-    dim3 gb((unsigned)blas_grid_x(nreal, V16<T>::n), (unsigned)nrhs);
-    cg_update_p_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(p, r, nreal, h->state);
+    const Span sp = owned_span(h, V16<T>::n);
+    dim3 gb((unsigned)blas_grid_x(sp.seg ? 3 * sp.seg * V16<T>::n : nreal, V16<T>::n), (unsigned)nrhs);
+    cg_update_p_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(p, r, nreal, h->state, sp);
     h->stats.launches++;
     CK(cudaGetLastError());
     return HISQ_OK;
@@ -945,7 +955,8 @@ static int cgp_phase(hisq_ctx* h, const T* links, int phase, double mass)
     const size_t nreal = (size_t)6 * h->g.Vh;
     CgpFields f = cgp_fields(h);
     T *r = (T*)f.r, *p = (T*)f.p, *q = (T*)f.q, *t = (T*)f.t, *x = (T*)h->cgp_x;
-    dim3 gb((unsigned)blas_grid_x(nreal, V16<T>::n), (unsigned)nrhs);
+    const Span sp = owned_span(h, V16<T>::n);
+    dim3 gb((unsigned)blas_grid_x(sp.seg ? 3 * sp.seg * V16<T>::n : nreal, V16<T>::n), (unsigned)nrhs);
     switch (phase) {
     case 0:  // after the all-reduce of rho (= ||b||^2)
         cgp_finalize_init_kernel<<<1, 1, 0, h->stream>>>(h->state, nrhs, h->cgp_tol, h->max_iter);
@@ -976,7 +987,7 @@ static int cgp_phase(hisq_ctx* h, const T* links, int phase, double mass)
         return HISQ_OK;
     }
     case 4:
-        cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial, 1, h->fuse_push_sums, h->fuse_red_pq);
+        cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial, 1, h->fuse_push_sums, h->fuse_red_pq, sp);
         h->stats.launches++;
         break;
     case 5:  // after the all-reduce of sums (= ||r||^2)
