@@ -209,6 +209,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-multishift", action="store_true")
     ap.add_argument("--no-compression", action="store_true")
+    ap.add_argument("--no-partition", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--ref-budget", type=float, default=10.0)
     ap.add_argument("--dslash-reps", type=int, default=100)
@@ -361,6 +362,30 @@ def main():
         del xs
     ctx.close()
     del ctx, b, x
+    # ---- row f3: the same solve on a t-partitioned context with ONE rank (ring closed on itself): what the multi-GPU
+    # machinery (mailbox halos and all-reduces, unfused updates) costs per iteration on one GPU.  Context, not a scaling number.
+    part = None
+    if not args.no_partition and cfg["prec"] != "mixed" and rank == 0 and L[3] >= 4 and L[3] % 2 == 0:
+        from paper_2306_01098_b200 import partition
+        pc = binding.Hisq(L, cfg["prec"], n, dev, part=(0, 1))
+        fat, naik = partition.make_links_part(L, rank, 0, 1, dev, pc.cdtype, gen_device=gen_dev)
+        pc.set_links(fat, naik)
+        del fat, naik
+        pb = pc.pack(partition.make_sources_part(L, rank, n, 0, 0, 1, dev, pc.cdtype, gen_device=gen_dev))
+        peer = partition.PeerHalo(pc, 0, 1, n)
+        px = pc.new_field(n)
+        pc.cg(pb, cfg["mass"], cfg["tol"], x=px)
+        torch.cuda.synchronize()
+        e0.record()
+        _, pi = pc.cg(pb, cfg["mass"], cfg["tol"], x=px)
+        e1.record()
+        e1.synchronize()
+        part = {"ranks": 1, "transport": "peer mailboxes (ring closed on the rank)", "solve_ms": e0.elapsed_time(e1),
+                "iterations": pi["iterations"], "ms_per_iteration": e0.elapsed_time(e1) / max(pi["iterations"], 1),
+                "true_rel_resid": pi["true_rel_resid"]}
+        peer.close()
+        pc.close()
+        del pc, pb, px
 
     out = {
         "metric": "hisq_dslash_gflops", "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
@@ -372,6 +397,7 @@ def main():
                "true_rel_resid": info["true_rel_resid"], "ms_per_iteration": ms_all / args.steps / max(info["iterations"], 1)},
         "dslash": dsl,
         "multishift_cg": ms,
+        "partitioned_cg": part,
         "naik_compression": comp,
         "roofline": {"bound": "hbm", "kernel": f"dslash_kernel<{'float' if w == 4 else 'double'},NR={min(n, 8 if w == 4 else 4)}>",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
