@@ -318,6 +318,67 @@ def test_hisq_cg_on_a_partitioned_context_single_rank_ring():
     ctx.close(); ref.close()
 
 
+def test_peer_calls_out_of_order_are_refused():
+    """The two-slot mailbox protocol is only safe if sends and recvs alternate strictly: the library enforces it."""
+    L, n = (4, 4, 4, 8), 2
+    dev = torch.device("cuda:0")
+    ctx = binding.Hisq(L, "fp64", n, dev, part=(0, 1))
+    f = ctx.new_field(n)
+    f.zero_()
+    with pytest.raises(binding.HisqError):
+        ctx.halo_send(f)                                   # no mailboxes attached
+    box = ctx.peer_mailbox(n)
+    with pytest.raises(binding.HisqError):
+        ctx.peer_attach([box, box], n)                     # one rank, two boxes
+    with pytest.raises(binding.HisqError):
+        ctx.peer_attach([box[8:]], n)                      # misaligned
+    ctx.peer_attach([box], n)
+    with pytest.raises(binding.HisqError):
+        ctx.halo_recv(f)                                   # nothing sent
+    ctx.halo_send(f)
+    with pytest.raises(binding.HisqError):
+        ctx.halo_send(f)                                   # two sends in a row
+    ctx.halo_recv(f)
+    with pytest.raises(binding.HisqError):
+        ctx.peer_reduce_recv(3, n)                         # nothing sent
+    with pytest.raises(binding.HisqError):
+        ctx.peer_reduce_send(7, n)                         # not a state array
+    ctx.peer_reduce_send(3, n)
+    with pytest.raises(binding.HisqError):
+        ctx.peer_reduce_send(4, n)                         # one reduce at a time
+    ctx.peer_reduce_recv(3, n)
+    torch.cuda.synchronize()
+    # a plain (not partitioned) context has no mailbox
+    plain = binding.Hisq(L, "fp64", n, dev)
+    with pytest.raises(binding.HisqError):
+        plain.peer_mailbox(n)
+    plain.close(); ctx.close()
+
+
+def test_peer_allreduce_sums_in_rank_order_same_bits_everywhere():
+    """Emulated ranks: values chosen so that the floating-point sum depends on the order; every rank must end up with
+    the rank-order sum, bit for bit."""
+    L, n, nranks = (4, 4, 4, 16), 3, 4
+    dev = torch.device("cuda:0")
+    ctxs = [binding.Hisq(L, "fp64", n, dev, part=(r, nranks)) for r in range(nranks)]
+    boxes = [c.peer_mailbox(n) for c in ctxs]
+    for c in ctxs:
+        c.peer_attach(boxes, n)
+    vals = torch.tensor([[1e16, 1.0, -3.5], [1.0, 1e-16, 2.25], [-1e16, 1.0, 1e8], [1.0, -1.0, -1e8]], dtype=torch.float64, device=dev)
+    for rep in range(5):                                   # several rounds: both slots are reused
+        for r, c in enumerate(ctxs):
+            c.cgp_tensor(3, n).copy_(vals[r] * (rep + 1))
+        for c in ctxs: c.peer_reduce_send(3, n)
+        for c in ctxs: c.peer_reduce_recv(3, n)
+        want = torch.zeros(n, dtype=torch.float64, device=dev)
+        for r in range(nranks):
+            want = want + vals[r] * (rep + 1)
+        for c in ctxs:
+            assert torch.equal(c.cgp_tensor(3, n), want)
+    for c in ctxs:
+        c.close()
+
+
 def _mp_worker(rank, world, port, L, m, tol, seed, q, transport):
     import os, sys
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
