@@ -155,6 +155,29 @@ def cg(L, X, W, mass: float, tol: float, b, max_iter: int = 100000, hist_len: in
     return x, iters, relres, int(st), hist
 
 
+def apply_M(L, X, W, mass: float, phi) -> np.ndarray:
+    """M phi = (D + m) phi on the whole lattice (Eq. (1))."""
+    V = volume(L)
+    X, W, phi = _links(X, V), _links(W, V), _field(phi, V)
+    out = np.empty_like(phi)
+    _lib().oracle_apply_M(_L(L), _c(X), _c(W), ctypes.c_double(mass), _c(phi), _c(out), ctypes.c_int(phi.shape[0]))
+    return out
+
+
+def solve_M(L, X, W, mass: float, tol: float, b, max_iter: int = 100000):
+    """Solve M x_k = b_k on the whole lattice by CG on the normal equations with full-lattice operators only.
+    Returns (x, iters[nrhs], relres[nrhs] = ||b - M x|| / ||b||, status)."""
+    V = volume(L)
+    X, W, b = _links(X, V), _links(W, V), _field(b, V)
+    n = b.shape[0]
+    x = np.empty_like(b)
+    iters = np.zeros(n, dtype=np.int32)
+    relres = np.zeros(n, dtype=np.float64)
+    st = _lib().oracle_solve_M(_L(L), _c(X), _c(W), ctypes.c_double(mass), ctypes.c_double(tol), ctypes.c_int(max_iter),
+                               _c(b), _c(x), ctypes.c_int(n), _c(iters), _c(relres))
+    return x, iters, relres, int(st)
+
+
 def counts_per_site(L, X, W, phi):
     """Pin P1: run the counting build on the full lattice, return per-site
     (flops, link words, vector words, output words)."""

@@ -33,7 +33,8 @@
  *
  * Pins (tests/test_oracle_pins.py): P1 counts, P2 free-field closed form, P3 anti-Hermiticity,
  * P4 gauge covariance, P5 parity, P6 boundary-sign folding, P7 dense 4^4 brute force, P8 point
- * source, P9 linearity, P10 index bijection, P11/P12 CG.  Parity UNPINNED: nothing here.
+ * source, P9 linearity, P10 index bijection, P11/P12 CG, P15 full-matrix solve (dense M on 4^4).
+ * Parity UNPINNED: nothing here.
  */
 #include <complex.h>
 #ifdef _OPENMP
@@ -345,6 +346,66 @@ int oracle_cg(const int *L, const cplx *X, const cplx *W, double mass, double to
         relres[k] = bb > 0.0 ? sqrt(re_dot(q, q, n) / bb) : 0.0;
     }
     free(r); free(p); free(q); free(bk);
+    return status;
+}
+
+/* ---------- the full fermion matrix M = D + m (Eq. (1) PAPER.md:131 writes det(D + m)) ---------- */
+
+/* out = (D + m) phi on the whole lattice (both parities). */
+void oracle_apply_M(const int *L, const cplx *X, const cplx *W, double mass, const cplx *phi, cplx *out,
+                    int nrhs)
+{
+    long n = 3 * volume_of(L) * nrhs;
+    oracle_dslash_rows(L, X, W, phi, out, nrhs, 3);
+    for (long i = 0; i < n; ++i) out[i] += mass * phi[i];
+}
+
+/* Solve M x_k = b_k on the WHOLE lattice, x_0 = 0, by textbook CG on the normal equations
+ *      M^+ M x = M^+ b,   M^+ = m - D  (D^+ = -D, pin P3),   M^+ M = m^2 - D D
+ * written with full-lattice operators only -- no even-odd decomposition, no Schur complement: this is the
+ * plain definition the GPU's even-odd preconditioned solve must reproduce.
+ * Stop when ||M^+ b - M^+ M x|| <= tol ||M^+ b||; relres[k] = ||b - M x|| / ||b|| recomputed at the end
+ * (the quantity the GPU call bounds).  Returns 0, or 1 if some RHS hit max_iter. */
+int oracle_solve_M(const int *L, const cplx *X, const cplx *W, double mass, double tol, int max_iter,
+                   const cplx *b, cplx *x, int nrhs, int *iters, double *relres)
+{
+    long V = volume_of(L);
+    long n = 3 * V;
+    int status = 0;
+    cplx *r = (cplx *)malloc(sizeof(cplx) * n), *p = (cplx *)malloc(sizeof(cplx) * n),
+         *q = (cplx *)malloc(sizeof(cplx) * n), *t = (cplx *)malloc(sizeof(cplx) * n);
+    for (int k = 0; k < nrhs; ++k) {
+        const cplx *bk = b + (long)k * n;
+        cplx *xk = x + (long)k * n;
+        memset(xk, 0, sizeof(cplx) * n);
+        /* r = M^+ b = m b - D b */
+        oracle_dslash_rows(L, X, W, bk, t, 1, 3);
+        for (long i = 0; i < n; ++i) r[i] = mass * bk[i] - t[i];
+        memcpy(p, r, sizeof(cplx) * n);
+        double cc = re_dot(r, r, n), rho = cc;
+        int it = 0;
+        while (cc > 0.0 && sqrt(rho) > tol * sqrt(cc)) {
+            if (it >= max_iter) { status = 1; break; }
+            /* q = M^+ M p = m^2 p - D (D p) */
+            oracle_dslash_rows(L, X, W, p, t, 1, 3);
+            oracle_dslash_rows(L, X, W, t, q, 1, 3);
+            for (long i = 0; i < n; ++i) q[i] = mass * mass * p[i] - q[i];
+            double alpha = rho / re_dot(p, q, n);
+            for (long i = 0; i < n; ++i) xk[i] += alpha * p[i];
+            for (long i = 0; i < n; ++i) r[i] -= alpha * q[i];
+            double rho_new = re_dot(r, r, n);
+            ++it;
+            double beta = rho_new / rho;
+            for (long i = 0; i < n; ++i) p[i] = r[i] + beta * p[i];
+            rho = rho_new;
+        }
+        iters[k] = it;
+        oracle_apply_M(L, X, W, mass, xk, q, 1);
+        for (long i = 0; i < n; ++i) q[i] = bk[i] - q[i];
+        double bb = re_dot(bk, bk, n);
+        relres[k] = bb > 0.0 ? sqrt(re_dot(q, q, n) / bb) : 0.0;
+    }
+    free(r); free(p); free(q); free(t);
     return status;
 }
 

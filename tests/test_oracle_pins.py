@@ -378,3 +378,49 @@ def test_shifted_system_is_a_mass_shift_dense_check():
     xd = np.linalg.solve(A + sigma * np.eye(A.shape[0]), b[0].reshape(-1)[rows_e])
     x, _, _, st, _ = oracle.cg(L, X, W, float(np.sqrt(m * m + sigma)), 1e-12, b)
     assert st == 0 and rel_l2(x[0].reshape(-1)[rows_e], xd) < 1e-10
+
+
+# ---------------------------------------------------------------- P15: the full fermion matrix M = D + m
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (4, 4, 4, 6)])
+def test_p15_full_matrix_solve_matches_dense_and_schur_identity(L):
+    """oracle.solve_M (full-lattice normal-equation CG) against numpy's dense solve of M = D + m built entry by entry
+    (oracle/dense.py); and, in dense algebra only, the even-odd identity the GPU path relies on:
+    x_e solves (m^2 - D_eo D_oe) x_e = m b_e - D_eo b_o and x_o = (b_o - D_oe x_e) / m."""
+    m, tol = 0.25, 1e-12
+    X, W = oracle_links(L, 15)
+    D = dense.dense_D(L, X, W)
+    n = D.shape[0]
+    M = D + m * np.eye(n)
+    b = oracle_field(L, 15, 2)
+    assert rel_l2(oracle.apply_M(L, X, W, m, b)[1], (M @ b[1].reshape(-1)).reshape(-1, 3)) < 1e-14
+    x, iters, relres, st = oracle.solve_M(L, X, W, m, tol, b)
+    kappa = np.linalg.cond(M)
+    assert st == 0 and np.all(relres < kappa * tol)
+    par = np.repeat(oracle.site_parity(L), 3)
+    e, o = np.nonzero(par == 0)[0], np.nonzero(par == 1)[0]
+    Deo, Doe = D[np.ix_(e, o)], D[np.ix_(o, e)]
+    assert np.abs(D[np.ix_(e, e)]).max() == 0 and np.abs(D[np.ix_(o, o)]).max() == 0    # P5 again, on the matrix
+    for k in range(2):
+        bk = b[k].reshape(-1)
+        xd = np.linalg.solve(M, bk)
+        assert rel_l2(x[k].reshape(-1), xd) < kappa * kappa * tol
+        xe = np.linalg.solve(m * m * np.eye(e.size) - Deo @ Doe, m * bk[e] - Deo @ bk[o])
+        xo = (bk[o] - Doe @ xe) / m
+        assert rel_l2(xe, xd[e]) < 1e-11 and rel_l2(xo, xd[o]) < 1e-11
+
+
+def test_p15_free_field_inverse_closed_form():
+    """Plane waves are eigenvectors of D with eigenvalue i*lambda(x) = sum_mu eta_mu(x) 2i (c1 sin p + c3 sin 3p), but eta
+    depends on the site, so M^{-1} is pinned through M^+ M instead: M^+ M phi = (m^2 + sum_mu (...)^2) phi on the whole
+    lattice, hence solve_M(M phi) = phi and solve_M(phi) = M^+ phi / (m^2 + sum)."""
+    L = (4, 6, 8, 8)
+    c1, c3, m = 0.625, -1.0 / 24.0, 0.3
+    X, W, _ = _free_links(L, c1, c3)
+    phi, p = _plane_wave(L, (1, 2, 1, 0), np.array([1.0, 0.5j, -0.25]))
+    ev = m * m + ((2 * c1 * np.sin(p) + 2 * c3 * np.sin(3 * p)) ** 2).sum()
+    x, iters, relres, st = oracle.solve_M(L, X, W, m, 1e-13, phi[None])
+    Mdag_phi = m * phi - oracle.dslash(L, X, W, phi)[0]
+    assert st == 0 and iters[0] <= 2
+    assert rel_l2(x[0], Mdag_phi / ev) < 1e-12
+    y = oracle.solve_M(L, X, W, m, 1e-13, oracle.apply_M(L, X, W, m, phi[None]))[0]
+    assert rel_l2(y[0], phi) < 1e-12
