@@ -112,6 +112,21 @@ int hisq_cg(hisq_ctx *h, void *x, const void *b, double mass, double tol, int nr
  * HISQ_FP64 and HISQ_FP32 contexts only (HISQ_MIXED: HISQ_EINVAL). */
 int hisq_cg_multishift(hisq_ctx *h, void *x, const void *b, double mass, const double *shifts, int nshift, double tol);
 
+/* Solve the full staggered system  M x = b,  M = D + mass  (Eq. (1)), on BOTH parities for nrhs right-hand
+ * sides, by even-odd (Schur complement) preconditioning on top of hisq_cg (the solvers work on
+ * M^+ M, whose even-even block is mass^2 - D_eo D_oe):
+ *     s_e = mass b_e - D_eo b_o                     one Dslash, the xpay fused into its epilogue
+ *     (mass^2 - D_eo D_oe) x_e = s_e                hisq_cg (this context's precision mode, incl. HISQ_MIXED)
+ *     x_o = (b_o - D_oe x_e) / mass                 one Dslash + one element-wise kernel
+ * b_even, b_odd, x_even, x_odd: NATIVE half-lattice fields (nrhs each), pairwise non-overlapping; x_odd is also used as
+ * scratch during the solve.  mass > 0.  Since b - M x = (r_e / mass, 0) with r_e the residual of the even system,
+ * the even solve is run to tol * min_k( mass ||b_k|| / ||s_e,k|| ), so that on success every right-hand side has
+ * ||b_k - M x_k|| <= tol ||b_k|| over the whole lattice; hisq_get_info then reports that full-lattice ratio.
+ * Returns after the solve has finished (synchronises the stream).  Errors as hisq_cg; partitioned contexts:
+ * HISQ_EINVAL. */
+int hisq_solve_M(hisq_ctx *h, void *x_even, void *x_odd, const void *b_even, const void *b_odd, double mass, double tol,
+                 int nrhs);
+
 /* Options: "max_iter" (default 100000), "reliable_interval" (default 100 for HISQ_MIXED, 0 = off for
  * the others), "check_interval" (iterations enqueued between host polls of the convergence flag,
  * default 32), "use_graph" (1: replay one CG iteration as a CUDA graph, default 1),

@@ -16,6 +16,7 @@ from . import layout
 HISQ_FP32, HISQ_FP64, HISQ_MIXED = 4, 8, 12
 HISQ_EVEN, HISQ_ODD = 0, 1
 HISQ_MAX_NRHS = 16
+HISQ_EINVAL, HISQ_ENOLINKS, HISQ_ENOWORKSPACE, HISQ_ECUDA = -1, -2, -3, -4
 HISQ_ENOCONV, HISQ_EBREAKDOWN = -5, -6
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -23,7 +24,7 @@ LIB_PATH = os.environ.get("HISQ_LIB", os.path.join(_HERE, "libhisq.so"))
 
 EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
-    "hisq_set_links", "hisq_dslash", "hisq_apply_A", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
+    "hisq_set_links", "hisq_dslash", "hisq_apply_A", "hisq_solve_M", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
     "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count",
     "hisq_create_part", "hisq_peer_bytes", "hisq_peer_attach", "hisq_halo_send", "hisq_halo_recv", "hisq_peer_reduce_send", "hisq_peer_reduce_recv", "hisq_dslash_slices", "hisq_dslash_edges", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
     "hisq_cgp_begin", "hisq_cgp_phase", "hisq_cgp_ptr", "hisq_cgp_status", "hisq_strerror",
@@ -61,6 +62,7 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_dslash_edges.argtypes = [vp, vp, vp, i, i, i]
     lib.hisq_cg.argtypes = [vp, vp, vp, d, d, i]
     lib.hisq_apply_A.argtypes = [vp, vp, vp, d, i]
+    lib.hisq_solve_M.argtypes = [vp, vp, vp, vp, vp, d, d, i]
     lib.hisq_cg_multishift.argtypes = [vp, vp, vp, d, ctypes.POINTER(d), i, d]
     lib.hisq_set_option.argtypes = [vp, ctypes.c_char_p, d]
     lib.hisq_get_info.argtypes = [vp, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(d)]
@@ -240,6 +242,18 @@ class Hisq:
                                 float(mass), float(tol), n)
         self._check(code, allow=() if strict else (HISQ_ENOCONV, HISQ_EBREAKDOWN))
         return x, self.info(n, code)
+
+    def solve_M(self, b_even: torch.Tensor, b_odd: torch.Tensor, mass: float, tol: float, strict: bool = True):
+        """(D + mass) x = b on both parities.  Returns (x_even, x_odd, info); info['true_rel_resid'] is the
+        full-lattice ||b - M x|| / ||b|| per right-hand side."""
+        n = b_even.shape[0]
+        xe, xo = self.new_field(n), self.new_field(n)
+        shp = (n, 3, self.Vh)
+        code = self.lib.hisq_solve_M(self._h, self._ptr(xe, shp, self.cdtype), self._ptr(xo, shp, self.cdtype),
+                                     self._ptr(b_even, shp, self.cdtype), self._ptr(b_odd, shp, self.cdtype),
+                                     float(mass), float(tol), n)
+        self._check(code, allow=() if strict else (HISQ_ENOCONV, HISQ_EBREAKDOWN))
+        return xe, xo, self.info(n, code)
 
     def cg_multishift(self, b: torch.Tensor, mass: float, shifts, tol: float, x: Optional[torch.Tensor] = None,
                       strict: bool = True):

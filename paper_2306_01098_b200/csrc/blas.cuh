@@ -320,6 +320,41 @@ __global__ void __launch_bounds__(kBlasBlock) cg_fused_update_kernel(T* __restri
     }
 }
 
+// ---- full-lattice solve M x = b (hisq_solve_M): norms and the odd-site reconstruction ------------------------------
+// out[k] = ||a_k||^2 (+ ||b_k||^2 if b != nullptr), k = blockIdx.y, summed in fp64 in the fixed two-stage order
+template <typename T>
+__global__ void __launch_bounds__(kBlasBlock) norm2_kernel(const T* __restrict__ a, const T* __restrict__ b, size_t nreal, CgState* st,
+                                                           double* partial, double* out)
+{
+    const int k = blockIdx.y;
+    const size_t base = (size_t)k * nreal;
+    double sum[1] = { 0.0 };
+    for (int it = 0; it < kBlasItems * 4; ++it) {
+        size_t i = ((size_t)blockIdx.x * kBlasItems * 4 + it) * kBlasBlock + threadIdx.x;
+        if (i < nreal) {
+            const double v = (double)a[base + i];
+            sum[0] += v * v;
+            if (b != nullptr) {
+                const double w = (double)b[base + i];
+                sum[0] += w * w;
+            }
+        }
+    }
+    __shared__ double totals[kMaxNrhs];
+    if (grid_reduce<1, kBlasBlock>(sum, k, partial, gridDim.x, blockIdx.x, &st->ticket[0], gridDim.x * gridDim.y, gridDim.y, totals)) {
+        if (threadIdx.x < gridDim.y) out[threadIdx.x] = totals[threadIdx.x];
+    }
+}
+
+// x_o = (b_o - t) * inv_m   with t = D_oe x_e
+template <typename T>
+__global__ void __launch_bounds__(kBlasBlock) recon_odd_kernel(T* __restrict__ x, const T* __restrict__ b, const T* __restrict__ t,
+                                                               size_t n, T inv_m)
+{
+    for (size_t i = (size_t)blockIdx.x * kBlasBlock + threadIdx.x; i < n; i += (size_t)gridDim.x * kBlasBlock)
+        x[i] = (b[i] - t[i]) * inv_m;
+}
+
 // ---- partitioned-lattice CG (row f3): scalar updates that consume GLOBAL (all-reduced) sums ------------------------
 __global__ void cgp_finalize_init_kernel(CgState* st, int n, double tol, int max_iter, const double* red = nullptr, int nranks = 0)
 {

@@ -4,6 +4,7 @@
 
 #include <cuda.h>   // types of the stream memory operations only: the entry points are looked up at run time, libcuda is not linked
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -818,6 +819,71 @@ extern "C" int hisq_cg(hisq_ctx* h, void* x, const void* b, double mass, double 
     if (h->prec == HISQ_FP32) return cg_solve<float, float>(h, h->links32, nullptr, (float*)x, (const float*)b, mass, tol, nrhs);
     if (h->prec == HISQ_FP64) return cg_solve<double, double>(h, h->links64, nullptr, (double*)x, (const double*)b, mass, tol, nrhs);
     return cg_solve<float, double>(h, h->links32, h->links64, (double*)x, (const double*)b, mass, tol, nrhs);
+}
+
+// ---- full-lattice solve M x = b, M = D + m (Eq. (1)) by even-odd preconditioning ----------------------
+template <typename T>
+static int solve_M_impl(hisq_ctx* h, const T* links, T* xe, T* xo, const T* be, const T* bo, double mass, double tol, int nrhs)
+{
+    const size_t nreal = (size_t)6 * h->g.Vh;
+    double* dsum = h->state->sums;
+    double bb[kMaxNrhs], ss[kMaxNrhs];
+    const dim3 gn((unsigned)init_grid_x(nreal), (unsigned)nrhs);
+    norm2_kernel<T><<<gn, kBlasBlock, 0, h->stream>>>(be, bo, nreal, h->state, h->partial, dsum);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(bb, dsum, nrhs * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    // s_e = m b_e - D_eo b_o, kept in the caller's x_odd until the even system is solved
+    T* s = xo;
+    int rc = run_dslash<T>(h, links, s, bo, HISQ_EVEN, nrhs, MODE_APPLY_A, be, nullptr, mass, h->state->pq, nullptr, 2);
+    if (rc) return rc;
+    norm2_kernel<T><<<gn, kBlasBlock, 0, h->stream>>>(s, nullptr, nreal, h->state, h->partial, dsum);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(ss, dsum, nrhs * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    double scale = 1e300;   // tol of the even system: ||r_e|| <= tol m ||b|| for every RHS
+    for (int k = 0; k < nrhs; ++k)
+        if (ss[k] > 0.0 && bb[k] > 0.0) scale = std::fmin(scale, mass * std::sqrt(bb[k] / ss[k]));
+    if (scale == 1e300) scale = 1.0;   // b = 0 (or s_e = 0: the even system is solved by x_e = 0)
+    const int rc_cg = hisq_cg(h, xe, s, mass, tol * scale, nrhs);
+    if (rc_cg != HISQ_OK && rc_cg != HISQ_ENOCONV) return rc_cg;
+    // x_o = (b_o - D_oe x_e) / m ; t in the solver's (now idle) temporary
+    const size_t fb = field_bytes(h, h->ws_nrhs, elem_size(h->prec));
+    T* t = (T*)(h->fields + 3 * fb);
+    rc = run_dslash<T>(h, links, t, xe, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, nullptr, 2);
+    if (rc) return rc;
+    const size_t n = nreal * nrhs;
+    unsigned grid = (unsigned)std::min<size_t>((n + kBlasBlock - 1) / kBlasBlock, (size_t)h->num_sms * 16);
+    recon_odd_kernel<T><<<grid, kBlasBlock, 0, h->stream>>>(xo, bo, t, n, (T)(1.0 / mass));
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(h->stream));
+    // hisq_cg left ||s_e - A x_e|| / ||s_e||; the full-lattice residual is ||r_e|| / (m ||b||)
+    for (int k = 0; k < nrhs; ++k)
+        h->info_relres[k] = bb[k] > 0.0 ? h->info_relres[k] * std::sqrt(ss[k] / bb[k]) / mass : 0.0;
+    return rc_cg;
+}
+
+extern "C" int hisq_solve_M(hisq_ctx* h, void* x_even, void* x_odd, const void* b_even, const void* b_odd, double mass, double tol,
+                            int nrhs)
+{
+    if (!h || !x_even || !x_odd || !b_even || !b_odd || nrhs < 1 || nrhs > HISQ_MAX_NRHS || !(tol > 0.0) || !std::isfinite(mass) ||
+        !(mass > 0.0))
+        return HISQ_EINVAL;
+    const void* ptr[4] = { x_even, x_odd, b_even, b_odd };
+    const size_t bytes = (size_t)nrhs * 6 * h->g.Vh * elem_size(h->prec);
+    for (int i = 0; i < 4; ++i) {
+        if ((uintptr_t)ptr[i] & 15) return HISQ_EINVAL;
+        for (int j = i + 1; j < 4; ++j)
+            if (overlap(ptr[i], ptr[j], bytes)) return HISQ_EINVAL;
+    }
+    if (!h->ws || nrhs > h->ws_nrhs) return HISQ_ENOWORKSPACE;
+    if (!h->have_links) return HISQ_ENOLINKS;
+    if (h->g.part) return HISQ_EINVAL;
+    if (h->prec == HISQ_FP32)
+        return solve_M_impl<float>(h, h->links32, (float*)x_even, (float*)x_odd, (const float*)b_even, (const float*)b_odd, mass, tol, nrhs);
+    return solve_M_impl<double>(h, h->links64, (double*)x_even, (double*)x_odd, (const double*)b_even, (const double*)b_odd, mass, tol, nrhs);
 }
 
 // ---- options / info ----------------------------------------------------------------------------------
