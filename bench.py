@@ -316,6 +316,20 @@ def main():
            "frac_of_measured_copy": achieved / peak, "frac_of_8TBs": achieved / 8000.0,
            "frac_of_measured_read_only": achieved / READ_ONLY_GBS,
            "frac_of_fma_peak": FLOP_PER_SITE * Vh * n / (d_ms * 1e-3) / 1e9 / FMA_PEAK_GFLOPS[w], "tiles": ctx.tiles(n)}
+    # ---- row f4 (part): the full system (D + m) x = b on both parities, same lattice, mass and tol, one solve ----
+    full = None
+    if not args.no_multishift and rank == 0:
+        bo = ctx.pack(binding.make_sources(L, rank, n, 1, dev, ctx.cdtype, gen_device=gen_dev))
+        ctx.solve_M(b, bo, cfg["mass"], cfg["tol"])
+        torch.cuda.synchronize()
+        e0.record()
+        _, _, fi = ctx.solve_M(b, bo, cfg["mass"], cfg["tol"])
+        e1.record()
+        e1.synchronize()
+        full = {"what": "hisq_solve_M: s_e = m b_e - D_eo b_o, CG on the even system, x_o = (b_o - D_oe x_e) / m",
+                "solve_ms": e0.elapsed_time(e1), "iterations": fi["iterations"],
+                "full_lattice_rel_resid": fi["true_rel_resid"]}
+        del bo
     # ---- row f2: the same Dslash and solve with compressed Naik links (13 instead of 18 reals per Naik link) ----
     comp = None
     if not args.no_compression:
@@ -397,6 +411,7 @@ def main():
                "true_rel_resid": info["true_rel_resid"], "ms_per_iteration": ms_all / args.steps / max(info["iterations"], 1)},
         "dslash": dsl,
         "multishift_cg": ms,
+        "full_system_solve": full,
         "partitioned_cg": part,
         "naik_compression": comp,
         "roofline": {"bound": "hbm", "kernel": f"dslash_kernel<{'float' if w == 4 else 'double'},NR={min(n, 8 if w == 4 else 4)}>",
