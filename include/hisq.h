@@ -127,6 +127,23 @@ int hisq_cg_multishift(hisq_ctx *h, void *x, const void *b, double mass, const d
 int hisq_solve_M(hisq_ctx *h, void *x_even, void *x_odd, const void *b_even, const void *b_odd, double mass, double tol,
                  int nrhs);
 
+/* HISQ link smearing ("X and W are smeared gauge fields"; HISQ action):
+ * from the thin gauge links U build the two link fields hisq_set_links takes,
+ *     V = F7[U]  (fat7: weights 1/8, 1/16, 1/64, 1/384 for the 1-, 3-, 5-, 7-link paths)
+ *     W = V (V^+ V)^(-1/2)                              (projection to U(3))
+ *     fat  = fat_scale  * eta_mu(x) * F7L[W]            (fat7 with one-link weight 1 plus the Lepage term, weight -1/8)
+ *     naik = naik_scale * eta_mu(x) * W_mu(x) W_mu(x+mu) W_mu(x+2mu)
+ * eta_mu(x) = 1, (-1)^x, (-1)^(x+y), (-1)^(x+y+z) if fold_phases != 0, else 1.  With fat_scale = 1 and
+ * naik_scale = -1/24 the free-field operator is 2 i sum_mu eta_mu (9/8 sin p - 1/24 sin 3p) = 2 i (p + O(p^5)); halve
+ * both for the conventionally normalised derivative.  The gauge field is periodic.
+ * thin, fat, naik, scratch: CANONICAL link arrays (4*V matrices each, Eq. (5)) in the context's element type, pairwise
+ * non-overlapping; scratch needs hisq_smear_bytes(h) bytes (it holds W on return).  Needs a workspace (one counter).
+ * Synchronises the stream.  HISQ_EBREAKDOWN if a level-1 link is singular (no unitary factor); partitioned contexts:
+ * HISQ_EINVAL. */
+size_t hisq_smear_bytes(const hisq_ctx *h);
+int hisq_smear(hisq_ctx *h, const void *thin, void *fat, void *naik, void *scratch, double fat_scale, double naik_scale,
+               int fold_phases);
+
 /* Options: "max_iter" (default 100000), "reliable_interval" (default 100 for HISQ_MIXED, 0 = off for
  * the others), "check_interval" (iterations enqueued between host polls of the convergence flag,
  * default 32), "use_graph" (1: replay one CG iteration as a CUDA graph, default 1),

@@ -24,7 +24,7 @@ LIB_PATH = os.environ.get("HISQ_LIB", os.path.join(_HERE, "libhisq.so"))
 
 EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
-    "hisq_set_links", "hisq_dslash", "hisq_apply_A", "hisq_solve_M", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
+    "hisq_set_links", "hisq_dslash", "hisq_apply_A", "hisq_solve_M", "hisq_smear_bytes", "hisq_smear", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
     "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count",
     "hisq_create_part", "hisq_peer_bytes", "hisq_peer_attach", "hisq_halo_send", "hisq_halo_recv", "hisq_peer_reduce_send", "hisq_peer_reduce_recv", "hisq_dslash_slices", "hisq_dslash_edges", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
     "hisq_cgp_begin", "hisq_cgp_phase", "hisq_cgp_ptr", "hisq_cgp_status", "hisq_strerror",
@@ -63,6 +63,9 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_cg.argtypes = [vp, vp, vp, d, d, i]
     lib.hisq_apply_A.argtypes = [vp, vp, vp, d, i]
     lib.hisq_solve_M.argtypes = [vp, vp, vp, vp, vp, d, d, i]
+    lib.hisq_smear_bytes.argtypes = [vp]
+    lib.hisq_smear_bytes.restype = sz
+    lib.hisq_smear.argtypes = [vp, vp, vp, vp, vp, d, d, i]
     lib.hisq_cg_multishift.argtypes = [vp, vp, vp, d, ctypes.POINTER(d), i, d]
     lib.hisq_set_option.argtypes = [vp, ctypes.c_char_p, d]
     lib.hisq_get_info.argtypes = [vp, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(d)]
@@ -255,6 +258,18 @@ class Hisq:
         self._check(code, allow=() if strict else (HISQ_ENOCONV, HISQ_EBREAKDOWN))
         return xe, xo, self.info(n, code)
 
+    def smear(self, thin: torch.Tensor, fat_scale: float = 1.0, naik_scale: float = -1.0 / 24.0, fold_phases: bool = True):
+        """HISQ smearing of canonical thin links [4, V, 3, 3] -> (fat, naik, W), all canonical, ready for set_links."""
+        V = 2 * self.Vh
+        shp = (4, V, 3, 3)
+        fat, naik = torch.empty_like(thin), torch.empty_like(thin)
+        nbytes = self.lib.hisq_smear_bytes(self._h)
+        scratch = torch.empty(nbytes // thin.element_size(), dtype=thin.dtype, device=thin.device)
+        self._check(self.lib.hisq_smear(self._h, self._ptr(thin, shp, self.cdtype), self._ptr(fat, shp, self.cdtype),
+                                        self._ptr(naik, shp, self.cdtype), scratch.data_ptr(), float(fat_scale),
+                                        float(naik_scale), int(bool(fold_phases))))
+        return fat, naik, scratch[: 4 * V * 9].view(shp)
+
     def cg_multishift(self, b: torch.Tensor, mass: float, shifts, tol: float, x: Optional[torch.Tensor] = None,
                       strict: bool = True):
         """(mass^2 + shifts[k] - D_eo D_oe) x_k = b; b: [1, 3, Vh]; returns (x [nshift, 3, Vh], info)."""
@@ -385,6 +400,14 @@ def make_links(L, seed: int, device, cdtype=torch.complex128, gen_device=None):
     fat = inputs.fat_links(L, seed, sites).permute(1, 0, 2, 3).to(cdtype).contiguous().to(device)
     naik = inputs.naik_links(L, seed, sites).permute(1, 0, 2, 3).to(cdtype).contiguous().to(device)
     return fat, naik
+
+
+def make_thin_links(L, seed: int, device, cdtype=torch.complex128, spread: float = 0.0, gen_device=None):
+    """Thin SU(3) links, canonical [4, V, 3, 3] (inputs.thin_links)."""
+    from . import inputs
+    gdev = torch.device(gen_device) if gen_device is not None else torch.device("cpu")
+    sites = layout.lex_of_eo(L, device=gdev)
+    return inputs.thin_links(L, seed, sites, spread).permute(1, 0, 2, 3).to(cdtype).contiguous().to(device)
 
 
 def make_sources(L, seed: int, nrhs: int, parity: int, device, cdtype=torch.complex128, gen_device=None):

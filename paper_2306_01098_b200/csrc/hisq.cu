@@ -13,6 +13,7 @@
 
 #include "blas.cuh"
 #include "dslash_launch.cuh"
+#include "smear.cuh"
 
 using namespace hisq;
 
@@ -884,6 +885,101 @@ extern "C" int hisq_solve_M(hisq_ctx* h, void* x_even, void* x_odd, const void* 
     if (h->prec == HISQ_FP32)
         return solve_M_impl<float>(h, h->links32, (float*)x_even, (float*)x_odd, (const float*)b_even, (const float*)b_odd, mass, tol, nrhs);
     return solve_M_impl<double>(h, h->links64, (double*)x_even, (double*)x_odd, (const double*)b_even, (const double*)b_odd, mass, tol, nrhs);
+}
+
+// ---- HISQ link smearing (row f4): thin links -> fat and Naik links, canonical layout in and out ----------------------
+struct SmearCoeff { double c1, c3, c5, c7, cL; };
+
+// out (4V matrices) = smeared `in` (4V); A, B, C: V matrices of scratch each
+template <typename T>
+static int smear_level(hisq_ctx* h, const T* in, T* out, T* A, T* B, T* C, const SmearCoeff& k)
+{
+    const Geom& g = h->g;
+    const size_t V = (size_t)2 * g.Vh, mat = 18;
+    const unsigned grid = (unsigned)((V + 127) / 128);
+    for (int mu = 0; mu < 4; ++mu) {
+        const T* Umu = in + (size_t)mu * V * mat;
+        T* acc = out + (size_t)mu * V * mat;
+        smear_init_kernel<T><<<(unsigned)std::min<size_t>((V * mat + 127) / 128, (size_t)h->num_sms * 32), 128, 0, h->stream>>>(acc, Umu, V * mat, (T)k.c1);
+        h->stats.launches++;
+        for (int nu = 0; nu < 4; ++nu) {
+            if (nu == mu) continue;
+            // S3_nu: up part -> A, down part -> B
+            staple_kernel<T><<<grid, 128, 0, h->stream>>>(g, in, Umu, Umu, nullptr, A, B, acc, mu, nu, (T)k.c3);
+            h->stats.launches++;
+            if (k.cL != 0.0) {   // Lepage: the straight two-step staples only (up of up, down of down)
+                staple_kernel<T><<<grid, 128, 0, h->stream>>>(g, in, A, B, nullptr, nullptr, nullptr, acc, mu, nu, (T)k.cL);
+                h->stats.launches++;
+            }
+            for (int rho = 0; rho < 4; ++rho) {
+                if (rho == mu || rho == nu) continue;
+                // S5_nu,rho = G_rho[A + B] -> C
+                staple_kernel<T><<<grid, 128, 0, h->stream>>>(g, in, A, A, B, C, C, acc, mu, rho, (T)k.c5);
+                h->stats.launches++;
+                const int sig = 6 - mu - nu - rho;
+                staple_kernel<T><<<grid, 128, 0, h->stream>>>(g, in, C, C, nullptr, nullptr, nullptr, acc, mu, sig, (T)k.c7);
+                h->stats.launches++;
+            }
+        }
+    }
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+
+template <typename T>
+static int smear_impl(hisq_ctx* h, const T* thin, T* fat, T* naik, T* W, double fat_scale, double naik_scale, int fold)
+{
+    const Geom& g = h->g;
+    const size_t V = (size_t)2 * g.Vh;
+    // the Naik output doubles as the three staple fields until the very end
+    T* A = naik; T* B = naik + V * 18; T* C = naik + 2 * V * 18;
+    const SmearCoeff fat7 = { 1.0 / 8.0, 1.0 / 16.0, 1.0 / 64.0, 1.0 / 384.0, 0.0 };
+    const SmearCoeff fat7L = { 1.0, 1.0 / 16.0, 1.0 / 64.0, 1.0 / 384.0, -1.0 / 8.0 };
+    int rc = smear_level<T>(h, thin, W, A, B, C, fat7);
+    if (rc) return rc;
+    unsigned long long* bad = h->bad_count;
+    CK(cudaMemsetAsync(bad, 0, sizeof(unsigned long long), h->stream));
+    project_u3_kernel<T><<<(unsigned)((4 * V + 127) / 128), 128, 0, h->stream>>>(W, 4 * V, bad);
+    h->stats.launches++;
+    rc = smear_level<T>(h, W, fat, A, B, C, fat7L);
+    if (rc) return rc;
+    const dim3 gl((unsigned)((V + 127) / 128), 4);
+    fold_kernel<T><<<gl, 128, 0, h->stream>>>(g, fat, (T)fat_scale, fold);
+    naik_kernel<T><<<gl, 128, 0, h->stream>>>(g, W, naik, (T)naik_scale, fold);
+    h->stats.launches += 2;
+    CK(cudaGetLastError());
+    unsigned long long nbad = 0;
+    CK(cudaMemcpyAsync(&nbad, bad, sizeof(nbad), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    if (nbad) {
+        h->last_error = "hisq_smear: " + std::to_string(nbad) + " level-1 links are singular or not finite (no unitary projection)";
+        return HISQ_EBREAKDOWN;
+    }
+    return HISQ_OK;
+}
+
+extern "C" size_t hisq_smear_bytes(const hisq_ctx* h)
+{
+    if (!h) return 0;
+    return align_up((size_t)4 * 2 * h->g.Vh * 18 * elem_size(h->prec));
+}
+
+extern "C" int hisq_smear(hisq_ctx* h, const void* thin, void* fat, void* naik, void* scratch, double fat_scale, double naik_scale,
+                          int fold_phases)
+{
+    if (!h || !thin || !fat || !naik || !scratch || !std::isfinite(fat_scale) || !std::isfinite(naik_scale)) return HISQ_EINVAL;
+    const void* ptr[4] = { thin, fat, naik, scratch };
+    const size_t bytes = (size_t)4 * 2 * h->g.Vh * 18 * elem_size(h->prec);
+    for (int i = 0; i < 4; ++i) {
+        if ((uintptr_t)ptr[i] & 15) return HISQ_EINVAL;
+        for (int j = i + 1; j < 4; ++j)
+            if (overlap(ptr[i], ptr[j], bytes)) return HISQ_EINVAL;
+    }
+    if (h->g.part) return HISQ_EINVAL;
+    if (!h->ws) return HISQ_ENOWORKSPACE;   // the non-convergence counter lives there
+    if (h->prec == HISQ_FP32)
+        return smear_impl<float>(h, (const float*)thin, (float*)fat, (float*)naik, (float*)scratch, fat_scale, naik_scale, fold_phases);
+    return smear_impl<double>(h, (const double*)thin, (double*)fat, (double*)naik, (double*)scratch, fat_scale, naik_scale, fold_phases);
 }
 
 // ---- options / info ----------------------------------------------------------------------------------

@@ -172,6 +172,22 @@ def naik_links(L, seed: int, sites: torch.Tensor, fold_phases: bool = True,
     return out
 
 
+def thin_links(L, seed: int, sites: torch.Tensor, spread: float = 0.0, chunk: int = 1 << 18) -> torch.Tensor:
+    """Thin gauge links U_mu(x) in SU(3) for the smearing (row f4): spread = 0: Haar-random (a "hot" configuration);
+    spread > 0: Gram-Schmidt of 1 + spread * (complex Gaussian matrix), i.e. links scattered around the identity like
+    those of a thermalised configuration (stand-in: no gauge configurations here).  complex128 [len(sites), 4, 3, 3]."""
+    if spread == 0.0:
+        return naik_links(L, seed, sites, fold_phases=False, coeff=1.0, chunk=chunk)
+    out = torch.empty((sites.numel(), 4, 3, 3), dtype=torch.complex128, device=sites.device)
+    mu = torch.arange(4, dtype=torch.int64, device=sites.device)
+    eye = torch.eye(3, dtype=torch.complex128, device=sites.device)
+    for a, b in _chunks(sites.numel(), chunk):
+        base = sites[a:b].unsqueeze(-1) * 4 + mu
+        g = _complex_gauss(seed, STREAM_NAIK, base, 9).reshape(b - a, 4, 3, 3)
+        out[a:b] = _su3_from_gaussian(eye + spread * g)
+    return out
+
+
 def gauge_transform(L, seed: int, sites: torch.Tensor, chunk: int = 1 << 18) -> torch.Tensor:
     """Random g(x) in SU(3) for gauge-covariance checks: complex128 [len(sites), 3, 3]."""
     out = torch.empty((sites.numel(), 3, 3), dtype=torch.complex128, device=sites.device)
