@@ -330,6 +330,21 @@ def main():
                 "solve_ms": e0.elapsed_time(e1), "iterations": fi["iterations"],
                 "full_lattice_rel_resid": fi["true_rel_resid"]}
         del bo
+    # ---- row f4: HISQ smearing of seeded thin links on the same lattice (set-up work: time and launches, context) ----
+    smear = None
+    if not args.no_multishift and rank == 0:
+        thin = binding.make_thin_links(L, rank, dev, ctx.cdtype, 0.3, gen_device=gen_dev)
+        ctx.smear(thin)
+        torch.cuda.synchronize()
+        l0 = ctx.launch_count()
+        e0.record()
+        ctx.smear(thin)
+        e1.record()
+        e1.synchronize()
+        smear = {"what": "hisq_smear: fat7 -> U(3) projection -> fat7 + Lepage, Naik product, phases folded (canonical layout)",
+                 "ms": e0.elapsed_time(e1), "launches": int(ctx.launch_count() - l0),
+                 "thin_links": "Gram-Schmidt of 1 + 0.3 x Gaussian (seeded stand-in for a thermalised configuration)"}
+        del thin
     # ---- row f2: the same Dslash and solve with compressed Naik links (13 instead of 18 reals per Naik link) ----
     comp = None
     if not args.no_compression:
@@ -412,6 +427,7 @@ def main():
         "dslash": dsl,
         "multishift_cg": ms,
         "full_system_solve": full,
+        "link_smearing": smear,
         "partitioned_cg": part,
         "naik_compression": comp,
         "roofline": {"bound": "hbm", "kernel": f"dslash_kernel<{'float' if w == 4 else 'double'},NR={min(n, 8 if w == 4 else 4)}>",

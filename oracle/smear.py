@@ -23,6 +23,9 @@ The gauge field is periodic in all four directions.
 
 Storage: U[lex, mu, a, b] complex128 with lex = x + Lx*(y + Ly*(z + Lz*t)), like the rest of the oracle.
 Everything is numpy on whole-lattice arrays; np.linalg.eigh is the library primitive of the projection.
+
+Parity unpinned in one respect: that THIS is the construction the paper's code uses is a reading (R26), the paper prints
+no formula for it.  The functions themselves are pinned (S1-S7).
 """
 from __future__ import annotations
 
