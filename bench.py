@@ -202,8 +202,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
-    ap.add_argument("--only", default="all", choices=["all", "dslash"],
-                    help="dslash: time only the Dslash kernel of --config at --nrhs (profiling driver)")
+    ap.add_argument("--only", default="all", choices=["all", "dslash", "smear"],
+                    help="dslash: time only the Dslash kernel of --config at --nrhs; smear: only hisq_smear on --config's "
+                         "lattice (profiling drivers)")
     ap.add_argument("--nrhs", type=int, default=0, help="override the config's nRHS (--only dslash)")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -223,6 +224,8 @@ def main():
         return run_reference(args, cfg, rank, world)
     if args.only == "dslash":
         return run_dslash_only(args, cfg)
+    if args.only == "smear":
+        return run_smear_only(args, cfg)
     if args.config == "C3":
         raise SystemExit("C3 is a Dslash-only config: use --only dslash")
 
@@ -453,6 +456,30 @@ def main():
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
+
+
+def run_smear_only(args, cfg):
+    """Profiling driver: HISQ smearing of seeded thin links on one config's lattice (ncu -k regex:staple_kernel ...)."""
+    from paper_2306_01098_b200 import binding
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    L = cfg["L"]
+    prec = "fp64" if cfg["prec"] == "mixed" else cfg["prec"]
+    ctx = binding.Hisq(L, prec, 1, dev)
+    thin = binding.make_thin_links(L, 0, dev, ctx.cdtype, 0.3, gen_device=dev)
+    ctx.smear(thin)
+    torch.cuda.synchronize()
+    l0 = ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = max(1, args.steps)
+    e0.record()
+    for _ in range(reps):
+        ctx.smear(thin)
+    e1.record()
+    e1.synchronize()
+    print(json.dumps({"only": "smear", "config": args.config, "L": L, "prec": prec, "ms": e0.elapsed_time(e1) / reps,
+                      "launches_per_smearing": int((ctx.launch_count() - l0) // reps)}))
+    ctx.close()
 
 
 def run_dslash_only(args, cfg):
