@@ -78,3 +78,28 @@ def test_solve_M_even_source_reduces_to_cg_and_rejects_bad_arguments():
     two = [torch.zeros(2, 3, ctx.Vh, dtype=ctx.cdtype, device=ctx.device) for _ in range(4)]
     assert lib.hisq_solve_M(ctx._h, *[p(t) for t in two], m, tol, 2) == binding.HISQ_ENOWORKSPACE        # sized for 1
     ctx.close()
+
+
+def test_thin_links_to_propagator_pipeline():
+    """The whole chain a user runs: thin SU(3) links -> hisq_smear -> hisq_set_links -> hisq_solve_M, judged by the oracle's
+    M = D + m built from the ORACLE's smeared links (oracle/smear.py), i.e. two independent implementations end to end."""
+    from oracle import smear as osmear
+    from paper_2306_01098_b200 import inputs
+    L, seed, m, tol = (8, 8, 8, 8), 21, 0.05, 1e-9
+    ctx = binding.Hisq(L, "fp64", 2)
+    thin = binding.make_thin_links(L, seed, ctx.device, ctx.cdtype, 0.3)
+    fat, naik, _ = ctx.smear(thin, fat_scale=0.5, naik_scale=-0.5 / 24.0)
+    ctx.set_links(fat, naik)
+    U = inputs.thin_links(L, seed, torch.arange(inputs.volume(L), dtype=torch.int64), 0.3).numpy()
+    Xo, No, _ = osmear.hisq_links(L, U, fat_scale=0.5, naik_scale=-0.5 / 24.0)
+    be_dev, be_full = make_field(ctx, L, seed, 2, 0)
+    bo_dev, bo_full = make_field(ctx, L, seed, 2, 1)
+    b_full = be_full + bo_full
+    xe, xo, info = ctx.solve_M(be_dev, bo_dev, m, tol)
+    x = to_full(ctx, L, xe, 0) + to_full(ctx, L, xo, 1)
+    r = b_full - oracle.apply_M(L, Xo, No, m, x)
+    for k in range(2):
+        assert np.linalg.norm(r[k]) <= tol * np.linalg.norm(b_full[k]) * 1.001
+    # smeared links are close to unitary x 9/8 * 1/2: the spectrum of D is bounded by ~ 4 (9/8 + 1/24), so the solve is short
+    assert 10 < info["iterations"] < 2000
+    ctx.close()
