@@ -55,7 +55,8 @@ enum {
     HISQ_ENOWORKSPACE = -3, /* no workspace set, or it is smaller than hisq_workspace_bytes(nrhs)          */
     HISQ_ECUDA = -4,        /* a CUDA call failed; text via hisq_last_error                                */
     HISQ_ENOCONV = -5,      /* max_iter reached; x holds the last iterate, hisq_get_info the residuals     */
-    HISQ_EBREAKDOWN = -6    /* <p, A p> <= 0 or a non-finite scalar appeared in CG                         */
+    HISQ_EBREAKDOWN = -6,   /* <p, A p> <= 0 or a non-finite scalar appeared in CG                         */
+    HISQ_EIO = -7           /* file cannot be opened / is truncated / fails its checksum or link trace     */
 };
 
 /* Create a context for an Lx x Ly x Lz x Lt lattice on the current CUDA device.
@@ -143,6 +144,21 @@ int hisq_solve_M(hisq_ctx *h, void *x_even, void *x_odd, const void *b_even, con
 size_t hisq_smear_bytes(const hisq_ctx *h);
 int hisq_smear(hisq_ctx *h, const void *thin, void *fat, void *naik, void *scratch, double fat_scale, double naik_scale,
                int fold_phases);
+
+/* Gauge configurations in the NERSC archive format (PAPER.md:540 lists the formats the paper's code
+ * reads: ILDG, MILC, NERSC, openQCD -- only NERSC is built here).  HOST functions, no context, no CUDA: text header
+ * (DATATYPE = 4D_SU3_GAUGE_3x3 | 4D_SU3_GAUGE, DIMENSION_1..4, FLOATING_POINT = IEEE64BIG | IEEE32BIG | IEEE64LITTLE |
+ * IEEE32LITTLE, CHECKSUM, LINK_TRACE, PLAQUETTE) followed by the links in lexicographic site order (x fastest), mu = 0..3
+ * per site, row-major matrices; the two-row type is completed with row 2 = conj(row0 x row1).
+ * hisq_nersc_info: header only (any output pointer may be NULL; rows = 2 | 3, real_bytes = 4 | 8).
+ * hisq_nersc_read: links_host (HOST, `bytes` >= 4*V*9 complex double) receives the CANONICAL link array (Eq. (5)) as
+ *   complex double -- copy it to the device (convert for an fp32 context) and pass it to hisq_smear.  Verifies the
+ *   32-bit checksum and the link trace of the header: HISQ_EIO if either fails, the file is short or cannot be opened;
+ *   HISQ_EINVAL for a malformed header or extents the library does not take (odd or < 4).
+ * hisq_nersc_write: the inverse (IEEE64BIG, rows = 2 | 3; `plaquette` goes into the header as given). */
+int hisq_nersc_info(const char *path, int *L, int *rows, int *real_bytes, double *link_trace, double *plaquette);
+int hisq_nersc_read(const char *path, void *links_host, size_t bytes);
+int hisq_nersc_write(const char *path, const void *links_host, const int *L, int rows, double plaquette);
 
 /* Options: "max_iter" (default 100000), "reliable_interval" (default 100 for HISQ_MIXED, 0 = off for
  * the others), "check_interval" (iterations enqueued between host polls of the convergence flag,

@@ -17,14 +17,14 @@ HISQ_FP32, HISQ_FP64, HISQ_MIXED = 4, 8, 12
 HISQ_EVEN, HISQ_ODD = 0, 1
 HISQ_MAX_NRHS = 16
 HISQ_EINVAL, HISQ_ENOLINKS, HISQ_ENOWORKSPACE, HISQ_ECUDA = -1, -2, -3, -4
-HISQ_ENOCONV, HISQ_EBREAKDOWN = -5, -6
+HISQ_ENOCONV, HISQ_EBREAKDOWN, HISQ_EIO = -5, -6, -7
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("HISQ_LIB", os.path.join(_HERE, "libhisq.so"))
 
 EXPORTS = [
     "hisq_create", "hisq_destroy", "hisq_set_stream", "hisq_workspace_bytes", "hisq_set_workspace",
-    "hisq_set_links", "hisq_dslash", "hisq_apply_A", "hisq_solve_M", "hisq_smear_bytes", "hisq_smear", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
+    "hisq_set_links", "hisq_dslash", "hisq_apply_A", "hisq_solve_M", "hisq_smear_bytes", "hisq_smear", "hisq_nersc_info", "hisq_nersc_read", "hisq_nersc_write", "hisq_cg", "hisq_cg_multishift", "hisq_set_option", "hisq_get_info", "hisq_spinor_pack",
     "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count",
     "hisq_create_part", "hisq_peer_bytes", "hisq_peer_attach", "hisq_halo_send", "hisq_halo_recv", "hisq_peer_reduce_send", "hisq_peer_reduce_recv", "hisq_dslash_slices", "hisq_dslash_edges", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
     "hisq_cgp_begin", "hisq_cgp_phase", "hisq_cgp_ptr", "hisq_cgp_status", "hisq_strerror",
@@ -63,6 +63,9 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_cg.argtypes = [vp, vp, vp, d, d, i]
     lib.hisq_apply_A.argtypes = [vp, vp, vp, d, i]
     lib.hisq_solve_M.argtypes = [vp, vp, vp, vp, vp, d, d, i]
+    lib.hisq_nersc_info.argtypes = [ctypes.c_char_p, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(d), ctypes.POINTER(d)]
+    lib.hisq_nersc_read.argtypes = [ctypes.c_char_p, vp, sz]
+    lib.hisq_nersc_write.argtypes = [ctypes.c_char_p, vp, ctypes.POINTER(i), i, d]
     lib.hisq_smear_bytes.argtypes = [vp]
     lib.hisq_smear_bytes.restype = sz
     lib.hisq_smear.argtypes = [vp, vp, vp, vp, vp, d, d, i]
@@ -400,6 +403,41 @@ def make_links(L, seed: int, device, cdtype=torch.complex128, gen_device=None):
     fat = inputs.fat_links(L, seed, sites).permute(1, 0, 2, 3).to(cdtype).contiguous().to(device)
     naik = inputs.naik_links(L, seed, sites).permute(1, 0, 2, 3).to(cdtype).contiguous().to(device)
     return fat, naik
+
+
+def nersc_info(path: str) -> dict:
+    """Header of a NERSC-format configuration: L, rows (2 | 3), real_bytes, link_trace, plaquette."""
+    lib = load_library()
+    L = (ctypes.c_int * 4)()
+    rows, rb = ctypes.c_int(0), ctypes.c_int(0)
+    lt, pl = ctypes.c_double(0), ctypes.c_double(0)
+    code = lib.hisq_nersc_info(path.encode(), L, ctypes.byref(rows), ctypes.byref(rb), ctypes.byref(lt), ctypes.byref(pl))
+    if code:
+        raise HisqError(code, lib.hisq_strerror(code).decode())
+    return {"L": tuple(L), "rows": rows.value, "real_bytes": rb.value, "link_trace": lt.value, "plaquette": pl.value}
+
+
+def nersc_read(path: str) -> torch.Tensor:
+    """A NERSC-format configuration as canonical thin links [4, V, 3, 3] complex128 on the HOST (checksum and link
+    trace verified by the library)."""
+    lib = load_library()
+    L = nersc_info(path)["L"]
+    V = L[0] * L[1] * L[2] * L[3]
+    out = torch.empty((4, V, 3, 3), dtype=torch.complex128)
+    code = lib.hisq_nersc_read(path.encode(), ctypes.c_void_p(out.data_ptr()), out.numel() * 16)
+    if code:
+        raise HisqError(code, lib.hisq_strerror(code).decode())
+    return out
+
+
+def nersc_write(path: str, links: torch.Tensor, L, rows: int = 3, plaquette: float = 0.0) -> None:
+    """Canonical links [4, V, 3, 3] complex128 (host) -> NERSC file (IEEE64BIG)."""
+    lib = load_library()
+    links = links.to(torch.complex128).cpu().contiguous()
+    code = lib.hisq_nersc_write(path.encode(), ctypes.c_void_p(links.data_ptr()), (ctypes.c_int * 4)(*[int(v) for v in L]), int(rows),
+                                float(plaquette))
+    if code:
+        raise HisqError(code, lib.hisq_strerror(code).decode())
 
 
 def make_thin_links(L, seed: int, device, cdtype=torch.complex128, spread: float = 0.0, gen_device=None):

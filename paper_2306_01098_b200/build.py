@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libhisq.so")
-SOURCES = ["hisq.cu", "dslash_f32.cu", "dslash_f64.cu"]
+SOURCES = ["hisq.cu", "dslash_f32.cu", "dslash_f64.cu", "nersc_io.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 
@@ -33,7 +33,7 @@ def build(force: bool = False, verbose: bool = False, defines=(), lib: str = LIB
     nvcc = os.environ.get("NVCC", "nvcc")
 
     def compile_one(src: str) -> str:
-        obj = os.path.join(obj_dir, src.replace(".cu", ".o"))
+        obj = os.path.join(obj_dir, os.path.splitext(src)[0] + ".o")
         cmd = [nvcc, *NVCC_FLAGS, *defines, "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd[1:1] = ["-Xptxas", "-v"]

@@ -103,3 +103,19 @@ def test_smear_full_size_lattice_tiled_configuration():
         ref_big = ref[small].transpose(1, 0, 2, 3)
         assert rel_l2(got.cpu().numpy(), ref_big) <= 1e-13
     ctx.close()
+
+
+def test_configuration_file_to_smeared_links(tmp_path):
+    """NERSC file -> hisq_nersc_read (host) -> device -> hisq_smear: the same bits as smearing the links directly."""
+    L = (4, 6, 4, 8)
+    ctx = binding.Hisq(L, "fp64", 1)
+    thin = binding.make_thin_links(L, 14, ctx.device, ctx.cdtype, 0.3)
+    path = str(tmp_path / "cfg.nersc")
+    binding.nersc_write(path, thin, L, rows=3)
+    assert binding.nersc_info(path)["L"] == L
+    again = binding.nersc_read(path).to(ctx.device)
+    assert torch.equal(again, thin)
+    a, b = ctx.smear(thin), ctx.smear(again)
+    for u, v in zip(a, b):
+        assert torch.equal(u, v)
+    ctx.close()
