@@ -348,7 +348,7 @@ def main():
                  "ms": e0.elapsed_time(e1), "launches": int(ctx.launch_count() - l0),
                  "thin_links": "Gram-Schmidt of 1 + 0.3 x Gaussian (seeded stand-in for a thermalised configuration)"}
         del thin
-    # ---- row f2: the same Dslash and solve with compressed Naik links (13 instead of 18 reals per Naik link) ----
+    # ---- row f2: the same Dslash and solve with compressed Naik links (14 instead of 18 reals per Naik link) ----
     comp = None
     if not args.no_compression:
         ctx.close()
@@ -365,8 +365,8 @@ def main():
             _, ci = ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
             e1.record()
             e1.synchronize()
-            stored = (8 * 18 + 8 * 13 + 12 * n) * w * Vh
-            comp = {"format": "Naik links as 13 reals (rows 0,1 and 1/c), fat links 18", "dslash_ms": c_ms,
+            stored = (8 * 18 + 8 * 14 + 12 * n) * w * Vh
+            comp = {"format": "Naik links as 14 reals (rows 0,1 and d = det/|row0 x row1|^2; exact for c x U(3)), fat links 18", "dslash_ms": c_ms,
                     "dslash_gflops": FLOP_PER_SITE * Vh * n / (c_ms * 1e-3) / 1e9,
                     "stored_bytes_per_launch": stored, "stored_gbs": stored / (c_ms * 1e-3) / 1e9,
                     "uncompressed_alg_gbs": alg_bytes / (c_ms * 1e-3) / 1e9, "speedup_vs_full": d_ms / c_ms,

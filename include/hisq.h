@@ -273,9 +273,11 @@ void *hisq_cgp_ptr(hisq_ctx *h, int which);
 int hisq_cgp_status(hisq_ctx *h, int *iterations, int *done, int *breakdown, double *rel_resid);
 
 /* Row f2 (the paper's CompressionType).  With option "naik_compress" = 1, the next hisq_set_links
- * stores each Naik link as 13 reals (rows 0, 1 and 1/c of W = c U, U in SU(3), c real; row 2 = conj(row0 x row1)/c is
- * rebuilt in registers) PROVIDED every Naik link passes |row2 - conj(row0 x row1)/c| <= tol |c| (tol 1e-12 fp64, 1e-5
- * fp32); otherwise the links stay uncompressed.  Returns 1 if the context currently uses the compressed format. */
+ * stores each Naik link as 14 reals: rows 0, 1 and the complex number d = det(W) / |row0 x row1|^2, from which
+ * row 2 = conj(row0 x row1) d is rebuilt in registers.  That is exact for W = c U with c real and U in U(3) (d = det(U)/c):
+ * the U(3)-projected Naik links hisq_smear produces as well as real multiples of SU(3) matrices.  The format is used
+ * PROVIDED every Naik link passes |row2 - conj(row0 x row1) d| <= tol |row0| (tol 1e-12 fp64, 1e-5 fp32); otherwise the
+ * links stay uncompressed.  Returns 1 if the context currently uses the compressed format. */
 int hisq_naik_compressed(const hisq_ctx *h);
 
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches). */

@@ -579,11 +579,33 @@ __global__ void __launch_bounds__(256) link_repack_kernel(const TS* __restrict__
 }
 
 // ---- Naik-link compression (row f2; the paper's `CompressionType comp`) -----------------
-// A Naik link of the HISQ action is a real multiple of an SU(3) matrix, W = c U (here c = -eta/24).  Store rows 0
-// and 1 (12 reals) and 1/c (1 real): row 2 = conj(row0 x row1) / c.  13 instead of 18 reals per Naik link.
-// Layout inside the (unchanged) 18-real block: fp64: 6 planes of double2 then 1 plane of double;
-// fp32: 3 planes of float4 then 1 plane of float.  `bad` counts links whose row 2 is NOT reproduced to `tol`
-// (relative to |c|): the caller then falls back to the uncompressed format.
+// A Naik link of the HISQ action is a real multiple of a unitary matrix, W = c U: U in U(3) after the smearing's
+// projection (section 7c), in SU(3) for the BASELINE inputs (c = -eta/24).  Store rows 0 and 1 (12 reals) and the complex
+// number d = det(W) / |row0 x row1|^2 (= det(U) / c): row 2 = conj(row0 x row1) d.  14 instead of 18 reals per Naik link.
+// Layout inside the (unchanged) 18-real block: fp64: 7 planes of double2; fp32: 3 planes of float4 then 1 plane of
+// float2.  `bad` counts links whose row 2 is NOT reproduced to `tol` (relative to |row 0|): the caller then falls back
+// to the uncompressed format.
+// d = det(W) / |row0 x row1|^2 and the largest deviation of conj(row0 x row1) d from the stored row 2
+__device__ __forceinline__ double naik_row2_deviation(const double (&e)[18], double& dr, double& di)
+{
+    double cr[6], det_re = 0.0, det_im = 0.0, c2 = 0.0;   // cr = row0 x row1
+    for (int a = 0; a < 3; ++a) {
+        const int b = (a + 1) % 3, c = (a + 2) % 3;
+        cr[2 * a] = (e[2 * b] * e[6 + 2 * c] - e[2 * b + 1] * e[6 + 2 * c + 1]) - (e[2 * c] * e[6 + 2 * b] - e[2 * c + 1] * e[6 + 2 * b + 1]);
+        cr[2 * a + 1] = (e[2 * b] * e[6 + 2 * c + 1] + e[2 * b + 1] * e[6 + 2 * c]) - (e[2 * c] * e[6 + 2 * b + 1] + e[2 * c + 1] * e[6 + 2 * b]);
+        det_re += cr[2 * a] * e[12 + 2 * a] - cr[2 * a + 1] * e[12 + 2 * a + 1];
+        det_im += cr[2 * a] * e[12 + 2 * a + 1] + cr[2 * a + 1] * e[12 + 2 * a];
+        c2 += cr[2 * a] * cr[2 * a] + cr[2 * a + 1] * cr[2 * a + 1];
+    }
+    dr = c2 > 0.0 ? det_re / c2 : 0.0;
+    di = c2 > 0.0 ? det_im / c2 : 0.0;
+    double dev = 0.0;
+    for (int a = 0; a < 3; ++a) {   // (cr_re - i cr_im) (dr + i di)
+        dev = fmax(dev, fabs(cr[2 * a] * dr + cr[2 * a + 1] * di - e[12 + 2 * a]));
+        dev = fmax(dev, fabs(cr[2 * a] * di - cr[2 * a + 1] * dr - e[12 + 2 * a + 1]));
+    }
+    return dev;
+}
 // Dry run of the compression test on the caller's canonical array (writes nothing but the counter).
 template <typename TS>
 __global__ void __launch_bounds__(256) naik_check_kernel(const TS* __restrict__ src, int Vh, double tol, unsigned long long* bad)
@@ -596,19 +618,8 @@ __global__ void __launch_bounds__(256) naik_check_kernel(const TS* __restrict__ 
 #pragma unroll
     for (int i = 0; i < 18; ++i) e[i] = (double)s[i];
     double n0 = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2] + e[3] * e[3] + e[4] * e[4] + e[5] * e[5]);
-    double cr[6], det_re = 0.0;
-    for (int a = 0; a < 3; ++a) {
-        const int b = (a + 1) % 3, c = (a + 2) % 3;
-        cr[2 * a] = (e[2 * b] * e[6 + 2 * c] - e[2 * b + 1] * e[6 + 2 * c + 1]) - (e[2 * c] * e[6 + 2 * b] - e[2 * c + 1] * e[6 + 2 * b + 1]);
-        cr[2 * a + 1] = (e[2 * b] * e[6 + 2 * c + 1] + e[2 * b + 1] * e[6 + 2 * c]) - (e[2 * c] * e[6 + 2 * b + 1] + e[2 * c + 1] * e[6 + 2 * b]);
-        det_re += cr[2 * a] * e[12 + 2 * a] - cr[2 * a + 1] * e[12 + 2 * a + 1];
-    }
-    const double c = det_re < 0.0 ? -n0 : n0, ic = c != 0.0 ? 1.0 / c : 0.0;
-    double dev = 0.0;
-    for (int a = 0; a < 3; ++a) {
-        dev = fmax(dev, fabs(cr[2 * a] * ic - e[12 + 2 * a]));
-        dev = fmax(dev, fabs(-cr[2 * a + 1] * ic - e[12 + 2 * a + 1]));
-    }
+    double dr, di;
+    const double dev = naik_row2_deviation(e, dr, di);
     if (!(dev <= tol * n0) || n0 == 0.0) atomicAdd(bad, 1ull);
 }
 
@@ -628,25 +639,9 @@ __global__ void __launch_bounds__(256) naik_compress_kernel(const TS* __restrict
     double e[18];
 #pragma unroll
     for (int i = 0; i < 18; ++i) e[i] = (double)(TD)s[i];   // the values the kernel will see
-    // c = sign(Re det W) * |row 0|
-    double cr[6];  // row0 x row1 (complex 3-vector)
-    for (int a = 0; a < 3; ++a) {
-        const int b = (a + 1) % 3, c = (a + 2) % 3;
-        const double xr = e[2 * b], xi = e[2 * b + 1], yr = e[6 + 2 * c], yi = e[6 + 2 * c + 1];
-        const double zr = e[2 * c], zi = e[2 * c + 1], wr = e[6 + 2 * b], wi = e[6 + 2 * b + 1];
-        cr[2 * a] = (xr * yr - xi * yi) - (zr * wr - zi * wi);
-        cr[2 * a + 1] = (xr * yi + xi * yr) - (zr * wi + zi * wr);
-    }
-    double det_re = 0.0;  // Re( (row0 x row1) . row2 )
-    for (int a = 0; a < 3; ++a) det_re += cr[2 * a] * e[12 + 2 * a] - cr[2 * a + 1] * e[12 + 2 * a + 1];
     const double n0 = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2] + e[3] * e[3] + e[4] * e[4] + e[5] * e[5]);
-    const double c = det_re < 0.0 ? -n0 : n0;
-    const double ic = c != 0.0 ? 1.0 / c : 0.0;
-    double dev = 0.0;
-    for (int a = 0; a < 3; ++a) {
-        dev = fmax(dev, fabs(cr[2 * a] * ic - e[12 + 2 * a]));
-        dev = fmax(dev, fabs(-cr[2 * a + 1] * ic - e[12 + 2 * a + 1]));
-    }
+    double dr, di;
+    const double dev = naik_row2_deviation(e, dr, di);
     if (!(dev <= tol * n0) || n0 == 0.0) atomicAdd(bad, 1ull);
     if (sizeof(TD) == 8) {
 #pragma unroll
@@ -654,13 +649,15 @@ __global__ void __launch_bounds__(256) naik_compress_kernel(const TS* __restrict
             blk[((size_t)j * Vh + h) * 2] = (TD)e[2 * j];
             blk[((size_t)j * Vh + h) * 2 + 1] = (TD)e[2 * j + 1];
         }
-        blk[(size_t)12 * Vh + h] = (TD)ic;
+        blk[((size_t)6 * Vh + h) * 2] = (TD)dr;
+        blk[((size_t)6 * Vh + h) * 2 + 1] = (TD)di;
     } else {
 #pragma unroll
         for (int j = 0; j < 3; ++j)
 #pragma unroll
             for (int i = 0; i < 4; ++i) blk[((size_t)j * Vh + h) * 4 + i] = (TD)e[4 * j + i];
-        blk[(size_t)12 * Vh + h] = (TD)ic;
+        blk[(size_t)12 * Vh + (size_t)h * 2] = (TD)dr;
+        blk[(size_t)12 * Vh + (size_t)h * 2 + 1] = (TD)di;
     }
 }
 

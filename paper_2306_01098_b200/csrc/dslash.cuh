@@ -43,7 +43,7 @@ template <typename T> struct DslashArgs {
     int nchunks;         // RHS chunks of NR handled by this launch (consecutive CTAs)
     int slab_blocks;     // CTAs per (tile, t) slab and chunk
     unsigned total_blocks; // CTAs of the whole launch group (epilogue ticket)
-    int naik_c13;        // 1: Naik links are stored compressed (13 reals, row f2)
+    int naik_c14;        // 1: Naik links are stored compressed (14 reals, row f2)
     int t0, tn;          // this launch covers tn owned slices: blockIdx.y = j is slice g.t_lo + t0 + j, plus t_skip for
     PeerPush push;       // MODE_APPLY_A on a partitioned lattice: the last CTA also hands the sums to every rank's mailbox
     int t_skip_at, t_skip;  // j >= t_skip_at (two ranges in one launch: the first and last slices around an interior).
@@ -80,20 +80,23 @@ __device__ __forceinline__ void load_link(const float* blk, int Vh, int h, float
     U[16] = w.x; U[17] = w.y;
 }
 
-// Compressed Naik link (row f2): rows 0, 1 and 1/c are stored, row 2 = conj(row0 x row1) / c.
-template <typename T> __device__ __forceinline__ void reconstruct_row2(T (&U)[18], T ic)
+// Compressed Naik link (row f2): rows 0, 1 and one complex number d are stored (14 reals), row 2 = conj(row0 x row1) * d.
+// For W = c U with U in U(3) and c real, d = det(U) / c: SU(3) links (d real) and the U(3)-projected links of the
+// HISQ smearing (section 7c) are both covered.
+template <typename T> __device__ __forceinline__ void reconstruct_row2(T (&U)[18], T dr, T di)
 {
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const int b = (a + 1) % 3, c = (a + 2) % 3;
         const T re = (U[2 * b] * U[6 + 2 * c] - U[2 * b + 1] * U[6 + 2 * c + 1]) - (U[2 * c] * U[6 + 2 * b] - U[2 * c + 1] * U[6 + 2 * b + 1]);
         const T im = (U[2 * b] * U[6 + 2 * c + 1] + U[2 * b + 1] * U[6 + 2 * c]) - (U[2 * c] * U[6 + 2 * b + 1] + U[2 * c + 1] * U[6 + 2 * b]);
-        U[12 + 2 * a] = re * ic;
-        U[12 + 2 * a + 1] = -im * ic;
+        // (re - i im) (dr + i di)
+        U[12 + 2 * a] = fma(re, dr, im * di);
+        U[12 + 2 * a + 1] = fma(re, di, -(im * dr));
     }
 }
 
-__device__ __forceinline__ void load_link_c13(const double* blk, int Vh, int h, double (&U)[18])
+__device__ __forceinline__ void load_link_c14(const double* blk, int Vh, int h, double (&U)[18])
 {
     const double2* p = reinterpret_cast<const double2*>(blk) + h;
 #pragma unroll
@@ -102,11 +105,11 @@ __device__ __forceinline__ void load_link_c13(const double* blk, int Vh, int h, 
         U[2 * c] = w.x;
         U[2 * c + 1] = w.y;
     }
-    const double ic = __ldcs(blk + (size_t)12 * Vh + h);
-    reconstruct_row2(U, ic);
+    const double2 d = ld_stream(p + (size_t)6 * Vh);
+    reconstruct_row2(U, d.x, d.y);
 }
 
-__device__ __forceinline__ void load_link_c13(const float* blk, int Vh, int h, float (&U)[18])
+__device__ __forceinline__ void load_link_c14(const float* blk, int Vh, int h, float (&U)[18])
 {
     const float4* p4 = reinterpret_cast<const float4*>(blk) + h;
 #pragma unroll
@@ -114,8 +117,8 @@ __device__ __forceinline__ void load_link_c13(const float* blk, int Vh, int h, f
         float4 w = ld_stream(p4 + (size_t)j * Vh);
         U[4 * j] = w.x; U[4 * j + 1] = w.y; U[4 * j + 2] = w.z; U[4 * j + 3] = w.w;
     }
-    const float ic = __ldcs(blk + (size_t)12 * Vh + h);
-    reconstruct_row2(U, ic);
+    const float2 d = ld_stream(reinterpret_cast<const float2*>(blk + (size_t)12 * Vh) + h);
+    reconstruct_row2(U, d.x, d.y);
 }
 
 template <typename T>
@@ -209,11 +212,11 @@ template <typename T> __device__ __forceinline__ void mvdag_sub(const T (&U)[18]
 // s = -1 iff the hop crossed the t boundary (`flip`).  The gathered vectors are loaded VB at a time
 // (register budget: 18 reals of link + 6*VB of vectors live beside the 6*NR accumulators).
 template <typename T, int NR, int VB, bool FWD>
-__device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, int Vh, int hn, bool tdir, bool flip, bool c13,
+__device__ __forceinline__ void stencil_term(const T* blk, int hl, const T* in, int Vh, int hn, bool tdir, bool flip, bool c14,
                                              T (&acc)[NR][6])
 {
     T U[18];
-    if (c13) load_link_c13(blk, Vh, hl, U);
+    if (c14) load_link_c14(blk, Vh, hl, U);
     else load_link(blk, Vh, hl, U);
 #if HISQ_SIGN_BRANCH
     if (tdir && flip) {

@@ -7,7 +7,7 @@ namespace hisq {
 template <typename T, int NR, int MODE>
 static cudaError_t launch_one(const DslashArgs<T>& a, dim3 grid, cudaStream_t s)
 {
-    if (a.naik_c13) dslash_kernel<T, NR, MODE, kDslashBlock, true><<<grid, kDslashBlock, 0, s>>>(a);
+    if (a.naik_c14) dslash_kernel<T, NR, MODE, kDslashBlock, true><<<grid, kDslashBlock, 0, s>>>(a);
     else dslash_kernel<T, NR, MODE, kDslashBlock, false><<<grid, kDslashBlock, 0, s>>>(a);
     return cudaGetLastError();
 }

@@ -35,7 +35,7 @@ struct hisq_ctx {
     char* fields;          // CG temporaries
     char* stage;           // host-call staging (2 canonical + 2 native fields)
     bool have_links;
-    bool naik_c13;         // Naik links currently stored compressed
+    bool naik_c14;         // Naik links currently stored compressed
     int naik_compress;     // option: try to compress at the next hisq_set_links
     int fused_blas;        // option: cooperative fused x/r/p update for small fields
     void* cgp_x; int cgp_nrhs; double cgp_tol;   // phase-wise CG on partitioned lattices
@@ -133,7 +133,7 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     h->check_interval = 32;
     h->use_graph = 1;
     h->nrhs_inner = 0;
-    h->naik_c13 = false; h->naik_compress = 0; h->bad_count = nullptr;
+    h->naik_c14 = false; h->naik_compress = 0; h->bad_count = nullptr;
     h->fused_blas = 1; h->num_sms = 0; h->overlap_opt = -1;
     h->cgp_x = nullptr; h->cgp_nrhs = 0; h->cgp_tol = 0.0;
     { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev); }
@@ -260,7 +260,7 @@ extern "C" int hisq_set_links(hisq_ctx* h, const void* fat, const void* naik)
     const unsigned grid = (unsigned)((4 * V + 255) / 256);
     const size_t fstride = (size_t)8 * Vh * 18;  // reals per field (2 parities x 4 directions)
     const void* src[2] = { fat, naik };
-    h->naik_c13 = false;
+    h->naik_c14 = false;
     for (int f = 0; f < 2; ++f) {
         if (h->prec == HISQ_FP32) {
             link_repack_kernel<float, float><<<grid, 256, 0, h->stream>>>((const float*)src[f], h->links32 + f * fstride, Vh);
@@ -272,8 +272,8 @@ extern "C" int hisq_set_links(hisq_ctx* h, const void* fat, const void* naik)
         h->stats.launches += (h->prec == HISQ_MIXED) ? 2 : 1;
     }
     if (h->naik_compress) {
-        // row f2: try the 13-real format for the Naik links; keep it only if EVERY link is reproduced
-        // (|row2 - conj(row0 x row1)/c| <= tol |c|), otherwise the uncompressed copy written above stays
+        // row f2: try the 14-real format for the Naik links; keep it only if EVERY link is reproduced
+        // (|row2 - conj(row0 x row1) d| <= tol |row0|), otherwise the uncompressed copy written above stays
         CK(cudaMemsetAsync(h->bad_count, 0, sizeof(unsigned long long), h->stream));
         // scratch: the staging area is large enough only for small lattices, so test first, then overwrite in place
         if (h->prec == HISQ_FP32) {
@@ -294,9 +294,9 @@ extern "C" int hisq_set_links(hisq_ctx* h, const void* fat, const void* naik)
                     naik_compress_kernel<double, float><<<grid, 256, 0, h->stream>>>((const double*)naik, h->links32 + fstride, Vh, 1e-5, h->bad_count);
             }
             h->stats.launches += (h->prec == HISQ_MIXED) ? 2 : 1;
-            h->naik_c13 = true;
+            h->naik_c14 = true;
         } else {
-            h->last_error = "naik_compress: " + std::to_string(bad) + " Naik links are not a real multiple of an SU(3) matrix; stored uncompressed";
+            h->last_error = "naik_compress: " + std::to_string(bad) + " Naik links are not a real multiple of a U(3) matrix; stored uncompressed";
         }
     }
     CK(cudaGetLastError());
@@ -325,7 +325,7 @@ static int run_dslash(hisq_ctx* h, const T* links, T* out, const T* in, int pari
     a.m2 = m2;
     a.par = parity;
     a.k0 = 0; a.nrhs_total = nrhs; a.nchunks = 1; a.slab_blocks = 0; a.total_blocks = 0;
-    a.naik_c13 = h->naik_c13 ? 1 : 0;
+    a.naik_c14 = h->naik_c14 ? 1 : 0;
     a.t0 = t_first; a.tn = t_count < 0 ? h->g.t_cnt - t_first : t_count;
     a.t_skip_at = t_skip_at; a.t_skip = t_skip;
     a.push = mode == MODE_APPLY_A ? h->fuse_push_pq : PeerPush();
@@ -1479,7 +1479,7 @@ static int cgp_solve(hisq_ctx* h, void* x, const void* b, double mass, double to
     }
 }
 
-extern "C" int hisq_naik_compressed(const hisq_ctx* h) { return h && h->naik_c13 ? 1 : 0; }
+extern "C" int hisq_naik_compressed(const hisq_ctx* h) { return h && h->naik_c14 ? 1 : 0; }
 
 extern "C" long long hisq_launch_count(const hisq_ctx* h) { return h ? h->stats.launches : 0; }
 

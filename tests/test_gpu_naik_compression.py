@@ -1,5 +1,6 @@
-"""-m gpu: row f2, Naik-link compression (13 reals: rows 0, 1 and 1/c; row 2 rebuilt in registers).  Same oracle,
-same tolerances as the uncompressed kernel; links that are not c * SU(3) must fall back to the full format."""
+"""-m gpu: row f2, Naik-link compression (14 reals: rows 0, 1 and d = det / |row0 x row1|^2; row 2 = conj(row0 x row1) d
+rebuilt in registers).  Same oracle, same tolerances as the uncompressed kernel; exact for c x SU(3) (the BASELINE inputs) and
+for c x U(3) (the Naik links of the HISQ smearing); links that are neither must fall back to the full format."""
 import numpy as np
 import pytest
 import torch
@@ -79,4 +80,33 @@ def test_cg_with_compressed_links(prec):
     r = b_full - oracle.apply_A(L, X, W, m, x)
     for k in range(2):
         assert np.linalg.norm(r[k]) / np.linalg.norm(b_full[k]) <= tol
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_smeared_u3_naik_links_compress(prec):
+    """The Naik links hisq_smear makes are products of U(3)-projected links (det = a phase, not 1): the 14-real format
+    holds them exactly; the operator on the compressed links matches the oracle on the oracle's smeared links."""
+    from oracle import smear as osmear
+    from paper_2306_01098_b200 import inputs
+    L, seed = (8, 6, 4, 10), 17
+    ctx = binding.Hisq(L, prec, 2)
+    thin = binding.make_thin_links(L, seed, ctx.device, ctx.cdtype, 0.3)
+    fat, naik, W = ctx.smear(thin, fat_scale=0.5, naik_scale=-0.5 / 24.0)
+    dets = torch.linalg.det(W.reshape(-1, 3, 3))
+    assert float((dets.abs() - 1).abs().max()) < (1e-4 if prec == "fp32" else 1e-12)
+    assert float((dets - 1).abs().max()) > 1e-2                       # genuinely U(3), not SU(3)
+    ctx.set_option("naik_compress", 1)
+    ctx.set_links(fat, naik)
+    assert ctx.naik_compressed()
+    U = inputs.thin_links(L, seed, torch.arange(inputs.volume(L), dtype=torch.int64), 0.3).numpy()
+    if prec == "fp32":
+        U = U.astype(np.complex64).astype(np.complex128)
+    Xo, No, _ = osmear.hisq_links(L, U, fat_scale=0.5, naik_scale=-0.5 / 24.0)
+    for parity in (0, 1):
+        dev_in, full_in = make_field(ctx, L, seed, 2, 1 - parity)
+        got = to_full(ctx, L, ctx.dslash(dev_in, parity), parity)
+        ref = oracle.dslash_parity(L, Xo, No, full_in, parity)
+        for k in range(2):
+            assert rel_l2(got[k], ref[k]) <= (2e-5 if prec == "fp32" else 1e-12)
     ctx.close()
