@@ -138,7 +138,8 @@ int hisq_solve_M(hisq_ctx *h, void *x_even, void *x_odd, const void *b_even, con
  * naik_scale = -1/24 the free-field operator is 2 i sum_mu eta_mu (9/8 sin p - 1/24 sin 3p) = 2 i (p + O(p^5)); halve
  * both for the conventionally normalised derivative.  The gauge field is periodic.
  * thin, fat, naik, scratch: CANONICAL link arrays (4*V matrices each, Eq. (5)) in the context's element type, pairwise
- * non-overlapping; scratch needs hisq_smear_bytes(h) bytes (it holds W on return).  Needs a workspace (one counter).
+ * non-overlapping; scratch: hisq_smear_bytes(h) bytes = two link arrays (on return the SECOND holds W, canonical).  Needs a
+ * workspace (one counter).  Intermediate fields are kept structure-of-arrays inside fat / naik / scratch.
  * Synchronises the stream.  HISQ_EBREAKDOWN if a level-1 link is singular (no unitary factor); partitioned contexts:
  * HISQ_EINVAL. */
 size_t hisq_smear_bytes(const hisq_ctx *h);

@@ -271,7 +271,7 @@ class Hisq:
         self._check(self.lib.hisq_smear(self._h, self._ptr(thin, shp, self.cdtype), self._ptr(fat, shp, self.cdtype),
                                         self._ptr(naik, shp, self.cdtype), scratch.data_ptr(), float(fat_scale),
                                         float(naik_scale), int(bool(fold_phases))))
-        return fat, naik, scratch[: 4 * V * 9].view(shp)
+        return fat, naik, scratch[4 * V * 9: 8 * V * 9].view(shp)
 
     def cg_multishift(self, b: torch.Tensor, mass: float, shifts, tol: float, x: Optional[torch.Tensor] = None,
                       strict: bool = True):

@@ -927,26 +927,35 @@ static int smear_level(hisq_ctx* h, const T* in, T* out, T* A, T* B, T* C, const
 }
 
 template <typename T>
-static int smear_impl(hisq_ctx* h, const T* thin, T* fat, T* naik, T* W, double fat_scale, double naik_scale, int fold)
+static int smear_impl(hisq_ctx* h, const T* thin, T* fat, T* naik, T* scratch, double fat_scale, double naik_scale, int fold)
 {
     const Geom& g = h->g;
-    const size_t V = (size_t)2 * g.Vh;
-    // the Naik output doubles as the three staple fields until the very end
+    const size_t V = (size_t)2 * g.Vh, field = 4 * V * 18;
+    // all intermediate fields are structure-of-arrays (smear.cuh); the outputs double as scratch until they are written:
+    //   fat  <- thin links transposed          (dead after level 1)
+    //   naik <- the three staple fields A, B, C (dead after level 2)
+    //   scratch[0] <- level 1 -> W             scratch[1] <- level 2 (X), later W in the canonical layout
+    T* Usoa = fat;
+    T* W = scratch;
+    T* X = scratch + field;
     T* A = naik; T* B = naik + V * 18; T* C = naik + 2 * V * 18;
+    const dim3 gl((unsigned)((V + 127) / 128), 4);
+    link_layout_kernel<T, true><<<gl, 128, 0, h->stream>>>(g, thin, Usoa, T(1), 0);
+    h->stats.launches++;
     const SmearCoeff fat7 = { 1.0 / 8.0, 1.0 / 16.0, 1.0 / 64.0, 1.0 / 384.0, 0.0 };
     const SmearCoeff fat7L = { 1.0, 1.0 / 16.0, 1.0 / 64.0, 1.0 / 384.0, -1.0 / 8.0 };
-    int rc = smear_level<T>(h, thin, W, A, B, C, fat7);
+    int rc = smear_level<T>(h, Usoa, W, A, B, C, fat7);
     if (rc) return rc;
     unsigned long long* bad = h->bad_count;
     CK(cudaMemsetAsync(bad, 0, sizeof(unsigned long long), h->stream));
-    project_u3_kernel<T><<<(unsigned)((4 * V + 127) / 128), 128, 0, h->stream>>>(W, 4 * V, bad);
+    project_u3_kernel<T><<<(unsigned)((4 * V + 127) / 128), 128, 0, h->stream>>>(W, V, bad);
     h->stats.launches++;
-    rc = smear_level<T>(h, W, fat, A, B, C, fat7L);
+    rc = smear_level<T>(h, W, X, A, B, C, fat7L);
     if (rc) return rc;
-    const dim3 gl((unsigned)((V + 127) / 128), 4);
-    fold_kernel<T><<<gl, 128, 0, h->stream>>>(g, fat, (T)fat_scale, fold);
+    link_layout_kernel<T, false><<<gl, 128, 0, h->stream>>>(g, X, fat, (T)fat_scale, fold);
     naik_kernel<T><<<gl, 128, 0, h->stream>>>(g, W, naik, (T)naik_scale, fold);
-    h->stats.launches += 2;
+    link_layout_kernel<T, false><<<gl, 128, 0, h->stream>>>(g, W, X, T(1), 0);   // W for the caller, canonical, in scratch[1]
+    h->stats.launches += 3;
     CK(cudaGetLastError());
     unsigned long long nbad = 0;
     CK(cudaMemcpyAsync(&nbad, bad, sizeof(nbad), cudaMemcpyDeviceToHost, h->stream));
@@ -961,18 +970,18 @@ static int smear_impl(hisq_ctx* h, const T* thin, T* fat, T* naik, T* W, double 
 extern "C" size_t hisq_smear_bytes(const hisq_ctx* h)
 {
     if (!h) return 0;
-    return align_up((size_t)4 * 2 * h->g.Vh * 18 * elem_size(h->prec));
+    return 2 * (size_t)4 * 2 * h->g.Vh * 18 * elem_size(h->prec);   // two link fields (see smear_impl)
 }
 
 extern "C" int hisq_smear(hisq_ctx* h, const void* thin, void* fat, void* naik, void* scratch, double fat_scale, double naik_scale,
                           int fold_phases)
 {
     if (!h || !thin || !fat || !naik || !scratch || !std::isfinite(fat_scale) || !std::isfinite(naik_scale)) return HISQ_EINVAL;
-    const void* ptr[4] = { thin, fat, naik, scratch };
     const size_t bytes = (size_t)4 * 2 * h->g.Vh * 18 * elem_size(h->prec);
-    for (int i = 0; i < 4; ++i) {
+    const void* ptr[5] = { thin, fat, naik, scratch, (const char*)scratch + bytes };
+    for (int i = 0; i < 5; ++i) {
         if ((uintptr_t)ptr[i] & 15) return HISQ_EINVAL;
-        for (int j = i + 1; j < 4; ++j)
+        for (int j = i + 1; j < 5; ++j)
             if (overlap(ptr[i], ptr[j], bytes)) return HISQ_EINVAL;
     }
     if (h->g.part) return HISQ_EINVAL;

@@ -11,9 +11,14 @@
 //     S3_nu = G_nu[U_mu]          S5_nu,rho = G_rho[S3_nu]          S7_nu,rho,sigma = G_sigma[S5_nu,rho]
 //     Lepage_nu = up-part of G_nu[up-part of S3_nu] + down-part of G_nu[down-part of S3_nu]
 // 18 launches of one kernel per direction and level instead of 84 path products.  The projection is a Newton iteration
-// for the polar factor, X <- (X + X^-+) / 2, not an eigen-decomposition.  Everything works on the CANONICAL link
-// layout of include/hisq.h (matrix of (x, mu) at slot mu*V + eo(x), 9 complex row-major): smearing is set-up work
-// whose output goes through hisq_set_links, and the gauge field is periodic in all four directions.
+// for the polar factor, X <- (X + X^-+) / 2, not an eigen-decomposition.  The gauge field is periodic in all four
+// directions.
+// Layouts: the ABI side is the CANONICAL link array of include/hisq.h (matrix of (x, mu) at slot mu*V + eo(x), 9 complex
+// row-major, i.e. 144-byte records in fp64).  Read lane by lane such records put every lane of a warp-level load on a
+// different cache line (first ncu capture of the staple kernel: DRAM traffic = algorithmic bytes but "Mem Busy" 73 % at
+// half the copy bandwidth), so all the work in between runs on a structure-of-arrays copy: entry e of the matrix of
+// (x, mu) at complex index (mu*9 + e)*V + eo(x) -- a warp reads 32 consecutive complex numbers per load.  The thin links
+// are transposed once on the way in, the three results once on the way out.
 #pragma once
 #include "common.cuh"
 
@@ -36,6 +41,23 @@ template <typename T> __device__ __forceinline__ void mat_store(T* p, const Mat3
     C* q = reinterpret_cast<C*>(p);
 #pragma unroll
     for (int e = 0; e < 9; ++e) { C w; w.x = m.r[e]; w.y = m.i[e]; q[e] = w; }
+}
+// structure-of-arrays field of n matrices: entry e of matrix i at complex index e*n + i
+template <typename T> __device__ __forceinline__ Mat3<T> soa_load(const T* p, size_t n, size_t i)
+{
+    using C = typename Vec<T>::c1;
+    const C* q = reinterpret_cast<const C*>(p) + i;
+    Mat3<T> m;
+#pragma unroll
+    for (int e = 0; e < 9; ++e) { const C w = q[e * n]; m.r[e] = w.x; m.i[e] = w.y; }
+    return m;
+}
+template <typename T> __device__ __forceinline__ void soa_store(T* p, size_t n, size_t i, const Mat3<T>& m)
+{
+    using C = typename Vec<T>::c1;
+    C* q = reinterpret_cast<C*>(p) + i;
+#pragma unroll
+    for (int e = 0; e < 9; ++e) { C w; w.x = m.r[e]; w.y = m.i[e]; q[e * n] = w; }
 }
 template <typename T> __device__ __forceinline__ Mat3<T> mat_add(const Mat3<T>& a, const Mat3<T>& b)
 {
@@ -104,50 +126,54 @@ __global__ void __launch_bounds__(128) smear_init_kernel(T* __restrict__ out, co
 // ---- one generalised staple (see the header): up(x) = U_nu(x) Lu(x+nu) U_nu(x+mu)^+ , dn(x) = U_nu(x-nu)^+ Ld(x-nu) U_nu(x-nu+mu)
 // with Lu = a_up (+ b), Ld = a_dn (+ b); acc(x) += coef (up + dn); up / dn are stored to out_up / out_dn if given (their
 // sum if both point to the same array).  U: the 4V links being smeared; a_*, b, out_*, acc: V matrices of direction mu.
+// All structure-of-arrays (V matrices per block).
 template <typename T>
 __global__ void __launch_bounds__(128) staple_kernel(const Geom g, const T* __restrict__ U, const T* __restrict__ a_up,
                                                      const T* __restrict__ a_dn, const T* __restrict__ b, T* out_up, T* out_dn,
                                                      T* __restrict__ acc, int mu, int nu, T coef)
 {
     const int eo = blockIdx.x * 128 + threadIdx.x;
-    const int V = 2 * g.Vh;
-    if (eo >= V) return;
+    const size_t V = (size_t)2 * g.Vh;
+    if (eo >= (int)V) return;
     const Site x = site_of_eo(g, eo);
     const T* Unu = U + (size_t)nu * V * 18;
     // up
     const int xpn = eo_of_site(g, hop(g, x, nu, 1));
     const int xpm = eo_of_site(g, hop(g, x, mu, 1));
-    Mat3<T> L = mat_load(a_up + (size_t)xpn * 18);
-    if (b) L = mat_add(L, mat_load(b + (size_t)xpn * 18));
-    Mat3<T> up = mat_mul<T, false, true>(mat_mul<T, false, false>(mat_load(Unu + (size_t)eo * 18), L), mat_load(Unu + (size_t)xpm * 18));
+    Mat3<T> L = soa_load(a_up, V, xpn);
+    if (b) L = mat_add(L, soa_load(b, V, xpn));
+    Mat3<T> up = mat_mul<T, false, true>(mat_mul<T, false, false>(soa_load(Unu, V, eo), L), soa_load(Unu, V, xpm));
     // down
     const Site xm = hop(g, x, nu, -1);
     const int xmn = eo_of_site(g, xm);
     const int xmnpm = eo_of_site(g, hop(g, xm, mu, 1));
-    L = mat_load(a_dn + (size_t)xmn * 18);
-    if (b) L = mat_add(L, mat_load(b + (size_t)xmn * 18));
-    Mat3<T> dn = mat_mul<T, false, false>(mat_mul<T, true, false>(mat_load(Unu + (size_t)xmn * 18), L), mat_load(Unu + (size_t)xmnpm * 18));
+    L = soa_load(a_dn, V, xmn);
+    if (b) L = mat_add(L, soa_load(b, V, xmn));
+    Mat3<T> dn = mat_mul<T, false, false>(mat_mul<T, true, false>(soa_load(Unu, V, xmn), L), soa_load(Unu, V, xmnpm));
     const Mat3<T> sum = mat_add(up, dn);
-    if (out_up != nullptr && out_up == out_dn) mat_store(out_up + (size_t)eo * 18, sum);
+    if (out_up != nullptr && out_up == out_dn) soa_store(out_up, V, eo, sum);
     else {
-        if (out_up) mat_store(out_up + (size_t)eo * 18, up);
-        if (out_dn) mat_store(out_dn + (size_t)eo * 18, dn);
+        if (out_up) soa_store(out_up, V, eo, up);
+        if (out_dn) soa_store(out_dn, V, eo, dn);
     }
-    Mat3<T> f = mat_load(acc + (size_t)eo * 18);
+    Mat3<T> f = soa_load(acc, V, eo);
 #pragma unroll
     for (int e = 0; e < 9; ++e) { f.r[e] = fma(coef, sum.r[e], f.r[e]); f.i[e] = fma(coef, sum.i[e], f.i[e]); }
-    mat_store(acc + (size_t)eo * 18, f);
+    soa_store(acc, V, eo, f);
 }
 
 // ---- W = V (V^+ V)^(-1/2), in place: Newton iteration for the unitary polar factor, X <- (X + X^-+) / 2 ------------------
 // (quadratically convergent for any non-singular V; singular values s -> (s + 1/s)/2).  *bad counts links that did not
 // converge (singular or non-finite input).
+// links: 4 structure-of-arrays blocks of V matrices.
 template <typename T>
-__global__ void __launch_bounds__(128) project_u3_kernel(T* __restrict__ links, size_t nmat, unsigned long long* bad)
+__global__ void __launch_bounds__(128) project_u3_kernel(T* __restrict__ links, size_t V, unsigned long long* bad)
 {
     const size_t idx = (size_t)blockIdx.x * 128 + threadIdx.x;
-    if (idx >= nmat) return;
-    Mat3<T> X = mat_load(links + idx * 18);
+    if (idx >= 4 * V) return;
+    T* blk = links + (idx / V) * V * 18;
+    const size_t site = idx % V;
+    Mat3<T> X = soa_load(blk, V, site);
     const T tol = sizeof(T) == 4 ? T(1e-5) : T(1e-12);   // of the LAST step; the error after it is its square
     bool ok = false;
     for (int it = 0; it < 60 && !ok; ++it) {
@@ -184,10 +210,10 @@ __global__ void __launch_bounds__(128) project_u3_kernel(T* __restrict__ links, 
         ok = change <= tol * tol * size;
     }
     if (!ok) atomicAdd(bad, 1ull);
-    mat_store(links + idx * 18, X);
+    soa_store(blk, V, site, X);
 }
 
-// ---- N_mu(x) = scale * eta_mu(x) * W_mu(x) W_mu(x+mu) W_mu(x+2mu) ---------------------------------------------------------
+// ---- N_mu(x) = scale * eta_mu(x) * W_mu(x) W_mu(x+mu) W_mu(x+2mu)  (W structure-of-arrays, N canonical) ---------------------------------------------------------
 __device__ __forceinline__ int eta_sign(const Site& s, int mu)
 {
     const int e = mu == 0 ? 0 : (mu == 1 ? s.c[0] : (mu == 2 ? s.c[0] + s.c[1] : s.c[0] + s.c[1] + s.c[2]));
@@ -203,27 +229,27 @@ __global__ void __launch_bounds__(128) naik_kernel(const Geom g, const T* __rest
     const Site x = site_of_eo(g, eo);
     const T* Wm = W + (size_t)mu * V * 18;
     const int x1 = eo_of_site(g, hop(g, x, mu, 1)), x2 = eo_of_site(g, hop(g, x, mu, 2));
-    Mat3<T> P = mat_mul<T, false, false>(mat_mul<T, false, false>(mat_load(Wm + (size_t)eo * 18), mat_load(Wm + (size_t)x1 * 18)),
-                                         mat_load(Wm + (size_t)x2 * 18));
+    Mat3<T> P = mat_mul<T, false, false>(mat_mul<T, false, false>(soa_load(Wm, V, eo), soa_load(Wm, V, x1)), soa_load(Wm, V, x2));
     const T s = fold ? scale * (T)eta_sign(x, mu) : scale;
 #pragma unroll
     for (int e = 0; e < 9; ++e) { P.r[e] *= s; P.i[e] *= s; }
     mat_store(out + ((size_t)mu * V + eo) * 18, P);
 }
-// ---- X_mu(x) *= scale * eta_mu(x), in place -----------------------------------------------------------------------------
-template <typename T>
-__global__ void __launch_bounds__(128) fold_kernel(const Geom g, T* __restrict__ X, T scale, int fold)
+// ---- layout conversion of a link field (4V matrices), optionally times scale * eta_mu(x) -------------------------------
+// TO_SOA: canonical -> structure-of-arrays; else structure-of-arrays -> canonical.  src != dst.
+template <typename T, bool TO_SOA>
+__global__ void __launch_bounds__(128) link_layout_kernel(const Geom g, const T* __restrict__ src, T* __restrict__ dst, T scale, int fold)
 {
-    const int V = 2 * g.Vh;
+    const size_t V = (size_t)2 * g.Vh;
     const int eo = blockIdx.x * 128 + threadIdx.x;
     const int mu = blockIdx.y;
-    if (eo >= V) return;
+    if (eo >= (int)V) return;
     const T s = fold ? scale * (T)eta_sign(site_of_eo(g, eo), mu) : scale;
-    T* p = X + ((size_t)mu * V + eo) * 18;
-    Mat3<T> m = mat_load(p);
+    Mat3<T> m = TO_SOA ? mat_load(src + ((size_t)mu * V + eo) * 18) : soa_load(src + (size_t)mu * V * 18, V, eo);
 #pragma unroll
     for (int e = 0; e < 9; ++e) { m.r[e] *= s; m.i[e] *= s; }
-    mat_store(p, m);
+    if (TO_SOA) soa_store(dst + (size_t)mu * V * 18, V, eo, m);
+    else mat_store(dst + ((size_t)mu * V + eo) * 18, m);
 }
 
 }  // namespace hisq
