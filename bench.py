@@ -344,10 +344,28 @@ def main():
         ctx.smear(thin)
         e1.record()
         e1.synchronize()
-        smear = {"what": "hisq_smear: fat7 -> U(3) projection -> fat7 + Lepage, Naik product, phases folded (canonical layout)",
+        smear = {"what": "hisq_smear: fat7 -> U(3) projection -> fat7 + Lepage, Naik product, phases folded",
                  "ms": e0.elapsed_time(e1), "launches": int(ctx.launch_count() - l0),
                  "thin_links": "Gram-Schmidt of 1 + 0.3 x Gaussian (seeded stand-in for a thermalised configuration)"}
+        # the chain a production run uses: smeared links (U(3) Naik links, 14-real compression) -> full-system solve
+        sfat, snaik, _ = ctx.smear(thin, fat_scale=0.5, naik_scale=-0.5 / 24.0)
         del thin
+        sc = binding.Hisq(L, cfg["prec"], n, dev)
+        sc.set_option("naik_compress", 1)
+        sc.set_links(sfat, snaik)
+        del sfat, snaik
+        bo = sc.pack(binding.make_sources(L, rank, n, 1, dev, sc.cdtype, gen_device=gen_dev))
+        sc.solve_M(b, bo, cfg["mass"], cfg["tol"])
+        torch.cuda.synchronize()
+        e0.record()
+        _, _, si = sc.solve_M(b, bo, cfg["mass"], cfg["tol"])
+        e1.record()
+        e1.synchronize()
+        smear["solve_on_smeared_links"] = {"naik_compressed": bool(sc.naik_compressed()), "solve_ms": e0.elapsed_time(e1),
+                                           "iterations": si["iterations"], "full_lattice_rel_resid": si["true_rel_resid"],
+                                           "dslash_ms": time_dslash(sc, n, args.dslash_reps)}
+        sc.close()
+        del sc, bo
     # ---- row f2: the same Dslash and solve with compressed Naik links (14 instead of 18 reals per Naik link) ----
     comp = None
     if not args.no_compression:
