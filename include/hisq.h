@@ -55,7 +55,7 @@ enum {
     HISQ_ENOWORKSPACE = -3, /* no workspace set, or it is smaller than hisq_workspace_bytes(nrhs)          */
     HISQ_ECUDA = -4,        /* a CUDA call failed; text via hisq_last_error                                */
     HISQ_ENOCONV = -5,      /* max_iter reached; x holds the last iterate, hisq_get_info the residuals     */
-    HISQ_EBREAKDOWN = -6,   /* <p, A p> <= 0 or a non-finite scalar appeared in CG                         */
+    HISQ_EBREAKDOWN = -6,   /* <p, A p> <= 0 or a non-finite scalar appeared in CG; hisq_smear: singular link */
     HISQ_EIO = -7           /* file cannot be opened / is truncated / fails its checksum or link trace     */
 };
 

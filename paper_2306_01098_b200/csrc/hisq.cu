@@ -1501,7 +1501,7 @@ extern "C" const char* hisq_strerror(int code)
     case HISQ_ENOWORKSPACE: return "workspace missing or too small";
     case HISQ_ECUDA: return "CUDA error (see hisq_last_error)";
     case HISQ_ENOCONV: return "CG did not converge within max_iter";
-    case HISQ_EBREAKDOWN: return "CG breakdown (<p,Ap> <= 0 or non-finite scalar)";
+    case HISQ_EBREAKDOWN: return "breakdown (CG: <p,Ap> <= 0 or non-finite scalar; smearing: singular link)";
     case HISQ_EIO: return "file cannot be read / written or fails its checksum";
     default: return "unknown error code";
     }
