@@ -455,7 +455,7 @@ def main():
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": ncu_traffic(args.config, cfg["prec"], n),
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
-                     "timing": f"CUDA events around {2 * args.dslash_reps} back-to-back launches (alternating parity), best of 3 bursts"},
+                     "timing": f"CUDA events around {2 * args.dslash_reps} back-to-back hisq_dslash calls (alternating parity), best of 3 bursts; the library launches them with programmatic dependent launch: the head of call i+1 overlaps the tail of call i (~2 us per call)"},
         "e2e": {"value": e2e_val, "unit": "GFLOP/s", "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": field_bytes,
                 "ms_per_step": ms2_all / args.steps},
         "gpu_launches": int(launches), "clocks": clocks,

@@ -149,6 +149,9 @@ template <typename T> __device__ __forceinline__ void mv_acc(const T (&U)[18], c
         }
 }
 
+#ifndef HISQ_PDL
+#define HISQ_PDL 1   // programmatic dependent launch of the Dslash kernels (dslash_launch_impl.cuh); 0: plain <<< >>> launches
+#endif
 #ifndef HISQ_F32X2
 #define HISQ_F32X2 1   // 1: fp32 complex multiply-adds as packed FFMA2 (fma.rn.f32x2, sm_100+): 2/3 of the FMA issue slots
 #endif
@@ -315,6 +318,12 @@ template <typename T, int NR, int MODE = 0> struct KernelShape {
 template <typename T, int NR, int MODE, int BLOCK, bool NC>
 __global__ void __launch_bounds__(BLOCK, KernelShape<T, NR, MODE>::minb) dslash_kernel(const DslashArgs<T> a)
 {
+#if HISQ_PDL
+    // let the next kernel of the stream start scheduling its CTAs as this grid's last wave drains, and do not touch
+    // memory before everything this launch depends on has completed (programmatic dependent launch, dslash_launch_impl.cuh)
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
     if (a.done != nullptr && *a.done != 0) {
         // solver finished: nothing to compute, but the other ranks' streams still wait for this rank's arrival in
         // the all-reduce of this iteration -- one designated CTA of the launch group keeps the count right

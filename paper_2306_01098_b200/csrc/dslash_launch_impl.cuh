@@ -7,9 +7,22 @@ namespace hisq {
 template <typename T, int NR, int MODE>
 static cudaError_t launch_one(const DslashArgs<T>& a, dim3 grid, cudaStream_t s)
 {
+#if HISQ_PDL
+    // programmatic dependent launch: the CTAs of this launch may become resident while the previous kernel of the
+    // stream drains its last wave; they wait in griddepcontrol.wait (top of dslash_kernel) until it has completed
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = dim3(kDslashBlock); cfg.dynamicSmemBytes = 0; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    if (a.naik_c14) return cudaLaunchKernelEx(&cfg, dslash_kernel<T, NR, MODE, kDslashBlock, true>, a);
+    return cudaLaunchKernelEx(&cfg, dslash_kernel<T, NR, MODE, kDslashBlock, false>, a);
+#else
     if (a.naik_c14) dslash_kernel<T, NR, MODE, kDslashBlock, true><<<grid, kDslashBlock, 0, s>>>(a);
     else dslash_kernel<T, NR, MODE, kDslashBlock, false><<<grid, kDslashBlock, 0, s>>>(a);
     return cudaGetLastError();
+#endif
 }
 
 template <typename T, int NR>
