@@ -890,6 +890,20 @@ extern "C" int hisq_solve_M(hisq_ctx* h, void* x_even, void* x_odd, const void* 
 // ---- HISQ link smearing (row f4): thin links -> fat and Naik links, canonical layout in and out ----------------------
 struct SmearCoeff { double c1, c3, c5, c7, cL; };
 
+template <typename T>
+static void launch_staple(hisq_ctx* h, unsigned grid, const T* U, const T* a_up, const T* a_dn, const T* b, T* out_up, T* out_dn, T* acc,
+                          int mu, int nu, T coef)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = 0; cfg.stream = h->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, staple_kernel<T>, h->g, U, a_up, a_dn, b, out_up, out_dn, acc, mu, nu, coef);
+    h->stats.launches++;
+}
+
 // out (4V matrices) = smeared `in` (4V); A, B, C: V matrices of scratch each
 template <typename T>
 static int smear_level(hisq_ctx* h, const T* in, T* out, T* A, T* B, T* C, const SmearCoeff& k)
@@ -905,20 +919,16 @@ static int smear_level(hisq_ctx* h, const T* in, T* out, T* A, T* B, T* C, const
         for (int nu = 0; nu < 4; ++nu) {
             if (nu == mu) continue;
             // S3_nu: up part -> A, down part -> B
-            staple_kernel<T><<<grid, 128, 0, h->stream>>>(g, in, Umu, Umu, nullptr, A, B, acc, mu, nu, (T)k.c3);
-            h->stats.launches++;
+            launch_staple<T>(h, grid, in, Umu, Umu, nullptr, A, B, acc, mu, nu, (T)k.c3);
             if (k.cL != 0.0) {   // Lepage: the straight two-step staples only (up of up, down of down)
-                staple_kernel<T><<<grid, 128, 0, h->stream>>>(g, in, A, B, nullptr, nullptr, nullptr, acc, mu, nu, (T)k.cL);
-                h->stats.launches++;
+                launch_staple<T>(h, grid, in, A, B, nullptr, nullptr, nullptr, acc, mu, nu, (T)k.cL);
             }
             for (int rho = 0; rho < 4; ++rho) {
                 if (rho == mu || rho == nu) continue;
                 // S5_nu,rho = G_rho[A + B] -> C
-                staple_kernel<T><<<grid, 128, 0, h->stream>>>(g, in, A, A, B, C, C, acc, mu, rho, (T)k.c5);
-                h->stats.launches++;
+                launch_staple<T>(h, grid, in, A, A, B, C, C, acc, mu, rho, (T)k.c5);
                 const int sig = 6 - mu - nu - rho;
-                staple_kernel<T><<<grid, 128, 0, h->stream>>>(g, in, C, C, nullptr, nullptr, nullptr, acc, mu, sig, (T)k.c7);
-                h->stats.launches++;
+                launch_staple<T>(h, grid, in, C, C, nullptr, nullptr, nullptr, acc, mu, sig, (T)k.c7);
             }
         }
     }

@@ -135,6 +135,9 @@ __global__ void __launch_bounds__(128, HISQ_STAPLE_MINB) staple_kernel(const Geo
                                                      const T* __restrict__ a_dn, const T* __restrict__ b, T* out_up, T* out_dn,
                                                      T* __restrict__ acc, int mu, int nu, T coef)
 {
+    // programmatic dependent launch (as the Dslash kernel): the next launch's CTAs become resident while this grid drains
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int eo = blockIdx.x * 128 + threadIdx.x;
     const size_t V = (size_t)2 * g.Vh;
     if (eo >= (int)V) return;
