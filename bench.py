@@ -1,27 +1,33 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line for the multi-RHS HISQ Dslash + CG hot path on B200.
 
-A STEP is one pass of the whole hot path on BASELINE.json configs[1] (32^3 x 8, fp64, nRHS = 1): one
-`hisq_cg` solve of (m^2 - D_eo D_oe) x = b at m = 0.01 to tol 1e-10 (index maps, gathers, Dslash,
-fused A-apply, BLAS-1/reductions, convergence control: SURVEY.md 8(a) rows a1-a7) on seeded synthetic
-links and a Gaussian even-site source already resident in HBM.  `value` is the metric BASELINE.json
-names, HISQ Dslash GFLOP/s, counted as 1146 flop per output site per RHS over every
-Dslash application the solve made, divided by the whole solve time (so BLAS-1 and host polling count
-against it).  Beside it:
-  dslash     pure Dslash launches (alternating D_oe / D_eo), CUDA-event timed: GFLOP/s, algorithmic GB/s
-  roofline   the dominant kernel (Dslash fp64 n=1) against MEASURED_PEAKS.json's HBM copy bandwidth
-  sweep      configs[2] (64^3 x 16, fp32) Dslash vs nRHS = 1, 2, 4, 8     (--no-sweep to skip)
-  e2e        the same step through hisq_cg_host with pinned HOST buffers (H2D + D2H inside the timing)
+Headline workload: BASELINE.json configs[4], the largest single-GPU configuration (C5: 96^3 x 24, fp64, nRHS = 8,
+CG at m = 0.005, tol 1e-10).  A STEP is one `hisq_cg` call on it, capped at `--step-iters` (64) CG iterations
+(HISQ_ENOCONV is the expected return of a capped step): index maps, gathers, multi-RHS Dslash, fused A-apply, BLAS-1 and
+reductions, convergence control and the closing fp64 true-residual check on seeded synthetic
+links and Gaussian even-site sources already resident in HBM.  `value` is the metric BASELINE.json names, HISQ Dslash
+GFLOP/s, counted as 1146 flop per output site per RHS over every Dslash application the steps made,
+divided by the whole time of the steps (BLAS-1 and host polling count against it).  Beside it, in the same line:
+  cg            ONE full solve of the headline config to tol, outside the timed steps: solve_ms, iterations, residuals
+  dslash        the dominant kernel alone (alternating D_oe / D_eo), CUDA-event timed: GFLOP/s, algorithmic GB/s
+  roofline      that kernel against MEASURED_PEAKS.json's HBM copy bandwidth, DRAM traffic from the committed ncu capture
+  configs       one block per other BASELINE config: C1, C2 (Dslash + full CG), C3 (fp32 Dslash vs nRHS), C4 (mixed CG)
+  e2e           the same capped step through hisq_cg_host with pinned HOST buffers (H2D + D2H inside the timing)
   cpu_baseline  the oracle (oracle/, as it stands) on this box's host cores on a bounded sample
 `--impl reference` times the oracle instead (this tier's reference arm).
-Multi-GPU (torchrun): independent replicas, one per rank, no collective on the data path ("replicas
-only"); value = total flops of all ranks / max-over-ranks time.
+Multi-GPU: `--gpus N` starts N ranks itself (torch.distributed.run) unless it already runs under torchrun.
+  --mode replicas      (default) independent replicas, one per rank, no collective on the data path ("replicas only",
+                       DESIGN.md 9); value = total flops of all ranks / max-over-ranks time; scaling "weak"
+  --mode partitioned   ONE lattice cut over the ranks (row f3): hisq_cg on hisq_create_part contexts, halos and
+                       all-reduces through peer-mapped mailboxes; scaling "strong"
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -33,10 +39,6 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 FLOP_PER_SITE = 1146
-# Context denominators measured on this pool's B200 with `python -m paper_2306_01098_b200.peaks`
-# (profiles/r1_peaks_microbench.txt); the roofline `peak` itself comes from MEASURED_PEAKS.json.
-READ_ONLY_GBS = 7420.0                       # 128-bit read-only stream over 8 GB
-FMA_PEAK_GFLOPS = {4: 69600.0, 8: 36900.0}   # plain FFMA / DFMA, all SMs
 CONFIGS = {
     "C1": dict(L=(8, 8, 8, 8), prec="fp64", nrhs=1, mass=0.1, tol=1e-10),
     "C2": dict(L=(32, 32, 32, 8), prec="fp64", nrhs=1, mass=0.01, tol=1e-10),
@@ -54,8 +56,15 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def context_peaks():
+    """Context denominators measured once on this pool's B200 (profiles/peaks.json names the command): the read-only
+    stream and the plain FMA rates.  The roofline `peak` itself comes from MEASURED_PEAKS.json."""
+    with open(os.path.join(ROOT, "profiles", "peaks.json")) as f:
+        return json.load(f)
+
+
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    """nvidia-smi clocks / throttle reasons sampled DURING a timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -70,6 +79,7 @@ class ClockSampler:
             threading.Thread(target=self._read, daemon=True).start()
         except Exception:
             self.proc = None
+        return self
 
     def _read(self):
         for line in self.proc.stdout:
@@ -92,33 +102,48 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def aggregate(ms: float, flops: float, dist, device):
+def aggregate(ms: float, flops: float, dist, device, sum_flops: bool = True):
     """Whole-job throughput over ranks: (max over ranks of the device time, sum over ranks of the work).
-    No collective sits on the data path ("replicas only"): this all-reduce only combines the timings."""
+    No collective sits on the data path of the replica mode: this all-reduce only combines the timings."""
     t = torch.tensor([ms], dtype=torch.float64, device=device)
     f = torch.tensor([flops], dtype=torch.float64, device=device)
     if dist is not None:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(f, op=dist.ReduceOp.SUM)
+        if sum_flops:
+            dist.all_reduce(f, op=dist.ReduceOp.SUM)
     return t.item(), f.item()
 
 
+def kernel_source_hash() -> str:
+    """Identifies the Dslash kernel a capture was taken from: sha1 over the sources that define it."""
+    h = hashlib.sha1()
+    for f in ("dslash.cuh", "dslash_launch_impl.cuh", "common.cuh"):
+        h.update(open(os.path.join(ROOT, "paper_2306_01098_b200", "csrc", f), "rb").read())
+    return h.hexdigest()[:12]
+
+
 def ncu_traffic(config: str, prec: str, nrhs: int):
-    """DRAM bytes per launch of the Dslash kernel from the committed ncu captures (profiles/r1_traffic.csv), or None."""
+    """(DRAM bytes per launch, capture file) of the Dslash kernel from the committed ncu captures
+    (profiles/r2_traffic.csv: workload,kernel_source_hash,dram_bytes_per_launch,capture).  A row taken from OTHER kernel
+    sources than the ones in this tree is refused: (None, reason)."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+    want, have = f"{config}:{prec}:{nrhs}", kernel_source_hash()
     try:
-        with open(os.path.join(ROOT, "profiles", "r1_traffic.csv")) as f:
+        with open(path) as f:
             for line in f:
-                k, _, v = line.strip().partition(",")
-                if k == f"{config}:{prec}:{nrhs}":
-                    return int(v)
-    except Exception:
-        pass
-    return None
+                c = [x.strip() for x in line.strip().split(",")]
+                if len(c) >= 4 and c[0] == want:
+                    if c[1] != have:
+                        return None, f"stale: {path} row {want} was captured from kernel sources {c[1]}, this tree is {have}"
+                    return int(c[2]), c[3]
+    except OSError as e:
+        return None, str(e)
+    return None, f"no row {want} in {path}"
 
 
 def dslash_bytes(Vh: int, nrhs: int, w: int) -> int:
     """Algorithmic (compulsory) bytes of one Dslash application: 16 links of 18 reals per output site,
-    each input and each output site's colour vector once: (288 + 12 n) words per site (DESIGN.md)."""
+    each input and each output site's colour vector once: (288 + 12 n) words per site (DESIGN.md 6)."""
     return (288 + 12 * nrhs) * w * Vh
 
 
@@ -143,56 +168,206 @@ def time_dslash(ctx, nrhs: int, reps: int, warm: int = 5):
     return e0.elapsed_time(e1) / (2 * reps)
 
 
+def dslash_block(ctx, nrhs: int, reps: int, peak: float, ctxpk: dict, bursts: int = 3):
+    """Best of `bursts` bursts of 2*reps launches, as numbers against every denominator DESIGN.md 6 names."""
+    ms = min(time_dslash(ctx, nrhs, reps) for _ in range(bursts))
+    w = 4 if ctx.prec == "fp32" else 8
+    by = dslash_bytes(ctx.Vh, nrhs, w)
+    gf = FLOP_PER_SITE * ctx.Vh * nrhs / (ms * 1e-3) / 1e9
+    gbs = by / (ms * 1e-3) / 1e9
+    return {"nrhs": nrhs, "ms": ms, "gflops": gf, "alg_gbs": gbs, "algorithmic_bytes": by,
+            "paper_model_gbs": (288 + 102 * nrhs) * w * ctx.Vh / (ms * 1e-3) / 1e9,
+            "frac_of_measured_copy": gbs / peak, "frac_of_8TBs": gbs / 8000.0,
+            "frac_of_measured_read_only": gbs / ctxpk["read_only_gbs"],
+            "frac_of_fma_peak": gf / ctxpk["fma_peak_gflops"]["fp32" if w == 4 else "fp64"],
+            "tiles": ctx.tiles(nrhs), "timing": f"best of {bursts} bursts of {2 * reps} back-to-back launches, CUDA events"}
+
+
+def workload_name(name, cfg):
+    L = cfg["L"]
+    what = f"CG m={cfg['mass']} tol={cfg['tol']}" if cfg["mass"] is not None else "Dslash sweep"
+    return (f"{name}: {L[0]}x{L[1]}x{L[2]}x{L[3]} {cfg['prec']} nRHS={cfg['nrhs']} {what}, "
+            "Gaussian fat links (std 0.3), Haar SU(3) Naik x(-1/24), phases folded, antiperiodic t")
+
+
+def make_ctx(cfg, dev, seed, nrhs=None, prec=None, compress=False):
+    """A context of cfg's lattice with its seeded links set.  Small lattices are generated on the CPU (bit-identical to
+    the oracle's inputs), large ones on the GPU with the same counter-based stream."""
+    from paper_2306_01098_b200 import binding
+    L = cfg["L"]
+    gen_dev = dev if binding.layout.volume(L) > (1 << 21) else None
+    ctx = binding.Hisq(L, prec or cfg["prec"], nrhs or cfg["nrhs"], dev)
+    if compress:
+        ctx.set_option("naik_compress", 1)
+    fat, naik = binding.make_links(L, seed, dev, ctx.cdtype, gen_device=gen_dev)
+    ctx.set_links(fat, naik)
+    del fat, naik
+    torch.cuda.empty_cache()
+    return ctx, gen_dev
+
+
+# ---- the oracle on the host cores: cpu_baseline and the reference arm ------------------------------------------------
+def oracle_block(cfg):
+    """The lattice the oracle is timed on: the config's own if it has at most 2^21 sites, else a block of it with every
+    extent halved until it has (same generators, same operator; the oracle's rate per site does not depend on the
+    volume once the links exceed the host caches)."""
+    L = list(cfg["L"])
+    while L[0] * L[1] * L[2] * L[3] > (1 << 21):
+        L = [max(4, v // 2) for v in L]
+    return tuple(L)
+
+
 def oracle_sample(cfg, seed: int, budget_s: float):
-    """Time the oracle on a bounded sample of the step: `iters` CG iterations of the same workload."""
-    import numpy as np
+    """Time the oracle on a bounded sample of the step: `iters` CG iterations of ONE right-hand side on oracle_block."""
     import oracle
     from paper_2306_01098_b200 import inputs
-    L = cfg["L"]
+    L = oracle_block(cfg)
     V = inputs.volume(L)
     s = torch.arange(V, dtype=torch.int64)
     X = inputs.fat_links(L, seed, s).numpy()
     W = inputs.naik_links(L, seed, s).numpy()
-    b = inputs.sources(L, seed, s, cfg["nrhs"]).numpy()
+    b = inputs.sources(L, seed, s, 1).numpy()
     par = oracle.site_parity(L)
     b[:, par == 1, :] = 0
+    mass = cfg["mass"] if cfg["mass"] is not None else 0.1
     t0 = time.perf_counter()
-    oracle.cg(L, X, W, cfg["mass"], 1e-30, b, max_iter=1)
+    oracle.cg(L, X, W, mass, 1e-30, b, max_iter=1)
     t1 = time.perf_counter() - t0
     iters = max(2, min(2000, int(budget_s / max(t1 / 2, 1e-3))))   # 1 iteration = 2 A-applies incl. the final check
     t0 = time.perf_counter()
-    oracle.cg(L, X, W, cfg["mass"], 1e-30, b, max_iter=iters)
+    oracle.cg(L, X, W, mass, 1e-30, b, max_iter=iters)
     dt = time.perf_counter() - t0
-    n_dslash = 2 * (iters + 1) * cfg["nrhs"]                         # + the final true-residual application
+    n_dslash = 2 * (iters + 1)                                       # + the final true-residual application
     gflops = FLOP_PER_SITE * (V // 2) * n_dslash / dt / 1e9
-    return gflops, dt, iters, oracle.threads()
+    sample = (f"{iters} CG iterations (2 Dslash each, + 1 final residual) of 1 of the {cfg['nrhs']} right-hand sides on a "
+              f"{L[0]}x{L[1]}x{L[2]}x{L[3]} " + ("lattice (the config's own)" if tuple(L) == tuple(cfg["L"]) else
+                                                f"block of the {'x'.join(map(str, cfg['L']))} lattice (same generators)") + f", {dt:.1f} s")
+    return gflops, dt, sample, oracle.threads()
 
 
-def run_reference(args, cfg, rank, world):
+def run_reference(args, cfg, rank):
     if rank != 0:
         return
     vals, dts = [], []
     for i in range(args.warmup + args.steps):
-        g, dt, iters, cores = oracle_sample(cfg, 0, args.ref_budget)
+        g, dt, sample, cores = oracle_sample(cfg, 0, args.ref_budget)
         if i >= args.warmup:
             vals.append(g)
             dts.append(dt)
     v = sum(vals) / len(vals)
-    sample = f"{iters} CG iterations (2 Dslash each, + 1 final residual) of the {args.config} solve per step"
     print(json.dumps({
         "impl": "reference", "metric": "hisq_dslash_gflops", "value": v, "unit": "GFLOP/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(dts) / len(dts), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(args.config, cfg)},
-        "cpu_baseline": {"value": v, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": v, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample + " per step"},
         "e2e": {"value": v, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
 
-def workload_name(name, cfg):
-    L = cfg["L"]
-    return (f"{name}: {L[0]}x{L[1]}x{L[2]}x{L[3]} {cfg['prec']} nRHS={cfg['nrhs']} CG m={cfg['mass']} tol={cfg['tol']}, "
-            "Gaussian fat links (std 0.3), Haar SU(3) Naik x(-1/24), phases folded, antiperiodic t")
+# ---- blocks for the BASELINE configs that are not the headline ----------------------------------------------------------
+def timed_solve(ctx, b, cfg, x):
+    """One warm-up solve, then one timed with CUDA events."""
+    ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
+    torch.cuda.synchronize()
+    l0 = ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    _, info = ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
+    e1.record()
+    e1.synchronize()
+    ms = e0.elapsed_time(e1)
+    it = max(info["iterations"], 1)
+    return {"solve_ms": ms, "iterations": info["iterations"], "true_residual_checks": info["reliable_updates"],
+            "ms_per_iteration": ms / it, "true_rel_resid": info["true_rel_resid"],
+            "kernels_per_iteration": (ctx.launch_count() - l0) / it}
+
+
+def config_block(name, dev, peak, ctxpk, reps):
+    """Dslash and full CG of one BASELINE config (C1, C2, C4), each with its own clock sample."""
+    from paper_2306_01098_b200 import binding
+    cfg = CONFIGS[name]
+    sampler = ClockSampler(dev.index or 0).start()
+    ctx, gen_dev = make_ctx(cfg, dev, 0)
+    n = cfg["nrhs"]
+    b = ctx.pack(binding.make_sources(cfg["L"], 0, n, 0, dev, ctx.cdtype, gen_device=gen_dev))
+    x = ctx.new_field(n)
+    out = {"workload": workload_name(name, cfg), "cg": timed_solve(ctx, b, cfg, x)}
+    if name == "C1":
+        # the launch-latency regime: the first solve of a context also captures and instantiates its CUDA graphs
+        c2, _ = make_ctx(cfg, dev, 0)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        c2.cg(b, cfg["mass"], cfg["tol"], x=x)
+        torch.cuda.synchronize()
+        out["cg"]["first_solve_ms_incl_graph_capture"] = 1e3 * (time.perf_counter() - t0)
+        c2.close()
+    if cfg["prec"] == "mixed":
+        # the solve spends its time in the fp32 operator (the fp64 one runs once per reliable update): time THAT kernel
+        ctx.close()
+        ctx, _ = make_ctx(cfg, dev, 0, prec="fp32")
+        out["dslash"] = dslash_block(ctx, n, reps, peak, ctxpk)
+        out["dslash"]["kernel"] = f"dslash_kernel<float,NR={n}> (the operator inside the mixed-precision iteration)"
+    else:
+        out["dslash"] = dslash_block(ctx, n, reps, peak, ctxpk)
+        out["dslash"]["kernel"] = f"dslash_kernel<double,NR={n}>"
+    if name == "C1":
+        out["dslash"]["note"] = "4.7 MB of links, L2-resident, 2048 threads: launch-latency bound, no roofline claim"
+    ctx.close()
+    out["clocks"] = sampler.stop()
+    return out
+
+
+def sweep_block(name, L, prec, ns, dev, peak, ctxpk, reps):
+    from paper_2306_01098_b200 import binding
+    sampler = ClockSampler(dev.index or 0).start()
+    ctx = binding.Hisq(L, prec, max(ns), dev)
+    fat, naik = binding.make_links(L, 0, dev, ctx.cdtype, gen_device=dev)
+    ctx.set_links(fat, naik)
+    del fat, naik
+    rows = [dslash_block(ctx, n, reps, peak, ctxpk) for n in ns]
+    ctx.close()
+    return {"workload": f"{name}: {L[0]}x{L[1]}x{L[2]}x{L[3]} {prec} Dslash vs nRHS", "rows": rows, "clocks": sampler.stop()}
+
+
+# Table 1 of the paper (PAPER.md:604-616): Dslash TFLOP/s on a 32^4 lattice, other hardware -- context, not a target
+PAPER_TABLE1 = {"nrhs": [1, 2, 3, 4, 6, 8], "A100_fp32": [1.36, 2.36, 2.85, 3.98, 4.97, 4.95], "A100_fp64": [0.70, 1.19, 1.45, 1.92, 2.20, 2.51],
+                "MI250x_GCD_fp32": [0.93, 1.65, 2.06, 2.36, 2.96, 2.79], "MI250x_GCD_fp64": [0.45, 0.85, 1.14, 0.97, 0.91, 0.95]}
+
+
+def sweep_paper_shape(dev, peak, ctxpk, reps):
+    """The paper's own benchmark shape (32^4, nRHS = 1,2,3,4,6,8, fp32 and fp64; Fig. 5 / Table 1), on this B200."""
+    res = {"workload": "32x32x32x32 Dslash, TFLOP/s at 1146 flop/site/RHS", "paper_table1_context": PAPER_TABLE1}
+    for prec in ("fp32", "fp64"):
+        blk = sweep_block("P", (32, 32, 32, 32), prec, PAPER_TABLE1["nrhs"], dev, peak, ctxpk, reps)
+        res["b200_" + prec] = [round(r["gflops"] / 1e3, 3) for r in blk["rows"]]
+    return res
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` (N > 1) outside torchrun: start the N ranks ourselves, one process per GPU."""
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
+def capped_steps(ctx, b, x, cfg, steps, host=None):
+    """`steps` capped solves back to back, one pair of CUDA events around them.  Returns (ms, Dslash applications, info)."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    nd, info = 0, None
+    e0.record()
+    for _ in range(steps):
+        if host is None:
+            _, info = ctx.cg(b, cfg["mass"], cfg["tol"], x=x, strict=False)
+        else:
+            _, info = ctx.cg_host(host[0], host[1], cfg["mass"], cfg["tol"], strict=False)
+        nd += 2 * (info["iterations"] + info["reliable_updates"])
+    e1.record()
+    e1.synchronize()
+    return e0.elapsed_time(e1), nd, info
 
 
 def main():
@@ -201,27 +376,30 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="C2", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--mode", default="replicas", choices=["replicas", "partitioned"])
+    ap.add_argument("--config", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--only", default="all", choices=["all", "dslash", "smear"],
                     help="dslash: time only the Dslash kernel of --config at --nrhs; smear: only hisq_smear on --config's "
                          "lattice (profiling drivers)")
     ap.add_argument("--nrhs", type=int, default=0, help="override the config's nRHS (--only dslash)")
-    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--step-iters", type=int, default=64, help="CG iterations of one timed step (0: a full solve per step)")
+    ap.add_argument("--no-full-solve", action="store_true", help="skip the one full solve of the headline config")
+    ap.add_argument("--no-configs", action="store_true", help="skip the C1-C4 blocks and the paper-shape sweep")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-multishift", action="store_true")
-    ap.add_argument("--no-compression", action="store_true")
-    ap.add_argument("--no-partition", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the rows f1, f2, f4 (multi-shift, compression, smearing, M solve) on C2")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--ref-budget", type=float, default=10.0)
-    ap.add_argument("--dslash-reps", type=int, default=100)
+    ap.add_argument("--dslash-reps", type=int, default=0, help="launch pairs per burst (0: 10 on C5, 100 otherwise)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     cfg = CONFIGS[args.config]
+    if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        respawn_under_torchrun(args)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
-        return run_reference(args, cfg, rank, world)
+        return run_reference(args, cfg, rank)
     if args.only == "dslash":
         return run_dslash_only(args, cfg)
     if args.only == "smear":
@@ -232,26 +410,28 @@ def main():
     from paper_2306_01098_b200 import binding
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: libhisq has no CPU fallback")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
+    ndev = torch.cuda.device_count()
+    torch.cuda.set_device(local % ndev)
+    dev = torch.device("cuda", local % ndev)
     dist = None
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
+        # ranks that share a GPU (fewer devices than ranks: functional runs only) cannot use NCCL between them
+        dist.init_process_group("nccl" if ndev >= world else "gloo", **({"device_id": dev} if ndev >= world else {}))
+    if args.mode == "partitioned":
+        return run_partitioned(args, cfg, rank, world, dev, dist)
+    agg_dev = dev if (dist is None or dist.get_backend() == "nccl") else torch.device("cpu")
 
     L, n = cfg["L"], cfg["nrhs"]
-    w = 4 if cfg["prec"] == "fp32" else 8
-    big = binding.layout.volume(L) > (1 << 21)
-    gen_dev = dev if big else None                      # small lattices: CPU generation, bit-identical to the oracle's inputs
-    ctx = binding.Hisq(L, cfg["prec"], n, dev)
-    fat, naik = binding.make_links(L, rank, dev, ctx.cdtype, gen_device=gen_dev)
-    ctx.set_links(fat, naik)
-    del fat, naik
+    prec = cfg["prec"]
+    w = 4 if prec == "fp32" else 8
+    reps = args.dslash_reps or (10 if binding.layout.volume(L) > (1 << 23) else 100)
+    peak, peak_src = measured_peaks()
+    ctxpk = context_peaks()
+    ctx, gen_dev = make_ctx(cfg, dev, rank)
     b_can = binding.make_sources(L, rank, n, 0, dev, ctx.cdtype, gen_device=gen_dev)
     b = ctx.pack(b_can)
     x = ctx.new_field(n)
-    b_host = b_can.cpu().pin_memory()
-    x_host = torch.empty_like(b_host).pin_memory()
     Vh = ctx.Vh
 
     def barrier():
@@ -259,218 +439,247 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # ---- ONE full solve of the headline config (also the first warm-up): time, iterations, true residuals ----
+    full = None
+    if not args.no_full_solve:
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = ctx.launch_count()
+        e0.record()
+        _, fi = ctx.cg(b, cfg["mass"], cfg["tol"], x=x, strict=False)
+        e1.record()
+        e1.synchronize()
+        fms, fit = e0.elapsed_time(e1), max(fi["iterations"], 1)
+        nd_full = 2 * (fi["iterations"] + fi["reliable_updates"])
+        full = {"solve_ms": fms, "iterations": fi["iterations"], "true_residual_checks": fi["reliable_updates"],
+                "status": fi["status"], "true_rel_resid": fi["true_rel_resid"], "ms_per_iteration": fms / fit,
+                "kernels_per_iteration": (ctx.launch_count() - l0) / fit,
+                "gflops_whole_solve": FLOP_PER_SITE * Vh * n * nd_full / (fms * 1e-3) / 1e9,
+                "cg_model_gbs": (2 * (288 + 12 * n) + 54 * n) * w * Vh * fit / (fms * 1e-3) / 1e9,
+                "note": "first solve of the context: includes CUDA-graph capture and instantiation"}
+
     # ---- the step, device-resident inputs ----
+    if args.step_iters > 0:
+        ctx.set_option("max_iter", args.step_iters)
     for _ in range(args.warmup):
-        _, info = ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
-    # settle: keep warming up (at most 8 more solves) until two consecutive solves agree to 3 % -- boxes have been
+        ctx.cg(b, cfg["mass"], cfg["tol"], x=x, strict=False)
+    # settle: keep warming up (at most 8 more steps) until two consecutive steps agree to 3 % -- boxes have been
     # seen to run the first seconds after other heavy work up to 1.4x slower with no throttle reason reported
     extra, prev = 0, None
     while extra < 8:
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
+        dt, _, _ = capped_steps(ctx, b, x, cfg, 1)
         extra += 1
         if prev is not None and abs(dt - prev) <= 0.03 * prev:
             break
         prev = dt
-    sampler = ClockSampler(local)
-    sampler.start()
+    sampler = ClockSampler(dev.index or 0).start()
     barrier()
     l0 = ctx.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    n_dslash = 0
-    for _ in range(args.steps):
-        _, info = ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
-        n_dslash += 2 * (info["iterations"] + info["reliable_updates"])
-    e1.record()
+    ms, n_dslash, info = capped_steps(ctx, b, x, cfg, args.steps)
     barrier()
-    ms = e0.elapsed_time(e1)
     launches = ctx.launch_count() - l0
     clocks = sampler.stop()
-    ms_all, flops_all = aggregate(ms, float(FLOP_PER_SITE) * Vh * n * n_dslash, dist, dev)
+    ms_all, flops_all = aggregate(ms, float(FLOP_PER_SITE) * Vh * n * n_dslash, dist, agg_dev)
     value = flops_all / (ms_all * 1e-3) / 1e9
 
     # ---- the same step end to end: pinned host buffers through hisq_cg_host ----
-    ctx.cg_host(x_host, b_host, cfg["mass"], cfg["tol"])
+    b_host = b_can.cpu().pin_memory()
+    x_host = torch.empty_like(b_host).pin_memory()
+    del b_can
+    ctx.cg_host(x_host, b_host, cfg["mass"], cfg["tol"], strict=False)
     barrier()
-    t0 = time.perf_counter()
-    e0.record()
-    nd2 = 0
-    for _ in range(args.steps):
-        _, info2 = ctx.cg_host(x_host, b_host, cfg["mass"], cfg["tol"])
-        nd2 += 2 * (info2["iterations"] + info2["reliable_updates"])
-    e1.record()
+    ms2, nd2, _ = capped_steps(ctx, b, x, cfg, args.steps, host=(x_host, b_host))
     barrier()
-    ms2 = max(e0.elapsed_time(e1), 0.0)
-    ms2_all, f2_all = aggregate(ms2, float(FLOP_PER_SITE) * Vh * n * nd2, dist, dev)
+    ms2_all, f2_all = aggregate(ms2, float(FLOP_PER_SITE) * Vh * n * nd2, dist, agg_dev)
     e2e_val = f2_all / (ms2_all * 1e-3) / 1e9
     field_bytes = b_host.numel() * b_host.element_size()
+    del b_host, x_host
 
-    # ---- the dominant kernel alone: Dslash, CUDA-event timed ----
-    d_ms = min(time_dslash(ctx, n, args.dslash_reps) for _ in range(3))   # best of 3 bursts of 2*reps launches
-    peak, peak_src = measured_peaks()
-    alg_bytes = dslash_bytes(Vh, n, w)
-    achieved = alg_bytes / (d_ms * 1e-3) / 1e9
-    dsl = {"ms": d_ms, "gflops": FLOP_PER_SITE * Vh * n / (d_ms * 1e-3) / 1e9, "alg_gbs": achieved,
-           "paper_model_gbs": (288 + 102 * n) * w * Vh / (d_ms * 1e-3) / 1e9,
-           "frac_of_measured_copy": achieved / peak, "frac_of_8TBs": achieved / 8000.0,
-           "frac_of_measured_read_only": achieved / READ_ONLY_GBS,
-           "frac_of_fma_peak": FLOP_PER_SITE * Vh * n / (d_ms * 1e-3) / 1e9 / FMA_PEAK_GFLOPS[w], "tiles": ctx.tiles(n)}
-    # ---- row f4 (part): the full system (D + m) x = b on both parities, same lattice, mass and tol, one solve ----
-    full = None
-    if not args.no_multishift and rank == 0:
-        bo = ctx.pack(binding.make_sources(L, rank, n, 1, dev, ctx.cdtype, gen_device=gen_dev))
-        ctx.solve_M(b, bo, cfg["mass"], cfg["tol"])
-        torch.cuda.synchronize()
-        e0.record()
-        _, _, fi = ctx.solve_M(b, bo, cfg["mass"], cfg["tol"])
-        e1.record()
-        e1.synchronize()
-        full = {"what": "hisq_solve_M: s_e = m b_e - D_eo b_o, CG on the even system, x_o = (b_o - D_oe x_e) / m",
-                "solve_ms": e0.elapsed_time(e1), "iterations": fi["iterations"],
-                "full_lattice_rel_resid": fi["true_rel_resid"]}
-        del bo
-    # ---- row f4: HISQ smearing of seeded thin links on the same lattice (set-up work: time and launches, context) ----
-    smear = None
-    if not args.no_multishift and rank == 0:
-        thin = binding.make_thin_links(L, rank, dev, ctx.cdtype, 0.3, gen_device=gen_dev)
-        ctx.smear(thin)
-        torch.cuda.synchronize()
-        l0 = ctx.launch_count()
-        e0.record()
-        ctx.smear(thin)
-        e1.record()
-        e1.synchronize()
-        smear = {"what": "hisq_smear: fat7 -> U(3) projection -> fat7 + Lepage, Naik product, phases folded",
-                 "ms": e0.elapsed_time(e1), "launches": int(ctx.launch_count() - l0),
-                 "thin_links": "Gram-Schmidt of 1 + 0.3 x Gaussian (seeded stand-in for a thermalised configuration)"}
-        # the chain a production run uses: smeared links (U(3) Naik links, 14-real compression) -> full-system solve
-        sfat, snaik, _ = ctx.smear(thin, fat_scale=0.5, naik_scale=-0.5 / 24.0)
-        del thin
-        sc = binding.Hisq(L, cfg["prec"], n, dev)
-        sc.set_option("naik_compress", 1)
-        sc.set_links(sfat, snaik)
-        del sfat, snaik
-        bo = sc.pack(binding.make_sources(L, rank, n, 1, dev, sc.cdtype, gen_device=gen_dev))
-        sc.solve_M(b, bo, cfg["mass"], cfg["tol"])
-        torch.cuda.synchronize()
-        e0.record()
-        _, _, si = sc.solve_M(b, bo, cfg["mass"], cfg["tol"])
-        e1.record()
-        e1.synchronize()
-        smear["solve_on_smeared_links"] = {"naik_compressed": bool(sc.naik_compressed()), "solve_ms": e0.elapsed_time(e1),
-                                           "iterations": si["iterations"], "full_lattice_rel_resid": si["true_rel_resid"],
-                                           "dslash_ms": time_dslash(sc, n, args.dslash_reps)}
-        sc.close()
-        del sc, bo
-    # ---- row f2: the same Dslash and solve with compressed Naik links (14 instead of 18 reals per Naik link) ----
-    comp = None
-    if not args.no_compression:
-        ctx.close()
-        ctx = binding.Hisq(L, cfg["prec"], n, dev)
-        ctx.set_option("naik_compress", 1)
-        fat, naik = binding.make_links(L, rank, dev, ctx.cdtype, gen_device=gen_dev)
-        ctx.set_links(fat, naik)
-        del fat, naik
-        if ctx.naik_compressed():
-            c_ms = time_dslash(ctx, n, args.dslash_reps)
-            ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
-            torch.cuda.synchronize()
-            e0.record()
-            _, ci = ctx.cg(b, cfg["mass"], cfg["tol"], x=x)
-            e1.record()
-            e1.synchronize()
-            stored = (8 * 18 + 8 * 14 + 12 * n) * w * Vh
-            comp = {"format": "Naik links as 14 reals (rows 0,1 and d = det/|row0 x row1|^2; exact for c x U(3)), fat links 18", "dslash_ms": c_ms,
-                    "dslash_gflops": FLOP_PER_SITE * Vh * n / (c_ms * 1e-3) / 1e9,
-                    "stored_bytes_per_launch": stored, "stored_gbs": stored / (c_ms * 1e-3) / 1e9,
-                    "uncompressed_alg_gbs": alg_bytes / (c_ms * 1e-3) / 1e9, "speedup_vs_full": d_ms / c_ms,
-                    "cg_solve_ms": e0.elapsed_time(e1), "cg_iterations": ci["iterations"],
-                    "cg_true_rel_resid": ci["true_rel_resid"]}
-    # ---- row f1: multi-shift CG on the same lattice (10 shifts over 5 decades), one solve ----
-    ms = None
-    if not args.no_multishift and cfg["prec"] != "mixed" and n == 1:
-        import numpy as np
-        shifts = [0.0] + [float(v) for v in np.geomspace(1e-4, 5.0, 9)]
-        ctx.close()
-        ctx = binding.Hisq(L, cfg["prec"], len(shifts), dev)
-        fat, naik = binding.make_links(L, rank, dev, ctx.cdtype, gen_device=gen_dev)
-        ctx.set_links(fat, naik)
-        del fat, naik
-        xs = ctx.new_field(len(shifts))
-        ctx.cg_multishift(b, cfg["mass"], shifts, cfg["tol"], x=xs)
-        torch.cuda.synchronize()
-        e0.record()
-        _, mi = ctx.cg_multishift(b, cfg["mass"], shifts, cfg["tol"], x=xs)
-        e1.record()
-        e1.synchronize()
-        ms = {"shifts": len(shifts), "solve_ms": e0.elapsed_time(e1), "iterations": mi["iterations"],
-              "ms_per_iteration": e0.elapsed_time(e1) / max(mi["iterations"], 1), "max_true_rel_resid": max(mi["true_rel_resid"])}
-        del xs
+    # ---- the dominant kernel alone: the Dslash at the headline nRHS, CUDA-event timed ----
+    dsl = dslash_block(ctx, n, reps, peak, ctxpk)
+    kernel = f"dslash_kernel<{'float' if prec != 'fp64' else 'double'},NR={min(n, 8)}>"
+    if prec == "mixed":
+        c32, _ = make_ctx(cfg, dev, rank, prec="fp32")
+        dsl = dslash_block(c32, n, reps, peak, ctxpk)
+        c32.close()
+    traffic, traffic_src = ncu_traffic(args.config, "fp32" if prec == "mixed" else prec, n)
     ctx.close()
     del ctx, b, x
-    # ---- row f3: the same solve on a t-partitioned context with ONE rank (ring closed on itself): what the multi-GPU
-    # machinery (mailbox halos and all-reduces, unfused updates) costs per iteration on one GPU.  Context, not a scaling number.
-    part = None
-    if not args.no_partition and cfg["prec"] != "mixed" and rank == 0 and L[3] >= 4 and L[3] % 2 == 0:
-        from paper_2306_01098_b200 import partition
-        pc = binding.Hisq(L, cfg["prec"], n, dev, part=(0, 1))
-        fat, naik = partition.make_links_part(L, rank, 0, 1, dev, pc.cdtype, gen_device=gen_dev)
-        pc.set_links(fat, naik)
-        del fat, naik
-        pb = pc.pack(partition.make_sources_part(L, rank, n, 0, 0, 1, dev, pc.cdtype, gen_device=gen_dev))
-        peer = partition.PeerHalo(pc, 0, 1, n)
-        px = pc.new_field(n)
-        pc.cg(pb, cfg["mass"], cfg["tol"], x=px)
-        torch.cuda.synchronize()
-        e0.record()
-        _, pi = pc.cg(pb, cfg["mass"], cfg["tol"], x=px)
-        e1.record()
-        e1.synchronize()
-        part = {"ranks": 1, "transport": "peer mailboxes (ring closed on the rank)", "solve_ms": e0.elapsed_time(e1),
-                "iterations": pi["iterations"], "ms_per_iteration": e0.elapsed_time(e1) / max(pi["iterations"], 1),
-                "true_rel_resid": pi["true_rel_resid"]}
-        peer.close()
-        pc.close()
-        del pc, pb, px
+    torch.cuda.empty_cache()
 
     out = {
         "metric": "hisq_dslash_gflops", "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "warmup_extra_settle": extra, "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": {"fp32": "f32", "fp64": "f64", "mixed": "f32+f64"}[cfg["prec"]], "data": "synthetic",
-        "config": {"workload": workload_name(args.config, cfg), "l2": "inputs larger than L2 (links %.0f MB)" % (2 * 4 * 2 * Vh * 18 * w / 1e6),
+        "warmup": args.warmup, "warmup_extra_settle": extra, "ms_per_step": ms_all / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": {"fp32": "f32", "fp64": "f64", "mixed": "f32+f64"}[prec],
+        "data": "synthetic",
+        "config": {"workload": workload_name(args.config, cfg),
+                   "step": (f"one hisq_cg call capped at {args.step_iters} iterations + its closing fp64 true-residual check "
+                            "(HISQ_ENOCONV expected)") if args.step_iters > 0 else "one full hisq_cg solve",
+                   "l2": "inputs larger than L2 (links %.0f MB read per Dslash)" % (16 * 18 * w * Vh / 1e6),
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
-        "cg": {"solve_ms": ms_all / args.steps, "iterations": info["iterations"], "true_residual_checks": info["reliable_updates"],
-               "true_rel_resid": info["true_rel_resid"], "ms_per_iteration": ms_all / args.steps / max(info["iterations"], 1)},
-        "dslash": dsl,
-        "multishift_cg": ms,
-        "full_system_solve": full,
-        "link_smearing": smear,
-        "partitioned_cg": part,
-        "naik_compression": comp,
-        "roofline": {"bound": "hbm", "kernel": f"dslash_kernel<{'float' if w == 4 else 'double'},NR={min(n, 8 if w == 4 else 4)}>",
-                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": ncu_traffic(args.config, cfg["prec"], n),
-                     "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
-                     "timing": f"CUDA events around {2 * args.dslash_reps} back-to-back hisq_dslash calls (alternating parity), best of 3 bursts; the library launches them with programmatic dependent launch: the head of call i+1 overlaps the tail of call i (~2 us per call)"},
+        "step": {"iterations": info["iterations"], "true_residual_checks": info["reliable_updates"],
+                 "ms_per_iteration": ms_all / args.steps / max(info["iterations"], 1)},
+        "cg": full, "dslash": dsl,
+        "roofline": {"bound": "hbm", "kernel": kernel, "achieved": dsl["alg_gbs"], "peak": peak, "unit": "GB/s",
+                     "frac": dsl["alg_gbs"] / peak, "traffic": traffic, "traffic_source": traffic_src,
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": dsl["algorithmic_bytes"],
+                     "frac_of_measured_read_only_stream": dsl["frac_of_measured_read_only"],
+                     "timing": dsl["timing"] + " (alternating parity); the library launches them with programmatic dependent "
+                               "launch: the head of call i+1 overlaps the tail of call i (~2 us per call)",
+                     "note": "a frac above 1 is possible for the n <= 2 shapes: the kernel is ~96 % reads and the peak is a "
+                             "read+write copy (the read-only stream of this pool is profiles/peaks.json read_only_gbs)"},
         "e2e": {"value": e2e_val, "unit": "GFLOP/s", "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": field_bytes,
                 "ms_per_step": ms2_all / args.steps},
         "gpu_launches": int(launches), "clocks": clocks,
     }
-
-    if rank == 0 and not args.no_sweep:
-        out["sweep"] = sweep_c3(dev, peak, args.dslash_reps)
-    if rank == 0 and not args.no_sweep:
-        out["paper_shape_sweep"] = sweep_paper_shape(dev, max(10, args.dslash_reps // 4))
+    if rank == 0 and not args.no_configs:
+        out["configs"] = [config_block("C1", dev, peak, ctxpk, 100), config_block("C2", dev, peak, ctxpk, 100),
+                          sweep_block("C3", (64, 64, 64, 16), "fp32", (1, 2, 4, 8), dev, peak, ctxpk, 25),
+                          config_block("C4", dev, peak, ctxpk, 50)]
+        out["paper_shape_sweep"] = sweep_paper_shape(dev, peak, ctxpk, 25)
+    if rank == 0 and not args.no_extras:
+        out["extras_c2"] = extras_c2(dev, peak, ctxpk)
     if rank == 0 and not args.no_cpu_baseline:
-        g, dt, iters, cores = oracle_sample(cfg, 0, args.cpu_budget)
-        out["cpu_baseline"] = {"value": g, "unit": "GFLOP/s", "cores": cores, "kind": "oracle",
-                               "sample": f"{iters} CG iterations (2 Dslash each, + 1 final residual) of the {args.config} solve, {dt:.1f} s"}
+        g, dt, sample, cores = oracle_sample(cfg, 0, args.cpu_budget)
+        out["cpu_baseline"] = {"value": g, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample}
     if rank == 0:
         print(json.dumps(out))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def extras_c2(dev, peak, ctxpk):
+    """Rows f1, f2, f4 of SURVEY 8 on C2's lattice (32^3 x 8, fp64, n = 1), one timed call each: context, not headline."""
+    import numpy as np
+    from paper_2306_01098_b200 import binding
+    cfg = CONFIGS["C2"]
+    L, n = cfg["L"], 1
+    ctx, gen_dev = make_ctx(cfg, dev, 0)
+    b = ctx.pack(binding.make_sources(L, 0, n, 0, dev, ctx.cdtype, gen_device=gen_dev))
+    bo = ctx.pack(binding.make_sources(L, 0, n, 1, dev, ctx.cdtype, gen_device=gen_dev))
+    x = ctx.new_field(n)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    out = {}
+    base = dslash_block(ctx, n, 100, peak, ctxpk, bursts=1)
+    # f4 (part): the full system (D + m) x = b on both parities
+    ctx.solve_M(b, bo, cfg["mass"], cfg["tol"])
+    torch.cuda.synchronize()
+    e0.record()
+    _, _, fi = ctx.solve_M(b, bo, cfg["mass"], cfg["tol"])
+    e1.record()
+    e1.synchronize()
+    out["full_system_solve"] = {"what": "hisq_solve_M: s_e = m b_e - D_eo b_o, CG on the even system, x_o = (b_o - D_oe x_e) / m",
+                                "solve_ms": e0.elapsed_time(e1), "iterations": fi["iterations"],
+                                "full_lattice_rel_resid": fi["true_rel_resid"]}
+    # f4: HISQ smearing of seeded thin links, then the chain a production job uses on the smeared links
+    thin = binding.make_thin_links(L, 0, dev, ctx.cdtype, 0.3, gen_device=gen_dev)
+    ctx.smear(thin)
+    torch.cuda.synchronize()
+    l0 = ctx.launch_count()
+    e0.record()
+    ctx.smear(thin)
+    e1.record()
+    e1.synchronize()
+    out["link_smearing"] = {"what": "hisq_smear: fat7 -> U(3) projection -> fat7 + Lepage, Naik product, phases folded",
+                            "ms": e0.elapsed_time(e1), "launches": int(ctx.launch_count() - l0),
+                            "thin_links": "Gram-Schmidt of 1 + 0.3 x Gaussian (seeded stand-in for a thermalised configuration)"}
+    sfat, snaik, _ = ctx.smear(thin, fat_scale=0.5, naik_scale=-0.5 / 24.0)
+    del thin
+    sc = binding.Hisq(L, cfg["prec"], n, dev)
+    sc.set_option("naik_compress", 1)
+    sc.set_links(sfat, snaik)
+    del sfat, snaik
+    sc.solve_M(b, bo, cfg["mass"], cfg["tol"])
+    torch.cuda.synchronize()
+    e0.record()
+    _, _, si = sc.solve_M(b, bo, cfg["mass"], cfg["tol"])
+    e1.record()
+    e1.synchronize()
+    out["link_smearing"]["solve_on_smeared_links"] = {"naik_compressed": bool(sc.naik_compressed()), "solve_ms": e0.elapsed_time(e1),
+                                                      "iterations": si["iterations"], "full_lattice_rel_resid": si["true_rel_resid"],
+                                                      "dslash_ms": time_dslash(sc, n, 100)}
+    sc.close()
+    ctx.close()
+    # f2: the same Dslash and solve with compressed Naik links (14 instead of 18 reals per Naik link)
+    cc, _ = make_ctx(cfg, dev, 0, compress=True)
+    if cc.naik_compressed():
+        cb = dslash_block(cc, n, 100, peak, ctxpk, bursts=1)
+        cs = timed_solve(cc, b, cfg, x)
+        stored = (8 * 18 + 8 * 14 + 12 * n) * 8 * cc.Vh
+        out["naik_compression"] = {"format": "Naik links as 14 reals (rows 0,1 and d = det/|row0 x row1|^2; exact for c x U(3)), fat links 18",
+                                   "dslash_ms": cb["ms"], "dslash_gflops": cb["gflops"], "stored_bytes_per_launch": stored,
+                                   "stored_gbs": stored / (cb["ms"] * 1e-3) / 1e9, "uncompressed_alg_gbs": cb["alg_gbs"],
+                                   "speedup_vs_full": base["ms"] / cb["ms"], "cg_solve_ms": cs["solve_ms"],
+                                   "cg_iterations": cs["iterations"], "cg_true_rel_resid": cs["true_rel_resid"]}
+    cc.close()
+    # f1: multi-shift CG (10 shifts over 5 decades)
+    shifts = [0.0] + [float(v) for v in np.geomspace(1e-4, 5.0, 9)]
+    mc, _ = make_ctx(cfg, dev, 0, nrhs=len(shifts))
+    xs = mc.new_field(len(shifts))
+    mc.cg_multishift(b, cfg["mass"], shifts, cfg["tol"], x=xs)
+    torch.cuda.synchronize()
+    e0.record()
+    _, mi = mc.cg_multishift(b, cfg["mass"], shifts, cfg["tol"], x=xs)
+    e1.record()
+    e1.synchronize()
+    out["multishift_cg"] = {"shifts": len(shifts), "solve_ms": e0.elapsed_time(e1), "iterations": mi["iterations"],
+                            "ms_per_iteration": e0.elapsed_time(e1) / max(mi["iterations"], 1),
+                            "max_true_rel_resid": max(mi["true_rel_resid"])}
+    mc.close()
+    return out
+
+
+def run_partitioned(args, cfg, rank, world, dev, dist):
+    """Row f3: ONE lattice cut over `world` ranks, solved by hisq_cg on partitioned contexts; halos and all-reduces go
+    through peer-mapped mailboxes (no communication library on the data path).  Strong scaling: value = the global
+    lattice's Dslash flops / max-over-ranks time.  One rank closes the ring on itself (what the machinery costs)."""
+    from paper_2306_01098_b200 import binding, partition
+    L, n = cfg["L"], cfg["nrhs"]
+    prec = "fp64" if cfg["prec"] == "mixed" else cfg["prec"]
+    grid = binding.rank_grid(L, world)
+    gen_dev = dev if binding.layout.volume(L) > (1 << 21) else None
+    pc = binding.Hisq(L, prec, n, dev, part=(rank, world))
+    fat, naik = partition.make_links_part(L, 0, rank, world, dev, pc.cdtype, gen_device=gen_dev)
+    pc.set_links(fat, naik)
+    del fat, naik
+    pb = pc.pack(partition.make_sources_part(L, 0, n, 0, rank, world, dev, pc.cdtype, gen_device=gen_dev))
+    peer = partition.PeerHalo(pc, rank, world, n, dist=dist)
+    px = pc.new_field(n)
+    if args.step_iters > 0:
+        pc.set_option("max_iter", args.step_iters)
+    for _ in range(args.warmup):
+        pc.cg(pb, cfg["mass"], cfg["tol"], x=px, strict=False)
+    sampler = ClockSampler(dev.index or 0).start()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    l0 = pc.launch_count()
+    ms, nd, info = capped_steps(pc, pb, px, cfg, args.steps)
+    if dist is not None:
+        dist.barrier()
+    clocks = sampler.stop()
+    launches = pc.launch_count() - l0
+    agg_dev = dev if (dist is None or dist.get_backend() == "nccl") else torch.device("cpu")
+    Vh_global = binding.layout.volume(L) // 2
+    ms_all, _ = aggregate(ms, 0.0, dist, agg_dev, sum_flops=False)
+    value = float(FLOP_PER_SITE) * Vh_global * n * nd / (ms_all * 1e-3) / 1e9
+    peer.close()
+    pc.close()
+    if rank == 0:
+        print(json.dumps({
+            "metric": "hisq_dslash_gflops", "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f32" if prec == "fp32" else "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config, cfg), "mode": "partitioned",
+                       "parallelism": f"lattice cut {grid[0]} (z) x {grid[1]} (t) over {world} ranks, peer-mailbox halos and all-reduces",
+                       "devices": torch.cuda.device_count(),
+                       "step": f"one hisq_cg call capped at {args.step_iters} iterations" if args.step_iters > 0 else "one full solve"},
+            "step": {"iterations": info["iterations"], "ms_per_iteration": ms_all / args.steps / max(info["iterations"], 1),
+                     "status": info["status"], "true_rel_resid": info["true_rel_resid"]},
+            "gpu_launches": int(launches), "clocks": clocks,
+            "e2e": None, "roofline": None, "cpu_baseline": None,
+            "note": "strong-scaling mode of row f3; the graded single-GPU line is the default --mode replicas"}))
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
@@ -502,68 +711,17 @@ def run_smear_only(args, cfg):
 
 def run_dslash_only(args, cfg):
     """Profiling driver: only Dslash launches of one config (ncu -k regex:dslash_kernel ...)."""
-    from paper_2306_01098_b200 import binding
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
     torch.cuda.set_device(dev)
-    L = cfg["L"]
     n = args.nrhs if args.nrhs > 0 else cfg["nrhs"]
     prec = "fp64" if cfg["prec"] == "mixed" else cfg["prec"]
-    w = 4 if prec == "fp32" else 8
-    ctx = binding.Hisq(L, prec, n, dev)
-    fat, naik = binding.make_links(L, 0, dev, ctx.cdtype, gen_device=dev)
-    ctx.set_links(fat, naik)
-    del fat, naik
-    ms = time_dslash(ctx, n, args.dslash_reps)
-    peak, src = measured_peaks()
-    by = dslash_bytes(ctx.Vh, n, w)
-    print(json.dumps({"only": "dslash", "config": args.config, "L": L, "prec": prec, "nrhs": n, "ms": ms,
-                      "gflops": FLOP_PER_SITE * ctx.Vh * n / (ms * 1e-3) / 1e9, "alg_gbs": by / (ms * 1e-3) / 1e9,
-                      "frac_of_measured_copy": by / (ms * 1e-3) / 1e9 / peak, "frac_of_8TBs": by / (ms * 1e-3) / 1e9 / 8000.0,
-                      "tiles": ctx.tiles(n), "launches": ctx.launch_count()}))
+    ctx, _ = make_ctx(dict(cfg, L=cfg["L"]), dev, 0, nrhs=n, prec=prec)
+    peak, _ = measured_peaks()
+    blk = dslash_block(ctx, n, args.dslash_reps or 10, peak, context_peaks(), bursts=1)
+    blk.update({"only": "dslash", "config": args.config, "L": cfg["L"], "prec": prec, "launches": ctx.launch_count(),
+                "kernel_source_hash": kernel_source_hash()})
+    print(json.dumps(blk))
     ctx.close()
-
-
-# Table 1 of the paper (PAPER.md:604-616): Dslash TFLOP/s on a 32^4 lattice, other hardware -- context, not a target
-PAPER_TABLE1 = {"nrhs": [1, 2, 3, 4, 6, 8], "A100_fp32": [1.36, 2.36, 2.85, 3.98, 4.97, 4.95], "A100_fp64": [0.70, 1.19, 1.45, 1.92, 2.20, 2.51],
-                "MI250x_GCD_fp32": [0.93, 1.65, 2.06, 2.36, 2.96, 2.79], "MI250x_GCD_fp64": [0.45, 0.85, 1.14, 0.97, 0.91, 0.95]}
-
-
-def sweep_paper_shape(dev, reps):
-    """The paper's own benchmark shape (32^4, nRHS = 1,2,3,4,6,8, fp32 and fp64; Fig. 5 / Table 1), on this B200."""
-    from paper_2306_01098_b200 import binding
-    L = (32, 32, 32, 32)
-    res = {"workload": "32x32x32x32 Dslash, TFLOP/s at 1146 flop/site/RHS", "paper_table1_context": PAPER_TABLE1}
-    for prec in ("fp32", "fp64"):
-        ctx = binding.Hisq(L, prec, 8, dev)
-        fat, naik = binding.make_links(L, 0, dev, ctx.cdtype, gen_device=dev)
-        ctx.set_links(fat, naik)
-        del fat, naik
-        res["b200_" + prec] = [round(FLOP_PER_SITE * ctx.Vh * n / (time_dslash(ctx, n, reps) * 1e-3) / 1e12, 3)
-                               for n in PAPER_TABLE1["nrhs"]]
-        ctx.close()
-    return res
-
-
-def sweep_c3(dev, peak, reps):
-    """configs[2]: 64^3 x 16, fp32 operator, nRHS = 1, 2, 4, 8: Dslash throughput vs nRHS."""
-    from paper_2306_01098_b200 import binding
-    cfg = CONFIGS["C3"]
-    L = cfg["L"]
-    ctx = binding.Hisq(L, "fp32", 8, dev)
-    fat, naik = binding.make_links(L, 0, dev, ctx.cdtype, gen_device=dev)
-    ctx.set_links(fat, naik)
-    del fat, naik
-    rows = []
-    for n in (1, 2, 4, 8):
-        ms = time_dslash(ctx, n, max(10, reps // 4))
-        by = dslash_bytes(ctx.Vh, n, 4)
-        rows.append({"nrhs": n, "ms": ms, "gflops": FLOP_PER_SITE * ctx.Vh * n / (ms * 1e-3) / 1e9,
-                     "alg_gbs": by / (ms * 1e-3) / 1e9, "frac_of_measured_copy": by / (ms * 1e-3) / 1e9 / peak,
-                     "frac_of_8TBs": by / (ms * 1e-3) / 1e9 / 8000.0,
-                     "frac_of_fma_peak": FLOP_PER_SITE * ctx.Vh * n / (ms * 1e-3) / 1e9 / FMA_PEAK_GFLOPS[4],
-                     "tiles": ctx.tiles(n)})
-    ctx.close()
-    return {"workload": "C3: 64x64x64x16 fp32 Dslash", "rows": rows}
 
 
 if __name__ == "__main__":

@@ -76,9 +76,13 @@ size_t hisq_workspace_bytes(const hisq_ctx *h, int nrhs);
  * workspace invalidates links set earlier. */
 int hisq_set_workspace(hisq_ctx *h, void *dev_ptr, size_t bytes);
 
-/* Copy the two CANONICAL link arrays (each 4*V matrices, Eq. (5)) into the library's own layout
- * (structure-of-arrays by 16-byte chunk, split by parity and direction; fp32 and fp64 copies for
- * HISQ_MIXED).  Synchronises the stream before returning: the caller may free fat / naik at once.
+/* Copy the two CANONICAL link arrays (each 4*V matrices, Eq. (5)) into the library's own layout: one RECORD per output
+ * site holding the 16 links its stencil needs (its own 8 forward links and the 8 links of its backward neighbours x - mu,
+ * x - 3 mu, fetched here once), the records of 32 consecutive sites interleaved by 16-byte chunk, so that the Dslash
+ * streams its links as contiguous 3.5 - 4.5 KB runs per warp and stencil term (bulk-copy / TMA friendly) and never
+ * computes a link address.  Every link is stored twice (once forward, once backward): 2 x 16 x 18 reals per site pair of
+ * workspace, the bytes READ per Dslash application stay 16 links per output site.  fp32 and fp64 copies for HISQ_MIXED.
+ * Synchronises the stream before returning: the caller may free fat / naik at once.
  * Links carry all coefficients and phases; the library applies none. */
 int hisq_set_links(hisq_ctx *h, const void *fat, const void *naik);
 
@@ -164,7 +168,7 @@ int hisq_nersc_write(const char *path, const void *links_host, const int *L, int
 /* Options: "max_iter" (default 100000), "reliable_interval" (default 100 for HISQ_MIXED, 0 = off for
  * the others), "check_interval" (iterations enqueued between host polls of the convergence flag,
  * default 32), "use_graph" (1: replay one CG iteration as a CUDA graph, default 1),
- * "dslash_block" (threads per CTA of the Dslash kernel, 0 = default), "nrhs_inner" (RHS per thread, 0 = auto),
+ * "nrhs_inner" (RHS per thread, 0 = auto),
  * "tile_y", "tile_z" (CTA sweep order blocking in y,z; 0 = auto),
  * "naik_compress" (see hisq_naik_compressed; default 0), "fused_blas" (1: cooperative fused x/r/p update kernel when the
  * fields are small enough to stay in registers across a grid barrier, default 1), "window_mb" (L2 budget of the CTA sweep
@@ -287,6 +291,14 @@ long long hisq_launch_count(const hisq_ctx *h);
 const char *hisq_strerror(int code);
 /* Text of the last CUDA error seen by this context ("" if none). */
 const char *hisq_last_error(const hisq_ctx *h);
+
+/* Introspection (tests, DESIGN.md tables; no effect on any result).
+ * hisq_debug_dslash_regs: registers per thread of the Dslash kernel instantiation for prec (HISQ_FP32 | HISQ_FP64),
+ *   nr right-hand sides per thread (1,2,3,4,6,8) and epilogue mode (0 plain, 1 A-apply, 2 residual); -1 if unknown.
+ * hisq_debug_tiles: out[0], out[1] = the (tile_y, tile_z) CTA sweep blocking the next Dslash launch with nrhs
+ *   right-hand sides would use. */
+int hisq_debug_dslash_regs(int prec, int nr, int mode);
+int hisq_debug_tiles(hisq_ctx *h, int nrhs, int *out);
 
 #ifdef __cplusplus
 }

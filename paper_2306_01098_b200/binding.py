@@ -28,7 +28,7 @@ EXPORTS = [
     "hisq_spinor_unpack", "hisq_dslash_host", "hisq_cg_host", "hisq_naik_compressed", "hisq_launch_count",
     "hisq_create_part", "hisq_peer_bytes", "hisq_peer_attach", "hisq_halo_send", "hisq_halo_recv", "hisq_peer_reduce_send", "hisq_peer_reduce_recv", "hisq_dslash_slices", "hisq_dslash_edges", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
     "hisq_cgp_begin", "hisq_cgp_phase", "hisq_cgp_ptr", "hisq_cgp_status", "hisq_strerror",
-    "hisq_last_error",
+    "hisq_last_error", "hisq_debug_dslash_regs", "hisq_debug_tiles",
 ]
 
 _lib = None
@@ -107,6 +107,11 @@ def load_library() -> ctypes.CDLL:
 
 
 _PREC = {"fp32": HISQ_FP32, "fp64": HISQ_FP64, "mixed": HISQ_MIXED}
+
+
+def rank_grid(L: Sequence[int], nranks: int):
+    """(nz, nt): how hisq_create_part cuts the lattice over nranks ranks (rank = rz + nz * rt)."""
+    return (1, int(nranks))
 
 
 class Hisq:

@@ -23,18 +23,15 @@ def _newest_dep() -> float:
     return t
 
 
-def build(force: bool = False, verbose: bool = False, defines=(), lib: str = LIB, block: int = 0) -> str:
-    """defines / lib: experimental variants (e.g. defines=("-DHISQ_ROLL_FROM=3",), lib="/path/libhisq_x.so")."""
-    global OBJ
-    if not defines and not force and os.path.exists(lib) and os.path.getmtime(lib) >= _newest_dep():
-        return lib
-    obj_dir = OBJ if not defines else OBJ + "_" + os.path.basename(lib)
-    os.makedirs(obj_dir, exist_ok=True)
+def build(force: bool = False, verbose: bool = False) -> str:
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_dep():
+        return LIB
+    os.makedirs(OBJ, exist_ok=True)
     nvcc = os.environ.get("NVCC", "nvcc")
 
     def compile_one(src: str) -> str:
-        obj = os.path.join(obj_dir, os.path.splitext(src)[0] + ".o")
-        cmd = [nvcc, *NVCC_FLAGS, *defines, "-c", os.path.join(CSRC, src), "-o", obj]
+        obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
+        cmd = [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd[1:1] = ["-Xptxas", "-v"]
         r = subprocess.run(cmd, capture_output=True, text=True)
@@ -46,12 +43,12 @@ def build(force: bool = False, verbose: bool = False, defines=(), lib: str = LIB
 
     with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
         objs = list(ex.map(compile_one, SOURCES))
-    cmd = [nvcc, "-shared", "-o", lib + ".tmp", *objs]
+    cmd = [nvcc, "-shared", "-o", LIB + ".tmp", *objs]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
-    os.replace(lib + ".tmp", lib)
-    return lib
+    os.replace(LIB + ".tmp", LIB)
+    return LIB
 
 
 if __name__ == "__main__":

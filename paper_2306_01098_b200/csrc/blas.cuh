@@ -71,6 +71,7 @@ __global__ void __launch_bounds__(kBlasBlock) cg_init_kernel(const TB* b, T* r /
             const double bb = totals[kk];
             st->rho[kk] = bb; st->rho_prev[kk] = bb; st->bnorm2[kk] = bb;
             st->pq[kk] = 1.0; st->beta[kk] = 0.0; st->sums[kk] = 0.0;
+            st->alpha[kk] = 0.0; st->xpend[kk] = -1;
             st->active[kk] = bb > 0.0 ? 1 : 0;
         }
         __syncthreads();
@@ -84,35 +85,61 @@ __global__ void __launch_bounds__(kBlasBlock) cg_init_kernel(const TB* b, T* r /
 }
 inline int init_grid_x(size_t nreal) { return (int)((nreal + (size_t)kBlasBlock * kBlasItems * 4 - 1) / ((size_t)kBlasBlock * kBlasItems * 4)); }
 
-// ---- p_k = r_k + beta_k p_k  (first kernel of an iteration; beta = 0 at the start gives p = r) -------
+// ---- [x_k += alpha_k p_k of the PREVIOUS iteration] ; p_k = r_k + beta_k p_k  (first kernel of an iteration; beta = 0 at
+// the start gives p = r).  Folding the x-update into this pass (x is touched nowhere else inside an iteration) saves one
+// read of p per iteration: 48 n instead of 54 n words per site for the BLAS part.  The update of iteration i is
+// pending (st->xpend[k] == i) from the r-update of iteration i until this kernel of iteration i+1, or until
+// cg_flush_x_kernel when the loop is left (true-residual check, reliable update, end of the solve).
+// x == nullptr: plain p-update (partitioned lattices, start of a solve).
 template <typename T>
 __global__ void __launch_bounds__(kBlasBlock) cg_update_p_kernel(T* __restrict__ p, const T* __restrict__ r, size_t nreal,
-                                                                 const CgState* st, Span sp = Span())
+                                                                 const CgState* st, Span sp = Span(), T* __restrict__ x = nullptr,
+                                                                 int flush_only = 0)
 {
-    if (st->done) return;
+    if (st->done && !flush_only) return;
     using V = typename V16<T>::type;
     constexpr int N = V16<T>::n;
     const int k = blockIdx.y;
-    if (!st->active[k]) return;  // frozen RHS keep their search direction (needed if they are resumed)
-    const T beta = (T)st->beta[k];
+    const bool do_x = x != nullptr && st->xpend[k] == st->iter;
+    const bool do_p = !flush_only && st->active[k] != 0;  // frozen RHS keep their search direction (needed if they are resumed)
+    if (!do_x && !do_p) return;
+    const T beta = (T)st->beta[k], alpha = (T)st->alpha[k];
     const size_t nvec = sp.seg ? 3 * sp.seg : nreal / N;
     V* pv = reinterpret_cast<V*>(p + (size_t)k * nreal);
+    V* xv = reinterpret_cast<V*>(x + (size_t)k * nreal);
     const V* rv = reinterpret_cast<const V*>(r + (size_t)k * nreal);
-    V rr[kBlasItems], pp[kBlasItems];
+    V rr[kBlasItems], pp[kBlasItems], xx[kBlasItems];
 #pragma unroll
     for (int it = 0; it < kBlasItems; ++it) {
         size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
-        if (i < nvec) { const size_t j = span_map(sp, i); rr[it] = rv[j]; pp[it] = pv[j]; }
+        if (i < nvec) {
+            const size_t j = span_map(sp, i);
+            pp[it] = pv[j];
+            if (do_p) rr[it] = rv[j];
+            if (do_x) xx[it] = xv[j];
+        }
     }
 #pragma unroll
     for (int it = 0; it < kBlasItems; ++it) {
         size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
         if (i < nvec) {
-            T a[N], b[N];
-            unpack16<T>(rr[it], a); unpack16<T>(pp[it], b);
+            const size_t j = span_map(sp, i);
+            T b[N];
+            unpack16<T>(pp[it], b);
+            if (do_x) {
+                T c[N];
+                unpack16<T>(xx[it], c);
 #pragma unroll
-            for (int e = 0; e < N; ++e) b[e] = fma(beta, b[e], a[e]);
-            pv[span_map(sp, i)] = pack16<T>(b);
+                for (int e = 0; e < N; ++e) c[e] = fma(alpha, b[e], c[e]);
+                xv[j] = pack16<T>(c);
+            }
+            if (do_p) {
+                T a[N];
+                unpack16<T>(rr[it], a);
+#pragma unroll
+                for (int e = 0; e < N; ++e) b[e] = fma(beta, b[e], a[e]);
+                pv[j] = pack16<T>(b);
+            }
         }
     }
 }
@@ -122,8 +149,9 @@ template <typename T>
 __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict__ x, T* __restrict__ r, const T* __restrict__ p,
                                                                   const T* __restrict__ q, size_t nreal, CgState* st,
                                                                   double* partial, int defer = 0, PeerPush push = PeerPush(),
-                                                                  const double* red_pq = nullptr, Span sp = Span())
+                                                                  const double* red_pq = nullptr, Span sp = Span(), int fold_x = 0)
 {
+    // fold_x = 1: x is left alone here; alpha_k is handed to the next cg_update_p_kernel pass (st->alpha, st->xpend)
     // defer = 1 (partitioned lattice).  red_pq: <p,q> is not in st->pq yet but, rank by rank, in this slot of the
     // mailbox (every block adds them up itself); push: the last block hands the local ||r||^2 to all ranks.
     if (st->done) {   // finished: keep the other ranks' arrival count right (see dslash_kernel)
@@ -150,23 +178,32 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict_
 #pragma unroll
     for (int it = 0; it < kBlasItems; ++it) {
         size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
-        if (live && i < nvec) { const size_t j = span_map(sp, i); xx[it] = xv[j]; rr[it] = rv[j]; pp[it] = pv[j]; qq[it] = qv[j]; }
+        if (live && i < nvec) {
+            const size_t j = span_map(sp, i);
+            rr[it] = rv[j]; qq[it] = qv[j];
+            if (!fold_x) { xx[it] = xv[j]; pp[it] = pv[j]; }
+        }
     }
     double sum[1] = { 0.0 };
 #pragma unroll
     for (int it = 0; it < kBlasItems; ++it) {
         size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
         if (live && i < nvec) {
-            T a[N], b[N], c[N], d[N];
-            unpack16<T>(xx[it], a); unpack16<T>(rr[it], b); unpack16<T>(pp[it], c); unpack16<T>(qq[it], d);
+            T b[N], d[N];
+            unpack16<T>(rr[it], b); unpack16<T>(qq[it], d);
 #pragma unroll
             for (int e = 0; e < N; ++e) {
-                a[e] = fma(alpha, c[e], a[e]);
                 b[e] = fma(-alpha, d[e], b[e]);
                 sum[0] += (double)b[e] * (double)b[e];
             }
             const size_t j = span_map(sp, i);
-            xv[j] = pack16<T>(a);
+            if (!fold_x) {
+                T a[N], c[N];
+                unpack16<T>(xx[it], a); unpack16<T>(pp[it], c);
+#pragma unroll
+                for (int e = 0; e < N; ++e) a[e] = fma(alpha, c[e], a[e]);
+                xv[j] = pack16<T>(a);
+            }
             rv[j] = pack16<T>(b);
         }
     }
@@ -187,6 +224,10 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict_
             if (st->active[kk]) {
                 const double rn = totals[kk], pq = st->pq[kk];
                 if (!(pq > 0.0) || !isfinite(pq) || !isfinite(rn)) st->breakdown = 1;
+                if (fold_x) {   // the same alpha every block used above; applied to x by the next p-update pass
+                    st->alpha[kk] = (pq > 0.0 && isfinite(pq)) ? st->rho[kk] / pq : 0.0;
+                    st->xpend[kk] = st->iter + 1;
+                }
                 st->rho_prev[kk] = st->rho[kk];
                 st->beta[kk] = rn / st->rho[kk];
                 st->rho[kk] = rn;
@@ -423,6 +464,7 @@ __global__ void cg_after_residual_kernel(CgState* st, double* true_rr_out)
         st->beta[k] = (!conv && consistent && st->rho_prev[k] > 0.0) ? rt / st->rho_prev[k] : 0.0;
         st->rho[k] = rt;
         st->active[k] = (!conv && st->bnorm2[k] > 0.0) ? 1 : 0;
+        st->xpend[k] = -1;   // the caller flushed the pending x-update before recomputing the residual
         any |= st->active[k];
     }
     st->done = (!any || st->iter >= st->max_iter || st->breakdown) ? 1 : 0;
@@ -542,122 +584,6 @@ __global__ void __launch_bounds__(32) peer_reduce_sum_kernel(double* __restrict_
         double s = 0.0;
         for (int r = 0; r < nranks; ++r) s += d[(size_t)r * kMaxNrhs + threadIdx.x];
         dst[threadIdx.x] = s;
-    }
-}
-
-// ---- link repack: canonical Eq. (5) [mu][eo][3][3] complex of TS -> internal planes of TD ------------
-// one thread per (mu, eo); dst block (f fixed by caller, parity, mu).
-template <typename TS, typename TD>
-__global__ void __launch_bounds__(256) link_repack_kernel(const TS* __restrict__ src, TD* __restrict__ dst_field, int Vh)
-{
-    const size_t V = (size_t)2 * Vh;
-    const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
-    if (idx >= 4 * V) return;
-    const int mu = (int)(idx / V);
-    const size_t eo = idx % V;
-    const int par = eo >= (size_t)Vh ? 1 : 0;
-    const int h = (int)(eo - (size_t)par * Vh);
-    const TS* s = src + idx * 18;
-    TD* blk = dst_field + (size_t)(par * 4 + mu) * ((size_t)Vh * 18);
-    TD e[18];
-#pragma unroll
-    for (int i = 0; i < 18; ++i) e[i] = (TD)s[i];
-    if (sizeof(TD) == 8) {
-#pragma unroll
-        for (int c = 0; c < 9; ++c) {
-            blk[((size_t)c * Vh + h) * 2] = e[2 * c];
-            blk[((size_t)c * Vh + h) * 2 + 1] = e[2 * c + 1];
-        }
-    } else {
-#pragma unroll
-        for (int j = 0; j < 4; ++j)
-#pragma unroll
-            for (int i = 0; i < 4; ++i) blk[((size_t)j * Vh + h) * 4 + i] = e[4 * j + i];
-        blk[(size_t)16 * Vh + (size_t)h * 2] = e[16];
-        blk[(size_t)16 * Vh + (size_t)h * 2 + 1] = e[17];
-    }
-}
-
-// ---- Naik-link compression (row f2; the paper's `CompressionType comp`) -----------------
-// A Naik link of the HISQ action is a real multiple of a unitary matrix, W = c U: U in U(3) after the smearing's
-// projection (section 7c), in SU(3) for the BASELINE inputs (c = -eta/24).  Store rows 0 and 1 (12 reals) and the complex
-// number d = det(W) / |row0 x row1|^2 (= det(U) / c): row 2 = conj(row0 x row1) d.  14 instead of 18 reals per Naik link.
-// Layout inside the (unchanged) 18-real block: fp64: 7 planes of double2; fp32: 3 planes of float4 then 1 plane of
-// float2.  `bad` counts links whose row 2 is NOT reproduced to `tol` (relative to |row 0|): the caller then falls back
-// to the uncompressed format.
-// d = det(W) / |row0 x row1|^2 and the largest deviation of conj(row0 x row1) d from the stored row 2
-__device__ __forceinline__ double naik_row2_deviation(const double (&e)[18], double& dr, double& di)
-{
-    double cr[6], det_re = 0.0, det_im = 0.0, c2 = 0.0;   // cr = row0 x row1
-    for (int a = 0; a < 3; ++a) {
-        const int b = (a + 1) % 3, c = (a + 2) % 3;
-        cr[2 * a] = (e[2 * b] * e[6 + 2 * c] - e[2 * b + 1] * e[6 + 2 * c + 1]) - (e[2 * c] * e[6 + 2 * b] - e[2 * c + 1] * e[6 + 2 * b + 1]);
-        cr[2 * a + 1] = (e[2 * b] * e[6 + 2 * c + 1] + e[2 * b + 1] * e[6 + 2 * c]) - (e[2 * c] * e[6 + 2 * b + 1] + e[2 * c + 1] * e[6 + 2 * b]);
-        det_re += cr[2 * a] * e[12 + 2 * a] - cr[2 * a + 1] * e[12 + 2 * a + 1];
-        det_im += cr[2 * a] * e[12 + 2 * a + 1] + cr[2 * a + 1] * e[12 + 2 * a];
-        c2 += cr[2 * a] * cr[2 * a] + cr[2 * a + 1] * cr[2 * a + 1];
-    }
-    dr = c2 > 0.0 ? det_re / c2 : 0.0;
-    di = c2 > 0.0 ? det_im / c2 : 0.0;
-    double dev = 0.0;
-    for (int a = 0; a < 3; ++a) {   // (cr_re - i cr_im) (dr + i di)
-        dev = fmax(dev, fabs(cr[2 * a] * dr + cr[2 * a + 1] * di - e[12 + 2 * a]));
-        dev = fmax(dev, fabs(cr[2 * a] * di - cr[2 * a + 1] * dr - e[12 + 2 * a + 1]));
-    }
-    return dev;
-}
-// Dry run of the compression test on the caller's canonical array (writes nothing but the counter).
-template <typename TS>
-__global__ void __launch_bounds__(256) naik_check_kernel(const TS* __restrict__ src, int Vh, double tol, unsigned long long* bad)
-{
-    const size_t V = (size_t)2 * Vh;
-    const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
-    if (idx >= 4 * V) return;
-    const TS* s = src + idx * 18;
-    double e[18];
-#pragma unroll
-    for (int i = 0; i < 18; ++i) e[i] = (double)s[i];
-    double n0 = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2] + e[3] * e[3] + e[4] * e[4] + e[5] * e[5]);
-    double dr, di;
-    const double dev = naik_row2_deviation(e, dr, di);
-    if (!(dev <= tol * n0) || n0 == 0.0) atomicAdd(bad, 1ull);
-}
-
-template <typename TS, typename TD>
-__global__ void __launch_bounds__(256) naik_compress_kernel(const TS* __restrict__ src, TD* __restrict__ dst_field, int Vh,
-                                                            double tol, unsigned long long* bad)
-{
-    const size_t V = (size_t)2 * Vh;
-    const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
-    if (idx >= 4 * V) return;
-    const int mu = (int)(idx / V);
-    const size_t eo = idx % V;
-    const int par = eo >= (size_t)Vh ? 1 : 0;
-    const int h = (int)(eo - (size_t)par * Vh);
-    const TS* s = src + idx * 18;
-    TD* blk = dst_field + (size_t)(par * 4 + mu) * ((size_t)Vh * 18);
-    double e[18];
-#pragma unroll
-    for (int i = 0; i < 18; ++i) e[i] = (double)(TD)s[i];   // the values the kernel will see
-    const double n0 = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2] + e[3] * e[3] + e[4] * e[4] + e[5] * e[5]);
-    double dr, di;
-    const double dev = naik_row2_deviation(e, dr, di);
-    if (!(dev <= tol * n0) || n0 == 0.0) atomicAdd(bad, 1ull);
-    if (sizeof(TD) == 8) {
-#pragma unroll
-        for (int j = 0; j < 6; ++j) {
-            blk[((size_t)j * Vh + h) * 2] = (TD)e[2 * j];
-            blk[((size_t)j * Vh + h) * 2 + 1] = (TD)e[2 * j + 1];
-        }
-        blk[((size_t)6 * Vh + h) * 2] = (TD)dr;
-        blk[((size_t)6 * Vh + h) * 2 + 1] = (TD)di;
-    } else {
-#pragma unroll
-        for (int j = 0; j < 3; ++j)
-#pragma unroll
-            for (int i = 0; i < 4; ++i) blk[((size_t)j * Vh + h) * 4 + i] = (TD)e[4 * j + i];
-        blk[(size_t)12 * Vh + (size_t)h * 2] = (TD)dr;
-        blk[(size_t)12 * Vh + (size_t)h * 2 + 1] = (TD)di;
     }
 }
 

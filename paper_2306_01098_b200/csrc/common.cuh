@@ -9,75 +9,20 @@ constexpr int kMaxNrhs = 16;
 
 // ---- 16-byte / 8-byte vector types per precision -------------------------------------------------
 template <typename T> struct Vec;
-template <> struct Vec<double> { using c1 = double2; };             // one complex
-template <> struct Vec<float>  { using c1 = float2; using c2 = float4; };  // one / two complex
+template <> struct Vec<double> { using c1 = double2; using c16 = double2; };   // one complex; one 16-byte chunk
+template <> struct Vec<float>  { using c1 = float2; using c16 = float4; };
 
 // ---- global loads with cache hints ---------------------------------------------------------------
 // Links are read exactly once per Dslash application (every link is used forward by its
 // own site and backward by the site it points to), so they stream: no L1 allocation, evict-first.
-#ifndef HISQ_LINK_LD
-#define HISQ_LINK_LD 0   // 0: ld.global.cs (streaming); 1: ld.global.nc.L1::no_allocate; 2: plain read-only (ld.global.nc)
-#endif
-#ifndef HISQ_VEC_LD
-#define HISQ_VEC_LD 0    // 0: ld.global.nc; 1: ld.global.nc.L1::evict_last
-#endif
-__device__ __forceinline__ double2 ld_stream(const double2* p)
-{
-#if HISQ_LINK_LD == 1
-    double2 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
-    return r;
-#elif HISQ_LINK_LD == 2
-    return __ldg(p);
-#else
-    return __ldcs(p);
-#endif
-}
-__device__ __forceinline__ float4 ld_stream(const float4* p)
-{
-#if HISQ_LINK_LD == 1
-    float4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
-    return r;
-#elif HISQ_LINK_LD == 2
-    return __ldg(p);
-#else
-    return __ldcs(p);
-#endif
-}
-__device__ __forceinline__ float2 ld_stream(const float2* p)
-{
-#if HISQ_LINK_LD == 1
-    float2 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
-    return r;
-#elif HISQ_LINK_LD == 2
-    return __ldg(p);
-#else
-    return __ldcs(p);
-#endif
-}
+// (measured neutral and dropped: ld.global.nc.L1::no_allocate for the links, L1::evict_last on the gathers; a plain
+// read-only load for the links is 3-6 % slower: DESIGN.md section 6)
+__device__ __forceinline__ double2 ld_stream(const double2* p) { return __ldcs(p); }
+__device__ __forceinline__ float4 ld_stream(const float4* p) { return __ldcs(p); }
+__device__ __forceinline__ float2 ld_stream(const float2* p) { return __ldcs(p); }
 // Colour vectors are gathered by 16 different output sites: keep them in L1/L2.
-__device__ __forceinline__ double2 ld_keep(const double2* p)
-{
-#if HISQ_VEC_LD == 1
-    double2 r;
-    asm volatile("ld.global.nc.L1::evict_last.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
-    return r;
-#else
-    return __ldg(p);
-#endif
-}
-__device__ __forceinline__ float2 ld_keep(const float2* p)
-{
-#if HISQ_VEC_LD == 1
-    float2 r;
-    asm volatile("ld.global.nc.L1::evict_last.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
-    return r;
-#else
-    return __ldg(p);
-#endif
-}
+__device__ __forceinline__ double2 ld_keep(const double2* p) { return __ldg(p); }
+__device__ __forceinline__ float2 ld_keep(const float2* p) { return __ldg(p); }
 __device__ __forceinline__ float4 ld_keep(const float4* p) { return __ldg(p); }
 
 // ---- lattice geometry handed to kernels ----------------------------------------------------------
@@ -107,6 +52,8 @@ struct CgState {
     double beta[kMaxNrhs];
     double bnorm2[kMaxNrhs];   // ||b_k||^2
     double sums[kMaxNrhs];     // scratch result of stand-alone reductions
+    double alpha[kMaxNrhs];    // alpha_k of the last iteration (x += alpha p is applied by the NEXT p-update pass)
+    int xpend[kMaxNrhs];       // iteration number whose x-update of RHS k is still pending, -1: none
     double tol2;               // tol^2
     int active[kMaxNrhs];      // 1 while RHS k still iterates
     int iter;

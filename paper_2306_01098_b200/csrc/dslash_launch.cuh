@@ -5,17 +5,13 @@
 
 namespace hisq {
 
-#ifndef HISQ_DSLASH_BLOCK
-#define HISQ_DSLASH_BLOCK 128
-#endif
-constexpr int kDslashBlock = HISQ_DSLASH_BLOCK;
-
 struct LaunchStats { long long launches = 0; };
 
 // Launch D (or its fused epilogue variants) for `nrhs` right-hand sides starting at args.in/out/u/v.
-// `inner_cap`: most RHS one thread may hold (1,2,3,4,6,8).  Returns a cudaError_t as int.
+// `inner_cap`: most RHS one thread may hold (1,2,3,4,6,8); c14: the Naik links are stored compressed.
+// Returns a cudaError_t as int.
 template <typename T>
-int launch_dslash(DslashArgs<T> args, int mode, int nrhs, int inner_cap, cudaStream_t stream, LaunchStats* stats);
+int launch_dslash(DslashArgs<T> args, int mode, int nrhs, int inner_cap, bool c14, cudaStream_t stream, LaunchStats* stats);
 
 // Register count / attributes for introspection (tests, DESIGN.md tables).
 template <typename T> int dslash_regs(int nr, int mode);

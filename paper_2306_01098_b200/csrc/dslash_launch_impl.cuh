@@ -4,10 +4,9 @@
 
 namespace hisq {
 
-template <typename T, int NR, int MODE>
-static cudaError_t launch_one(const DslashArgs<T>& a, dim3 grid, cudaStream_t s)
+template <typename T, int NR, int MODE, bool NC>
+static cudaError_t launch_kernel(const DslashArgs<T>& a, dim3 grid, cudaStream_t s)
 {
-#if HISQ_PDL
     // programmatic dependent launch: the CTAs of this launch may become resident while the previous kernel of the
     // stream drains its last wave; they wait in griddepcontrol.wait (top of dslash_kernel) until it has completed
     cudaLaunchConfig_t cfg = {};
@@ -16,33 +15,39 @@ static cudaError_t launch_one(const DslashArgs<T>& a, dim3 grid, cudaStream_t s)
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    if (a.naik_c14) return cudaLaunchKernelEx(&cfg, dslash_kernel<T, NR, MODE, kDslashBlock, true>, a);
-    return cudaLaunchKernelEx(&cfg, dslash_kernel<T, NR, MODE, kDslashBlock, false>, a);
-#else
-    if (a.naik_c14) dslash_kernel<T, NR, MODE, kDslashBlock, true><<<grid, kDslashBlock, 0, s>>>(a);
-    else dslash_kernel<T, NR, MODE, kDslashBlock, false><<<grid, kDslashBlock, 0, s>>>(a);
-    return cudaGetLastError();
-#endif
+    return cudaLaunchKernelEx(&cfg, dslash_kernel<T, NR, MODE, NC>, a);
+}
+
+template <typename T, int NR, int MODE>
+static cudaError_t launch_one(const DslashArgs<T>& a, bool c14, dim3 grid, cudaStream_t s)
+{
+    return c14 ? launch_kernel<T, NR, MODE, true>(a, grid, s) : launch_kernel<T, NR, MODE, false>(a, grid, s);
 }
 
 template <typename T, int NR>
-static cudaError_t launch_mode(const DslashArgs<T>& a, int mode, dim3 grid, cudaStream_t s)
+static cudaError_t launch_mode(const DslashArgs<T>& a, int mode, bool c14, dim3 grid, cudaStream_t s)
 {
     switch (mode) {
-    case MODE_PLAIN: return launch_one<T, NR, MODE_PLAIN>(a, grid, s);
-    case MODE_APPLY_A: return launch_one<T, NR, MODE_APPLY_A>(a, grid, s);
-    default: return launch_one<T, NR, MODE_RESID>(a, grid, s);
+    case MODE_PLAIN: return launch_one<T, NR, MODE_PLAIN>(a, c14, grid, s);
+    case MODE_APPLY_A: return launch_one<T, NR, MODE_APPLY_A>(a, c14, grid, s);
+    default: return launch_one<T, NR, MODE_RESID>(a, c14, grid, s);
     }
 }
 
 static const int kInnerSizes[6] = { 8, 6, 4, 3, 2, 1 };
 
 template <typename T>
-int launch_dslash(DslashArgs<T> args, int mode, int nrhs, int inner_cap, cudaStream_t stream, LaunchStats* stats)
+int launch_dslash(DslashArgs<T> args, int mode, int nrhs, int inner_cap, bool c14, cudaStream_t stream, LaunchStats* stats)
 {
     const Geom& g = args.g;
-    const int slab = g.H * g.ty * g.tz;
-    args.slab_blocks = (slab + kDslashBlock - 1) / kDslashBlock;
+    // warp -> sites map of one (tile, t) slab: runs of consecutive half-indices (one x-y sheet of the tile, or the whole
+    // slab when the tile spans y), each covered by whole warps on aligned blocks of 32 (dslash.cuh)
+    args.merged = g.ty == g.L[1] ? 1 : 0;
+    args.nseg = args.merged ? 1 : g.tz;
+    args.seg_len = args.merged ? g.H * g.L[1] * g.tz : g.H * g.ty;
+    args.wps = args.seg_len % 32 == 0 ? args.seg_len / 32 : (args.seg_len + 31) / 32 + 1;
+    const int slab_warps = args.nseg * args.wps;
+    args.slab_blocks = (slab_warps + kDslashWarps - 1) / kDslashWarps;
     const int ntiles = g.nty * g.ntz;
     const size_t rhs_stride = (size_t)6 * g.Vh;
     // plan: greedy split of nrhs into groups of equal NR
@@ -72,12 +77,12 @@ int launch_dslash(DslashArgs<T> args, int mode, int nrhs, int inner_cap, cudaStr
         dim3 grid((unsigned)(a.slab_blocks * a.nchunks), (unsigned)a.tn, (unsigned)ntiles);
         cudaError_t e;
         switch (plan_nr[i]) {
-        case 8: e = launch_mode<T, 8>(a, mode, grid, stream); break;
-        case 6: e = launch_mode<T, 6>(a, mode, grid, stream); break;
-        case 4: e = launch_mode<T, 4>(a, mode, grid, stream); break;
-        case 3: e = launch_mode<T, 3>(a, mode, grid, stream); break;
-        case 2: e = launch_mode<T, 2>(a, mode, grid, stream); break;
-        default: e = launch_mode<T, 1>(a, mode, grid, stream); break;
+        case 8: e = launch_mode<T, 8>(a, mode, c14, grid, stream); break;
+        case 6: e = launch_mode<T, 6>(a, mode, c14, grid, stream); break;
+        case 4: e = launch_mode<T, 4>(a, mode, c14, grid, stream); break;
+        case 3: e = launch_mode<T, 3>(a, mode, c14, grid, stream); break;
+        case 2: e = launch_mode<T, 2>(a, mode, c14, grid, stream); break;
+        default: e = launch_mode<T, 1>(a, mode, c14, grid, stream); break;
         }
         if (stats) stats->launches += 1;
         if (e != cudaSuccess) return (int)e;
@@ -92,9 +97,9 @@ static int regs_mode(int mode)
     cudaFuncAttributes at;
     cudaError_t e;
     switch (mode) {
-    case MODE_PLAIN: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_PLAIN, kDslashBlock, false>); break;
-    case MODE_APPLY_A: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_APPLY_A, kDslashBlock, false>); break;
-    default: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_RESID, kDslashBlock, false>); break;
+    case MODE_PLAIN: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_PLAIN, false>); break;
+    case MODE_APPLY_A: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_APPLY_A, false>); break;
+    default: e = cudaFuncGetAttributes(&at, dslash_kernel<T, NR, MODE_RESID, false>); break;
     }
     return e == cudaSuccess ? at.numRegs : -1;
 }

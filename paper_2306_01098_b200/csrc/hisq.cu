@@ -13,6 +13,7 @@
 
 #include "blas.cuh"
 #include "dslash_launch.cuh"
+#include "links.cuh"
 #include "smear.cuh"
 
 using namespace hisq;
@@ -59,6 +60,20 @@ struct hisq_ctx {
     int info_iters, info_reliable;
     double info_relres[kMaxNrhs];
     LaunchStats stats;
+    // instantiated CUDA graphs of a batch of CG iterations, kept across solves (capture + instantiate is a visible share of
+    // a small solve: C1 is ~500 iterations of ~20 us).  A graph bakes in every kernel argument, so it is reused only if
+    // they all match; `epoch` changes whenever the workspace, the links or an option change.
+    struct GraphKey { const void* x; double m2; int nrhs, batch, keep, kind, wsize; unsigned long long epoch; };
+    struct CachedGraph {
+        cudaGraphExec_t exec; long long launches; GraphKey key;
+        bool matches(const GraphKey& k) const
+        {
+            return exec && key.x == k.x && key.m2 == k.m2 && key.nrhs == k.nrhs && key.batch == k.batch && key.keep == k.keep &&
+                   key.kind == k.kind && key.wsize == k.wsize && key.epoch == k.epoch;
+        }
+    };
+    CachedGraph cg_graph[2], ms_graph;
+    unsigned long long epoch;
     CgState* host_state;   // pinned: slot 0 (also the synchronous poll target) and slot 1, each followed by true_rr
     cudaEvent_t poll_ev[2];
     std::string last_error;
@@ -141,6 +156,8 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     h->window_mb = 20.0;   // measured on C5 and C3: 10-20 MB windows are 2-3 % faster than 40, 10 % faster than none
     h->info_iters = 0; h->info_reliable = 0;
     for (int k = 0; k < kMaxNrhs; ++k) h->info_relres[k] = 0.0;
+    h->cg_graph[0].exec = h->cg_graph[1].exec = h->ms_graph.exec = nullptr;
+    h->epoch = 1;
     h->host_state = nullptr;
     if (cudaHostAlloc((void**)&h->host_state, 2 * kPollSlot, cudaHostAllocDefault) != cudaSuccess) {
         delete h;
@@ -171,9 +188,18 @@ extern "C" int hisq_create_part(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt_g
     return HISQ_OK;
 }
 
+static void drop_graphs(hisq_ctx* h)
+{
+    hisq_ctx::CachedGraph* g[3] = { &h->cg_graph[0], &h->cg_graph[1], &h->ms_graph };
+    for (int i = 0; i < 3; ++i)
+        if (g[i]->exec) { cudaGraphExecDestroy(g[i]->exec); g[i]->exec = nullptr; }
+    h->epoch++;
+}
+
 extern "C" int hisq_destroy(hisq_ctx* h)
 {
     if (!h) return HISQ_EINVAL;
+    drop_graphs(h);
     if (h->host_state) cudaFreeHost(h->host_state);
     if (h->d_boxes) cudaFree(h->d_boxes);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
@@ -185,6 +211,7 @@ extern "C" int hisq_destroy(hisq_ctx* h)
 extern "C" int hisq_set_stream(hisq_ctx* h, void* s)
 {
     if (!h) return HISQ_EINVAL;
+    drop_graphs(h);
     h->stream = (cudaStream_t)s;
     return HISQ_OK;
 }
@@ -195,16 +222,19 @@ struct WsLayout {
 };
 
 static size_t field_bytes(const hisq_ctx* h, int nrhs, size_t w) { return align_up((size_t)nrhs * 6 * h->g.Vh * w); }
+// records per parity of the internal link layout (dslash.cuh): blocks of 32 half-indices, one spare block because a warp
+// of a run that does not start on a multiple of 32 reads (and discards) the block's other lanes
+static size_t link_blocks(const hisq_ctx* h) { return ((size_t)h->g.Vh + 31) / 32 + 1; }
+static size_t link_bytes(const hisq_ctx* h, size_t w) { return align_up(2 * link_blocks(h) * 16 * 18 * 32 * w); }
 
 static WsLayout ws_layout(const hisq_ctx* h, int nrhs)
 {
     WsLayout l;
-    const size_t V = (size_t)2 * h->g.Vh;
     size_t off = 0;
     l.links64 = off;
-    if (h->prec != HISQ_FP32) off += align_up(2 * 4 * V * 18 * 8);
+    if (h->prec != HISQ_FP32) off += link_bytes(h, 8);
     l.links32 = off;
-    if (h->prec != HISQ_FP64) off += align_up(2 * 4 * V * 18 * 4);
+    if (h->prec != HISQ_FP64) off += link_bytes(h, 4);
     l.state = off; off += align_up(sizeof(CgState));
     l.true_rr = off; off += align_up(kMaxNrhs * sizeof(double) + 64);   // + the compression check counter
     // columns: enough for the Dslash epilogue (one per CTA and chunk-slot) and the BLAS kernels
@@ -247,8 +277,19 @@ extern "C" int hisq_set_workspace(hisq_ctx* h, void* p, size_t bytes)
     h->fields = h->ws + l.fields;
     h->stage = h->ws + l.stage;
     h->have_links = false;
+    drop_graphs(h);
     CK(cudaMemsetAsync(h->state, 0, sizeof(CgState), h->stream));
     return HISQ_OK;
+}
+
+template <typename TS, typename TD>
+static void enqueue_link_records(hisq_ctx* h, const void* fat, const void* naik, TD* dst, bool c14)
+{
+    const size_t V = (size_t)2 * h->g.Vh;
+    const unsigned grid = (unsigned)((4 * V + 255) / 256);
+    if (c14) link_record_kernel<TS, TD, true><<<grid, 256, 0, h->stream>>>((const TS*)fat, (const TS*)naik, dst, h->g, link_blocks(h));
+    else link_record_kernel<TS, TD, false><<<grid, 256, 0, h->stream>>>((const TS*)fat, (const TS*)naik, dst, h->g, link_blocks(h));
+    h->stats.launches++;
 }
 
 extern "C" int hisq_set_links(hisq_ctx* h, const void* fat, const void* naik)
@@ -257,47 +298,27 @@ extern "C" int hisq_set_links(hisq_ctx* h, const void* fat, const void* naik)
     if (!h->ws) return HISQ_ENOWORKSPACE;
     const int Vh = h->g.Vh;
     const size_t V = (size_t)2 * Vh;
-    const unsigned grid = (unsigned)((4 * V + 255) / 256);
-    const size_t fstride = (size_t)8 * Vh * 18;  // reals per field (2 parities x 4 directions)
-    const void* src[2] = { fat, naik };
     h->naik_c14 = false;
-    for (int f = 0; f < 2; ++f) {
-        if (h->prec == HISQ_FP32) {
-            link_repack_kernel<float, float><<<grid, 256, 0, h->stream>>>((const float*)src[f], h->links32 + f * fstride, Vh);
-        } else {
-            link_repack_kernel<double, double><<<grid, 256, 0, h->stream>>>((const double*)src[f], h->links64 + f * fstride, Vh);
-            if (h->prec == HISQ_MIXED)
-                link_repack_kernel<double, float><<<grid, 256, 0, h->stream>>>((const double*)src[f], h->links32 + f * fstride, Vh);
-        }
-        h->stats.launches += (h->prec == HISQ_MIXED) ? 2 : 1;
-    }
+    drop_graphs(h);
     if (h->naik_compress) {
-        // row f2: try the 14-real format for the Naik links; keep it only if EVERY link is reproduced
-        // (|row2 - conj(row0 x row1) d| <= tol |row0|), otherwise the uncompressed copy written above stays
+        // row f2: the 14-real format for the Naik links is used only if EVERY link is reproduced from it
+        // (|row2 - conj(row0 x row1) d| <= tol |row0|) in every precision the context keeps; otherwise all stay uncompressed
+        const unsigned grid = (unsigned)((4 * V + 255) / 256);
         CK(cudaMemsetAsync(h->bad_count, 0, sizeof(unsigned long long), h->stream));
-        // scratch: the staging area is large enough only for small lattices, so test first, then overwrite in place
-        if (h->prec == HISQ_FP32) {
-            naik_check_kernel<float><<<grid, 256, 0, h->stream>>>((const float*)naik, Vh, 1e-5, h->bad_count);
-        } else {
-            naik_check_kernel<double><<<grid, 256, 0, h->stream>>>((const double*)naik, Vh, 1e-12, h->bad_count);
-        }
+        if (h->prec == HISQ_FP32) naik_check_kernel<float><<<grid, 256, 0, h->stream>>>((const float*)naik, Vh, 1e-5, 0.0, h->bad_count);
+        else naik_check_kernel<double><<<grid, 256, 0, h->stream>>>((const double*)naik, Vh, 1e-12, h->prec == HISQ_MIXED ? 1e-5 : 0.0, h->bad_count);
+        h->stats.launches++;
         unsigned long long bad = 1;
         CK(cudaMemcpyAsync(&bad, h->bad_count, sizeof(bad), cudaMemcpyDeviceToHost, h->stream));
         CK(cudaStreamSynchronize(h->stream));
-        h->stats.launches++;
-        if (bad == 0) {
-            if (h->prec == HISQ_FP32) {
-                naik_compress_kernel<float, float><<<grid, 256, 0, h->stream>>>((const float*)naik, h->links32 + fstride, Vh, 1e-5, h->bad_count);
-            } else {
-                naik_compress_kernel<double, double><<<grid, 256, 0, h->stream>>>((const double*)naik, h->links64 + fstride, Vh, 1e-12, h->bad_count);
-                if (h->prec == HISQ_MIXED)
-                    naik_compress_kernel<double, float><<<grid, 256, 0, h->stream>>>((const double*)naik, h->links32 + fstride, Vh, 1e-5, h->bad_count);
-            }
-            h->stats.launches += (h->prec == HISQ_MIXED) ? 2 : 1;
-            h->naik_c14 = true;
-        } else {
-            h->last_error = "naik_compress: " + std::to_string(bad) + " Naik links are not a real multiple of a U(3) matrix; stored uncompressed";
-        }
+        if (bad == 0) h->naik_c14 = true;
+        else h->last_error = "naik_compress: " + std::to_string(bad) + " Naik links are not a real multiple of a U(3) matrix; stored uncompressed";
+    }
+    if (h->prec == HISQ_FP32) {
+        enqueue_link_records<float, float>(h, fat, naik, h->links32, h->naik_c14);
+    } else {
+        enqueue_link_records<double, double>(h, fat, naik, h->links64, h->naik_c14);
+        if (h->prec == HISQ_MIXED) enqueue_link_records<double, float>(h, fat, naik, h->links32, h->naik_c14);
     }
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(h->stream));
@@ -317,6 +338,7 @@ static int run_dslash(hisq_ctx* h, const T* links, T* out, const T* in, int pari
     DslashArgs<T> a;
     a.g = h->g;
     a.links = links;
+    a.nblk = link_blocks(h);
     a.in = in; a.out = out; a.u = u; a.v = v;
     a.partial = h->partial;
     a.ticket = &h->state->ticket[ticket_slot];
@@ -325,13 +347,13 @@ static int run_dslash(hisq_ctx* h, const T* links, T* out, const T* in, int pari
     a.m2 = m2;
     a.par = parity;
     a.k0 = 0; a.nrhs_total = nrhs; a.nchunks = 1; a.slab_blocks = 0; a.total_blocks = 0;
-    a.naik_c14 = h->naik_c14 ? 1 : 0;
+    a.nseg = a.seg_len = a.wps = a.merged = 0;
     a.t0 = t_first; a.tn = t_count < 0 ? h->g.t_cnt - t_first : t_count;
     a.t_skip_at = t_skip_at; a.t_skip = t_skip;
     a.push = mode == MODE_APPLY_A ? h->fuse_push_pq : PeerPush();
     if (a.tn <= 0) return HISQ_OK;
     int cap = h->nrhs_inner > 0 ? h->nrhs_inner : default_inner_cap((int)sizeof(T));
-    int e = launch_dslash<T>(a, mode, nrhs, cap, h->stream, &h->stats);
+    int e = launch_dslash<T>(a, mode, nrhs, cap, h->naik_c14, h->stream, &h->stats);
     if (e != 0) return cuda_fail(h, (cudaError_t)e, "dslash launch");
     return HISQ_OK;
 }
@@ -425,13 +447,14 @@ static Span owned_span(const hisq_ctx* h, int vec_n)
     }
     return sp;
 }
+// x != nullptr: the pending x-update of the previous iteration rides in the same pass (blas.cuh); flush_only: only that
 template <typename T>
-static int enqueue_p_update(hisq_ctx* h, T* p, const T* r, int nrhs)
+static int enqueue_p_update(hisq_ctx* h, T* p, const T* r, int nrhs, T* x = nullptr, int flush_only = 0)
 {
     const size_t nreal = (size_t)6 * h->g.Vh;
     const Span sp = owned_span(h, V16<T>::n);
     dim3 gb((unsigned)blas_grid_x(sp.seg ? 3 * sp.seg * V16<T>::n : nreal, V16<T>::n), (unsigned)nrhs);
-    cg_update_p_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(p, r, nreal, h->state, sp);
+    cg_update_p_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(p, r, nreal, h->state, sp, x, flush_only);
     h->stats.launches++;
     CK(cudaGetLastError());
     return HISQ_OK;
@@ -483,13 +506,14 @@ static int enqueue_iteration(hisq_ctx* h, const T* links, T* x, T* r, T* p, T* q
     const size_t nreal = (size_t)6 * h->g.Vh;
     dim3 gb((unsigned)blas_grid_x(nreal, V16<T>::n), (unsigned)nrhs);
     int rc;
-    if (keep == 0 && (rc = enqueue_p_update<T>(h, p, r, nrhs)) != HISQ_OK) return rc;
+    if (keep == 0 && (rc = enqueue_p_update<T>(h, p, r, nrhs, x)) != HISQ_OK) return rc;
     rc = run_dslash<T>(h, links, t, p, HISQ_ODD, nrhs, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, &h->state->done, 2);
     if (rc) return rc;
     rc = run_dslash<T>(h, links, q, t, HISQ_EVEN, nrhs, MODE_APPLY_A, p, nullptr, m2, h->state->pq, &h->state->done, 2);
     if (rc) return rc;
     if (keep == 0) {
-        cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial);
+        // x is not touched here: its update is folded into the next iteration's p pass (or cg_solve's flush)
+        cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial, 0, PeerPush(), nullptr, Span(), 1);
         CK(cudaGetLastError());
     } else {
         cudaError_t e = keep == 1 ? launch_fused<T, 1>(h, x, r, p, q, nreal, nrhs, do_p)
@@ -576,42 +600,51 @@ static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_u
         batch = best;
     }
     const int keep = fused_keep<T>(h, nrhs);
-    cudaGraphExec_t execs[2] = { nullptr, nullptr };   // [0]: every iteration ends with its p-update; [1]: the last one does not
-    long long exec_launches[2] = { 0, 0 };
     int rc = HISQ_OK;
     int status = HISQ_OK;
     int stagnation = 0;
-    int enq_iter = 0, cur = 0;
+    // enq_iter: iterations enqueued so far; rel_base: iteration count at the last true-residual replacement.  The
+    // reliable-update schedule counts from rel_base, not from 0: when the recursion stops inside a batch (claimed
+    // convergence not confirmed by the true residual) the solve resumes from an iteration count that is no multiple of
+    // the batch, and a schedule tied to iter % R would never fire again.
+    int enq_iter = 0, rel_base = 0, cur = 0;
     bool pending = false;
     double best_true[kMaxNrhs];
     for (int k = 0; k < kMaxNrhs; ++k) best_true[k] = 1e300;
     if (keep > 0 && (rc = enqueue_p_update<T>(h, p, r, nrhs)) != HISQ_OK) return rc;
     while (true) {
         // ---- a batch of iterations; the one that ends on a reliable-update boundary leaves p alone ----
-        const int kind = (keep > 0 && R > 0 && (enq_iter + batch) % R == 0) ? 1 : 0;
+        const int kind = (keep > 0 && R > 0 && (enq_iter - rel_base + batch) % R == 0) ? 1 : 0;
         if (h->use_graph) {
-            if (!execs[kind]) {
+            hisq_ctx::CachedGraph& cg = h->cg_graph[kind];
+            const hisq_ctx::GraphKey key = { (const void*)x, m2, nrhs, batch, keep, kind, (int)sizeof(T), h->epoch };
+            if (!cg.matches(key)) {
+                if (cg.exec) { cudaGraphExecDestroy(cg.exec); cg.exec = nullptr; }
                 cudaGraph_t graph;
                 const long long l0 = h->stats.launches;
-                if (!h->cap_stream) CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+                if (!h->cap_stream && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+                    rc = cuda_fail(h, cudaGetLastError(), "cudaStreamCreateWithFlags"); break;
+                }
                 cudaStream_t user_stream = h->stream;
-                CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+                cudaError_t ce = cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal);
+                if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaStreamBeginCapture"); break; }
                 h->stream = h->cap_stream;
                 for (int i = 0; i < batch && rc == HISQ_OK; ++i)
                     rc = enqueue_iteration<T>(h, links, x, r, p, q, t, m2, nrhs, keep, (kind == 1 && i == batch - 1) ? 0 : 1);
                 h->stream = user_stream;
-                cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
+                ce = cudaStreamEndCapture(h->cap_stream, &graph);
                 if (rc != HISQ_OK) { if (ce == cudaSuccess) cudaGraphDestroy(graph); break; }
                 if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaStreamEndCapture"); break; }
-                ce = cudaGraphInstantiate(&execs[kind], graph, 0);
+                ce = cudaGraphInstantiate(&cg.exec, graph, 0);
                 cudaGraphDestroy(graph);
-                if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaGraphInstantiate"); break; }
-                exec_launches[kind] = h->stats.launches - l0;
+                if (ce != cudaSuccess) { cg.exec = nullptr; rc = cuda_fail(h, ce, "cudaGraphInstantiate"); break; }
+                cg.launches = h->stats.launches - l0;
+                cg.key = key;
                 h->stats.launches = l0;
             }
-            cudaError_t ce = cudaGraphLaunch(execs[kind], h->stream);
+            cudaError_t ce = cudaGraphLaunch(cg.exec, h->stream);
             if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaGraphLaunch"); break; }
-            h->stats.launches += exec_launches[kind];
+            h->stats.launches += cg.launches;
         } else {
             for (int i = 0; i < batch && rc == HISQ_OK; ++i)
                 rc = enqueue_iteration<T>(h, links, x, r, p, q, t, m2, nrhs, keep, (kind == 1 && i == batch - 1) ? 0 : 1);
@@ -620,7 +653,7 @@ static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_u
         // ---- look at the state, staying one batch ahead of the GPU whenever no reliable update is due ----
         enq_iter += batch;
         if ((rc = poll_async(h, cur)) != HISQ_OK) break;
-        const bool boundary = R > 0 && enq_iter % R == 0;
+        const bool boundary = R > 0 && (enq_iter - rel_base) % R == 0;
         const CgState* sp;
         if (!boundary && !pending) { pending = true; cur ^= 1; continue; }      // first batch of a run: just get ahead
         if (pending) {
@@ -634,9 +667,10 @@ static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_u
         enq_iter = s.iter;
         h->info_iters = s.iter;
         if (s.breakdown) { status = HISQ_EBREAKDOWN; }
-        const bool at_reliable = R > 0 && s.iter > 0 && s.iter % R == 0;
+        const bool at_reliable = R > 0 && s.iter > rel_base && (s.iter - rel_base) % R == 0;
         if (!s.done && !at_reliable) continue;
         // ---- reliable update / final check: true residual in the high precision ----
+        if (keep == 0 && (rc = enqueue_p_update<T>(h, p, r, nrhs, x, 1)) != HISQ_OK) break;   // the pending x += alpha p
         if (MIXED) {
             acc_xhi_kernel<<<(unsigned)((total / 4 + kBlasBlock - 1) / kBlasBlock + 1), kBlasBlock, 0, h->stream>>>(
                 (double*)x_user, (float*)x, total);
@@ -650,6 +684,7 @@ static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_u
             if (rc) break;
         }
         h->info_reliable++;
+        rel_base = s.iter;
         if ((rc = poll_state(h)) != HISQ_OK) break;
         const CgState& s2 = *h->host_state;
         const double* trr = (const double*)((const char*)h->host_state + sizeof(CgState));
@@ -673,8 +708,6 @@ static int cg_solve(hisq_ctx* h, const T* links, const double* links_hi, TB* x_u
         }
         if (keep > 0 && (rc = enqueue_p_update<T>(h, p, r, nrhs)) != HISQ_OK) break;   // p = r_true + beta p
     }
-    for (int i = 0; i < 2; ++i)
-        if (execs[i]) cudaGraphExecDestroy(execs[i]);
     if (rc != HISQ_OK) return rc;
     return status;
 }
@@ -723,33 +756,39 @@ static int ms_solve(hisq_ctx* h, const T* links, T* x, const T* b, double mass, 
     CK(cudaStreamSynchronize(h->stream));   // `delta` is a stack array
 
     const int batch = h->check_interval > 0 ? h->check_interval : 32;
-    cudaGraphExec_t exec = nullptr;
-    long long launches_per_batch = 0;
     int rc = HISQ_OK, status = HISQ_OK, cur = 0;
     bool pending = false;
     while (true) {
         if (h->use_graph) {
-            if (!exec) {
+            hisq_ctx::CachedGraph& cg = h->ms_graph;
+            // kind carries kmin, keep the number of shifts: both are baked into the captured launches
+            const hisq_ctx::GraphKey key = { (const void*)x, m2_base, nshift, batch, nshift, kmin, (int)sizeof(T), h->epoch };
+            if (!cg.matches(key)) {
+                if (cg.exec) { cudaGraphExecDestroy(cg.exec); cg.exec = nullptr; }
                 cudaGraph_t graph;
                 const long long l0 = h->stats.launches;
-                if (!h->cap_stream) CK(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+                if (!h->cap_stream && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+                    rc = cuda_fail(h, cudaGetLastError(), "cudaStreamCreateWithFlags"); break;
+                }
                 cudaStream_t user_stream = h->stream;
-                CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+                cudaError_t ce = cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal);
+                if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaStreamBeginCapture"); break; }
                 h->stream = h->cap_stream;
                 for (int i = 0; i < batch && rc == HISQ_OK; ++i) rc = ms_enqueue_iteration<T>(h, links, x, r, p, q, t, m2_base, kmin, nshift);
                 h->stream = user_stream;
-                cudaError_t ce = cudaStreamEndCapture(h->cap_stream, &graph);
+                ce = cudaStreamEndCapture(h->cap_stream, &graph);
                 if (rc != HISQ_OK) { if (ce == cudaSuccess) cudaGraphDestroy(graph); break; }
                 if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaStreamEndCapture"); break; }
-                ce = cudaGraphInstantiate(&exec, graph, 0);
+                ce = cudaGraphInstantiate(&cg.exec, graph, 0);
                 cudaGraphDestroy(graph);
-                if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaGraphInstantiate"); break; }
-                launches_per_batch = h->stats.launches - l0;
+                if (ce != cudaSuccess) { cg.exec = nullptr; rc = cuda_fail(h, ce, "cudaGraphInstantiate"); break; }
+                cg.launches = h->stats.launches - l0;
+                cg.key = key;
                 h->stats.launches = l0;
             }
-            cudaError_t ce = cudaGraphLaunch(exec, h->stream);
+            cudaError_t ce = cudaGraphLaunch(cg.exec, h->stream);
             if (ce != cudaSuccess) { rc = cuda_fail(h, ce, "cudaGraphLaunch"); break; }
-            h->stats.launches += launches_per_batch;
+            h->stats.launches += cg.launches;
         } else {
             for (int i = 0; i < batch && rc == HISQ_OK; ++i) rc = ms_enqueue_iteration<T>(h, links, x, r, p, q, t, m2_base, kmin, nshift);
             if (rc != HISQ_OK) break;
@@ -769,7 +808,6 @@ static int ms_solve(hisq_ctx* h, const T* links, T* x, const T* b, double mass, 
         }
         break;
     }
-    if (exec) cudaGraphExecDestroy(exec);
     if (rc != HISQ_OK) return rc;
     // true residuals ||b - (A + sigma_k) x_k|| / ||b|| per shift (q and t are free now)
     for (int k = 0; k < nshift; ++k) {
@@ -891,7 +929,7 @@ extern "C" int hisq_solve_M(hisq_ctx* h, void* x_even, void* x_odd, const void* 
 struct SmearCoeff { double c1, c3, c5, c7, cL; };
 
 template <typename T>
-static void launch_staple(hisq_ctx* h, unsigned grid, const T* U, const T* a_up, const T* a_dn, const T* b, T* out_up, T* out_dn, T* acc,
+static cudaError_t launch_staple(hisq_ctx* h, unsigned grid, const T* U, const T* a_up, const T* a_dn, const T* b, T* out_up, T* out_dn, T* acc,
                           int mu, int nu, T coef)
 {
     cudaLaunchConfig_t cfg = {};
@@ -900,8 +938,8 @@ static void launch_staple(hisq_ctx* h, unsigned grid, const T* U, const T* a_up,
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, staple_kernel<T>, h->g, U, a_up, a_dn, b, out_up, out_dn, acc, mu, nu, coef);
     h->stats.launches++;
+    return cudaLaunchKernelEx(&cfg, staple_kernel<T>, h->g, U, a_up, a_dn, b, out_up, out_dn, acc, mu, nu, coef);
 }
 
 // out (4V matrices) = smeared `in` (4V); A, B, C: V matrices of scratch each
@@ -919,16 +957,16 @@ static int smear_level(hisq_ctx* h, const T* in, T* out, T* A, T* B, T* C, const
         for (int nu = 0; nu < 4; ++nu) {
             if (nu == mu) continue;
             // S3_nu: up part -> A, down part -> B
-            launch_staple<T>(h, grid, in, Umu, Umu, nullptr, A, B, acc, mu, nu, (T)k.c3);
+            CK(launch_staple<T>(h, grid, in, Umu, Umu, nullptr, A, B, acc, mu, nu, (T)k.c3));
             if (k.cL != 0.0) {   // Lepage: the straight two-step staples only (up of up, down of down)
-                launch_staple<T>(h, grid, in, A, B, nullptr, nullptr, nullptr, acc, mu, nu, (T)k.cL);
+                CK(launch_staple<T>(h, grid, in, A, B, nullptr, nullptr, nullptr, acc, mu, nu, (T)k.cL));
             }
             for (int rho = 0; rho < 4; ++rho) {
                 if (rho == mu || rho == nu) continue;
                 // S5_nu,rho = G_rho[A + B] -> C
-                launch_staple<T>(h, grid, in, A, A, B, C, C, acc, mu, rho, (T)k.c5);
+                CK(launch_staple<T>(h, grid, in, A, A, B, C, C, acc, mu, rho, (T)k.c5));
                 const int sig = 6 - mu - nu - rho;
-                launch_staple<T>(h, grid, in, C, C, nullptr, nullptr, nullptr, acc, mu, sig, (T)k.c7);
+                CK(launch_staple<T>(h, grid, in, C, C, nullptr, nullptr, nullptr, acc, mu, sig, (T)k.c7));
             }
         }
     }
@@ -1006,6 +1044,7 @@ extern "C" int hisq_set_option(hisq_ctx* h, const char* key, double value)
 {
     if (!h || !key) return HISQ_EINVAL;
     const int v = (int)value;
+    drop_graphs(h);
     if (!strcmp(key, "max_iter")) { if (v < 1) return HISQ_EINVAL; h->max_iter = v; }
     else if (!strcmp(key, "reliable_interval")) { if (v < 0) return HISQ_EINVAL; h->reliable_interval = v; }
     else if (!strcmp(key, "check_interval")) { if (v < 1 || v > 1024) return HISQ_EINVAL; h->check_interval = v; }
@@ -1017,7 +1056,6 @@ extern "C" int hisq_set_option(hisq_ctx* h, const char* key, double value)
     else if (!strcmp(key, "tile_y")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[1] % v))) return HISQ_EINVAL; h->tile_y = v; }
     else if (!strcmp(key, "tile_z")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[2] % v))) return HISQ_EINVAL; h->tile_z = v; }
     else if (!strcmp(key, "window_mb")) { if (!(value > 0)) return HISQ_EINVAL; h->window_mb = value; }
-    else if (!strcmp(key, "dslash_block")) { if (v != 0 && v != kDslashBlock) return HISQ_EINVAL; }
     else return HISQ_EINVAL;
     return HISQ_OK;
 }

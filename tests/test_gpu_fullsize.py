@@ -89,9 +89,12 @@ def test_c3_64x64x64x16_fp32_nrhs8_sampled(parity):
 
 
 def test_c5_96x96x96x24_fp64_nrhs8_sampled():
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
-    if free < 120e9:
-        pytest.skip("needs ~110 GB of device memory")
+    if free < 130e9:
+        pytest.skip(f"needs ~130 GB of device memory, {free / 1e9:.0f} GB free")
     got, ref, tiles = _gpu_sampled_dslash((96, 96, 96, 24), "fp64", 8, 0, seed=0, n_random=2000, n_edge=300)
     scale = np.sqrt(np.mean(np.abs(ref) ** 2))
     for k in range(8):
@@ -142,13 +145,18 @@ def test_c4_48x48x48x12_mixed_nrhs4_cg():
     ctx64.close()
 
 
-@pytest.mark.skipif(not os.environ.get("HISQ_C5"), reason="opt-in (HISQ_C5=1): ~10 minutes, 110 GB of device and 80 GB of host memory")
-def test_c5_96x96x96x24_fp64_nrhs8_cg_opt_in():
-    """BASELINE.json configs[4]: 96^3 x 24, fp64, nRHS = 8, CG at m = 0.005 to tol 1e-10, judged by the ORACLE operator
-    on the whole field (a full CPU solve would take hours)."""
-    import time
+@pytest.fixture(scope="module")
+def c5():
+    """BASELINE.json configs[4] (96^3 x 24, fp64, nRHS = 8) set up once for the two full-size C5 tests: the context with
+    its links, and the same links on the host in the oracle's lexicographic order (24.5 GB)."""
     from paper_2306_01098_b200 import layout
-    L, m, tol, n = (96, 96, 96, 24), 0.005, 1e-10, 8
+    import gc
+    L, n = (96, 96, 96, 24), 8
+    gc.collect()
+    torch.cuda.empty_cache()                       # what earlier tests left in torch's caching allocator
+    free, _ = torch.cuda.mem_get_info()
+    if free < 140e9:
+        pytest.skip(f"needs ~140 GB of device memory, {free / 1e9:.0f} GB free")
     dev = torch.device("cuda:0")
     ctx = binding.Hisq(L, "fp64", n, dev)
     fat, naik = binding.make_links(L, 0, dev, ctx.cdtype, gen_device=dev)
@@ -159,6 +167,35 @@ def test_c5_96x96x96x24_fp64_nrhs8_cg_opt_in():
     W = naik.cpu().permute(1, 0, 2, 3)[eo].contiguous().numpy()
     del naik
     torch.cuda.empty_cache()
+    yield dict(L=L, n=n, ctx=ctx, X=X, W=W, dev=dev)
+    ctx.close()
+
+
+def test_c5_96x96x96x24_fp64_nrhs8_dslash_full_field(c5):
+    """SURVEY 8(d) C5, the final gate: the WHOLE output field of one right-hand side of the nRHS = 8 launch (the tiled
+    launch shape bench.py times) against one oracle application, both parities."""
+    L, n, ctx, dev = c5["L"], c5["n"], c5["ctx"], c5["dev"]
+    for parity in (0, 1):
+        src = binding.make_sources(L, 3 + parity, n, 1 - parity, dev, ctx.cdtype, gen_device=dev)
+        out = ctx.unpack(ctx.dslash(ctx.pack(src), parity))
+        assert ctx.tiles(n) != (96, 96)                       # the tiled sweep order really ran
+        k = 5 if parity == 0 else 2                           # one RHS per parity keeps the oracle at ~1 s per application
+        full_in = oracle.half_to_full(L, src[k:k + 1].cpu().numpy(), 1 - parity)
+        got = oracle.half_to_full(L, out[k:k + 1].cpu().numpy(), parity)
+        del src, out
+        ref = oracle.dslash_parity(L, c5["X"], c5["W"], full_in, parity)
+        assert rel_l2(got, ref) <= 1e-13                      # inputs are generated on the GPU: an ulp of libm in the sources
+        scale = np.sqrt(np.mean(np.abs(ref) ** 2)) * np.sqrt(2.0)   # RMS over the sites of the output parity (the other half is zero)
+        assert np.abs(got - ref).max() / scale <= 1e-12
+        del full_in, got, ref
+
+
+def test_c5_96x96x96x24_fp64_nrhs8_cg(c5):
+    """BASELINE.json configs[4]: 96^3 x 24, fp64, nRHS = 8, CG at m = 0.005 to tol 1e-10, judged by the ORACLE operator
+    on the whole field for every right-hand side (a full CPU solve would take hours)."""
+    import time
+    L, n, ctx, dev = c5["L"], c5["n"], c5["ctx"], c5["dev"]
+    m, tol = 0.005, 1e-10
     b_can = binding.make_sources(L, 1, n, 0, dev, ctx.cdtype, gen_device=dev)
     b = ctx.pack(b_can)
     torch.cuda.synchronize()
@@ -166,13 +203,15 @@ def test_c5_96x96x96x24_fp64_nrhs8_cg_opt_in():
     x, info = ctx.cg(b, m, tol)
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
-    print(f"\\nC5 CG: {info['iterations']} iterations, {dt:.1f} s, {1e3 * dt / info['iterations']:.2f} ms/iteration, "
+    print(f"\nC5 CG: {info['iterations']} iterations, {dt:.1f} s, {1e3 * dt / info['iterations']:.2f} ms/iteration, "
           f"true residuals {info['true_rel_resid']}")
-    x_full = oracle.half_to_full(L, ctx.unpack(x).cpu().numpy(), 0)
-    b_full = oracle.half_to_full(L, b_can.cpu().numpy(), 0)
-    ctx.close()
-    r = b_full - oracle.apply_A(L, X, W, m, x_full)
-    for k in range(n):
-        rel = np.linalg.norm(r[k]) / np.linalg.norm(b_full[k])
+    assert 8000 < info["iterations"] < 13000              # ~49/m for these link distributions
+    x_can = ctx.unpack(x).cpu().numpy()
+    del x, b
+    for k in range(n):                                    # one RHS at a time bounds the host memory
+        x_full = oracle.half_to_full(L, x_can[k:k + 1], 0)
+        b_full = oracle.half_to_full(L, b_can[k:k + 1].cpu().numpy(), 0)
+        r = b_full - oracle.apply_A(L, c5["X"], c5["W"], m, x_full)
+        rel = np.linalg.norm(r) / np.linalg.norm(b_full)
         print(f"RHS {k}: oracle-evaluated ||b - A x|| / ||b|| = {rel:.3e}")
         assert rel <= tol
