@@ -151,7 +151,7 @@ int hisq_smear(hisq_ctx *h, const void *thin, void *fat, void *naik, void *scrat
                int fold_phases);
 
 /* Gauge configurations in the NERSC archive format (PAPER.md:540 lists the formats the paper's code
- * reads: ILDG, MILC, NERSC, openQCD -- only NERSC is built here).  HOST functions, no context, no CUDA: text header
+ * reads: ILDG, MILC, NERSC, openQCD; the other three: hisq_cfg_* below).  HOST functions, no context, no CUDA: text header
  * (DATATYPE = 4D_SU3_GAUGE_3x3 | 4D_SU3_GAUGE, DIMENSION_1..4, FLOATING_POINT = IEEE64BIG | IEEE32BIG | IEEE64LITTLE |
  * IEEE32LITTLE, CHECKSUM, LINK_TRACE, PLAQUETTE) followed by the links in lexicographic site order (x fastest), mu = 0..3
  * per site, row-major matrices; the two-row type is completed with row 2 = conj(row0 x row1).
@@ -164,6 +164,21 @@ int hisq_smear(hisq_ctx *h, const void *thin, void *fat, void *naik, void *scrat
 int hisq_nersc_info(const char *path, int *L, int *rows, int *real_bytes, double *link_trace, double *plaquette);
 int hisq_nersc_read(const char *path, void *links_host, size_t bytes);
 int hisq_nersc_write(const char *path, const void *links_host, const int *L, int rows, double plaquette);
+
+/* The other three formats of PAPER.md:540 -- ILDG (LIME container), MILC (version 5 binary) and openQCD (export_cnfg) --
+ * behind one trio of HOST functions (csrc/cfg_io.cpp states each format as it is read).  All deliver / take the CANONICAL
+ * link array (Eq. (5)) as complex double on the host.
+ * hisq_cfg_info : extents L[4] = (Lx, Ly, Lz, Lt) and the width in bytes of the reals in the file (ILDG 4 | 8, MILC 4,
+ *                 openQCD 8); either output pointer may be NULL.
+ * hisq_cfg_read : `bytes` >= 4*V*9 complex double.  Integrity: ILDG verifies the SciDAC checksum record when the file has
+ *                 one; MILC its two rotating-XOR checksums; openQCD recomputes the average plaquette (its only check).
+ *                 HISQ_EIO on a failed check, a short or unreadable file; HISQ_EINVAL for a malformed header, a MILC file
+ *                 with a site list (order != 0), or extents the library does not take (odd or < 4).
+ * hisq_cfg_write: the inverse; real_bytes selects the file precision (ILDG 4 | 8, MILC 4, openQCD 8, else HISQ_EINVAL). */
+enum { HISQ_FMT_ILDG = 1, HISQ_FMT_MILC = 2, HISQ_FMT_OPENQCD = 3 };
+int hisq_cfg_info(const char *path, int format, int *L, int *real_bytes);
+int hisq_cfg_read(const char *path, int format, void *links_host, size_t bytes);
+int hisq_cfg_write(const char *path, int format, const void *links_host, const int *L, int real_bytes);
 
 /* Options: "max_iter" (default 100000), "reliable_interval" (default 100 for HISQ_MIXED, 0 = off for
  * the others), "check_interval" (iterations enqueued between host polls of the convergence flag,

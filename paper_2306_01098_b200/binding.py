@@ -29,6 +29,7 @@ EXPORTS = [
     "hisq_create_part", "hisq_peer_bytes", "hisq_peer_attach", "hisq_halo_send", "hisq_halo_recv", "hisq_peer_reduce_send", "hisq_peer_reduce_recv", "hisq_dslash_slices", "hisq_dslash_edges", "hisq_halo_bytes", "hisq_halo_pack", "hisq_halo_unpack",
     "hisq_cgp_begin", "hisq_cgp_phase", "hisq_cgp_ptr", "hisq_cgp_status", "hisq_strerror",
     "hisq_last_error", "hisq_debug_dslash_regs", "hisq_debug_tiles",
+    "hisq_cfg_info", "hisq_cfg_read", "hisq_cfg_write",
 ]
 
 _lib = None
@@ -66,6 +67,9 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_nersc_info.argtypes = [ctypes.c_char_p, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(d), ctypes.POINTER(d)]
     lib.hisq_nersc_read.argtypes = [ctypes.c_char_p, vp, sz]
     lib.hisq_nersc_write.argtypes = [ctypes.c_char_p, vp, ctypes.POINTER(i), i, d]
+    lib.hisq_cfg_info.argtypes = [ctypes.c_char_p, i, ctypes.POINTER(i), ctypes.POINTER(i)]
+    lib.hisq_cfg_read.argtypes = [ctypes.c_char_p, i, vp, sz]
+    lib.hisq_cfg_write.argtypes = [ctypes.c_char_p, i, vp, ctypes.POINTER(i), i]
     lib.hisq_smear_bytes.argtypes = [vp]
     lib.hisq_smear_bytes.restype = sz
     lib.hisq_smear.argtypes = [vp, vp, vp, vp, vp, d, d, i]
@@ -441,6 +445,43 @@ def nersc_write(path: str, links: torch.Tensor, L, rows: int = 3, plaquette: flo
     links = links.to(torch.complex128).cpu().contiguous()
     code = lib.hisq_nersc_write(path.encode(), ctypes.c_void_p(links.data_ptr()), (ctypes.c_int * 4)(*[int(v) for v in L]), int(rows),
                                 float(plaquette))
+    if code:
+        raise HisqError(code, lib.hisq_strerror(code).decode())
+
+
+CFG_FORMATS = {"ildg": 1, "milc": 2, "openqcd": 3}
+
+
+def cfg_info(path: str, fmt: str) -> dict:
+    """Header of an ILDG / MILC v5 / openQCD configuration: L = (Lx, Ly, Lz, Lt), real_bytes."""
+    lib = load_library()
+    L = (ctypes.c_int * 4)()
+    rb = ctypes.c_int(0)
+    code = lib.hisq_cfg_info(path.encode(), CFG_FORMATS[fmt], L, ctypes.byref(rb))
+    if code:
+        raise HisqError(code, lib.hisq_strerror(code).decode())
+    return {"L": tuple(L), "real_bytes": rb.value}
+
+
+def cfg_read(path: str, fmt: str) -> torch.Tensor:
+    """An ILDG / MILC v5 / openQCD configuration as canonical thin links [4, V, 3, 3] complex128 on the HOST (the
+    format's integrity check is verified by the library)."""
+    lib = load_library()
+    L = cfg_info(path, fmt)["L"]
+    V = L[0] * L[1] * L[2] * L[3]
+    out = torch.empty((4, V, 3, 3), dtype=torch.complex128)
+    code = lib.hisq_cfg_read(path.encode(), CFG_FORMATS[fmt], ctypes.c_void_p(out.data_ptr()), out.numel() * 16)
+    if code:
+        raise HisqError(code, lib.hisq_strerror(code).decode())
+    return out
+
+
+def cfg_write(path: str, fmt: str, links: torch.Tensor, L, real_bytes: int = 8) -> None:
+    """Canonical links [4, V, 3, 3] (host) -> file in the given format."""
+    lib = load_library()
+    links = links.to(torch.complex128).cpu().contiguous()
+    code = lib.hisq_cfg_write(path.encode(), CFG_FORMATS[fmt], ctypes.c_void_p(links.data_ptr()),
+                              (ctypes.c_int * 4)(*[int(v) for v in L]), int(real_bytes))
     if code:
         raise HisqError(code, lib.hisq_strerror(code).decode())
 

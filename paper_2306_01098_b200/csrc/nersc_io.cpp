@@ -6,7 +6,7 @@
 //   DATATYPE = 4D_SU3_GAUGE_3x3 (all three rows stored) | 4D_SU3_GAUGE (rows 0, 1; row 2 = conj(row0 x row1))
 //   DIMENSION_1..4 = Lx, Ly, Lz, Lt        FLOATING_POINT = IEEE64BIG | IEEE32BIG | IEEE64LITTLE | IEEE32LITTLE
 //   CHECKSUM = hex: sum modulo 2^32 of all 32-bit words of the data (in the file's declared byte order)
-//   LINK_TRACE = mean of Re tr U / 3       PLAQUETTE = mean of Re tr U_plaq / 3 (not checked here: it needs products)
+//   LINK_TRACE = mean of Re tr U / 3       PLAQUETTE = mean of Re tr U_plaq / 3 (verified when the header gives a non-zero value)
 // followed by the links, site by site with x fastest (the lexicographic order of PAPER.md:433), and for each site
 // mu = 0..3, each matrix row-major (re, im).  The result goes to the CANONICAL layout of include/hisq.h (Eq. (5):
 // slot mu*V + eo(x)) as complex double.
@@ -20,6 +20,8 @@
 #include <string>
 #include <vector>
 
+double hisq_host_plaquette(const int* L, const double* links);   // cfg_io.cpp
+
 namespace {
 
 struct Header {
@@ -27,7 +29,7 @@ struct Header {
     bool rows3 = true, f64 = true, big = true;
     uint32_t checksum = 0;
     double link_trace = 0.0, plaquette = 0.0;
-    bool have_checksum = false, have_type = false, have_fp = false;
+    bool have_checksum = false, have_type = false, have_fp = false, have_link_trace = false, have_plaquette = false;
     long data_offset = 0;
 };
 
@@ -59,8 +61,11 @@ int read_header(FILE* f, Header& h)
         } else if (key == "CHECKSUM") {
             h.checksum = (uint32_t)strtoul(val.c_str(), nullptr, 16);
             h.have_checksum = true;
-        } else if (key == "LINK_TRACE") h.link_trace = atof(val.c_str());
-        else if (key == "PLAQUETTE") h.plaquette = atof(val.c_str());
+        } else if (key == "LINK_TRACE") { h.link_trace = atof(val.c_str()); h.have_link_trace = true; }
+        else if (key == "PLAQUETTE") { h.plaquette = atof(val.c_str()); h.have_plaquette = true; }
+        else if (key.rfind("BOUNDARY_", 0) == 0) {
+            if (val != "PERIODIC") return HISQ_EINVAL;   // the library's gauge field is periodic
+        }
         else if (key == "FLOATING_POINT") {
             if (val == "IEEE64BIG") { h.f64 = true; h.big = true; }
             else if (val == "IEEE32BIG" || val == "IEEE32") { h.f64 = false; h.big = true; }
@@ -72,7 +77,7 @@ int read_header(FILE* f, Header& h)
     }
     if (!ended || !h.have_type || !h.have_fp) return HISQ_EINVAL;
     for (int d = 0; d < 4; ++d)
-        if (h.L[d] < 1) return HISQ_EINVAL;
+        if (h.L[d] < 1 || h.L[d] > 4096) return HISQ_EINVAL;
     h.data_offset = ftell(f);
     return HISQ_OK;
 }
@@ -164,9 +169,14 @@ extern "C" int hisq_nersc_read(const char* path, void* links_host, size_t bytes)
         }
     }
     fclose(f);
-    if (h.have_checksum && sum != h.checksum) return HISQ_EIO;
+    if (!h.have_checksum) return HISQ_EINVAL;               // a file without its checksum cannot be trusted
+    if (sum != h.checksum) return HISQ_EIO;
     const double lt = trace / (3.0 * 4.0 * (double)V);
-    if (h.link_trace != 0.0 && std::fabs(lt - h.link_trace) > 1e-5 * (1.0 + std::fabs(h.link_trace))) return HISQ_EIO;
+    if (h.have_link_trace && std::fabs(lt - h.link_trace) > 1e-5 * (1.0 + std::fabs(h.link_trace))) return HISQ_EIO;
+    // the header's plaquette (mean Re tr / 3 over the 6 planes); writers that do not know it put 0: not checked then
+    if (h.have_plaquette && h.plaquette != 0.0 &&
+        std::fabs(hisq_host_plaquette(h.L, out) / 3.0 - h.plaquette) > 1e-5 * (1.0 + std::fabs(h.plaquette)))
+        return HISQ_EIO;
     return HISQ_OK;
 }
 

@@ -76,9 +76,16 @@ def test_library_writer_roundtrip_and_independent_parse(tmp_path):
     L = (4, 4, 6, 8)
     U = _thin_lex(L, 32)
     can = torch.from_numpy(_canonical(L, U))
+    plaq = _plaquette(L, U)
     for rows in (3, 2):
         path = str(tmp_path / f"w{rows}.nersc")
+        # a header PLAQUETTE that is not the links' own is refused on reading (the value used to be parsed and
+        # ignored); 0 means "not known" and is not checked
         binding.nersc_write(path, can, L, rows=rows, plaquette=0.5)
+        with pytest.raises(binding.HisqError) as e:
+            binding.nersc_read(path)
+        assert e.value.code == binding.HISQ_EIO
+        binding.nersc_write(path, can, L, rows=rows, plaquette=plaq)
         back = binding.nersc_read(path).numpy()
         assert np.array_equal(back[:, :, :2], can.numpy()[:, :, :2])
         assert np.abs(back - can.numpy()).max() < 1e-15
@@ -125,3 +132,11 @@ def test_error_paths(tmp_path):
     assert binding.nersc_info(str(odd))["L"] == Lo and read(odd) == binding.HISQ_EINVAL
     with pytest.raises(binding.HisqError):
         binding.nersc_read(str(tmp_path / "missing.nersc"))
+    # a file without CHECKSUM, or one that declares non-periodic links, is refused rather than accepted
+    nosum = tmp_path / "nosum.nersc"
+    head, raw = blob.split(b"END_HEADER\n", 1)
+    nosum.write_bytes(b"\n".join(l for l in head.split(b"\n") if not l.startswith(b"CHECKSUM")) + b"END_HEADER\n" + raw)
+    assert read(nosum) == binding.HISQ_EINVAL
+    anti = tmp_path / "anti.nersc"
+    anti.write_bytes(head + b"BOUNDARY_4 = ANTIPERIODIC\nEND_HEADER\n" + raw)
+    assert read(anti) == binding.HISQ_EINVAL
