@@ -56,7 +56,9 @@ enum {
     HISQ_ECUDA = -4,        /* a CUDA call failed; text via hisq_last_error                                */
     HISQ_ENOCONV = -5,      /* max_iter reached; x holds the last iterate, hisq_get_info the residuals     */
     HISQ_EBREAKDOWN = -6,   /* <p, A p> <= 0 or a non-finite scalar appeared in CG; hisq_smear: singular link */
-    HISQ_EIO = -7           /* file cannot be opened / is truncated / fails its checksum or link trace     */
+    HISQ_EIO = -7,          /* file cannot be opened / is truncated / fails its checksum or link trace     */
+    HISQ_EPEER = -8         /* multi-rank solve: another rank aborted (its error, or options that differ
+                               between the ranks); the mailboxes must be zeroed and re-attached             */
 };
 
 /* Create a context for an Lx x Ly x Lz x Lt lattice on the current CUDA device.
@@ -187,7 +189,10 @@ int hisq_cfg_write(const char *path, int format, const void *links_host, const i
  * "tile_y", "tile_z" (CTA sweep order blocking in y,z; 0 = auto),
  * "naik_compress" (see hisq_naik_compressed; default 0), "fused_blas" (1: cooperative fused x/r/p update kernel when the
  * fields are small enough to stay in registers across a grid barrier, default 1), "window_mb" (L2 budget of the CTA sweep
- * order, default 20), "overlap" (hisq_cg on a partitioned context: compute the slices that read no halo while the halo is
+ * order, default 20), "dot_fp64" (fp32 operator only: how the scalar products fused into the Dslash epilogue, <p,Ap> and
+ * ||b - A x||^2, are accumulated: 1 = every product in fp64, 0 = the 6 products of one site summed in fp32 and widened once,
+ * -1 = fp64 for the 1- and 2-RHS kernels (HBM-bound, free) and the per-site fp32 sum for the wider ones; default -1; sums
+ * across sites are fp64 in every case), "overlap" (hisq_cg on a partitioned context: compute the slices that read no halo while the halo is
  * in flight; -1 = when at least half of the owned slices qualify (Lt_loc >= 12), 0 never, 1 always; default -1). */
 int hisq_set_option(hisq_ctx *h, const char *key, double value);
 

@@ -17,7 +17,7 @@ HISQ_FP32, HISQ_FP64, HISQ_MIXED = 4, 8, 12
 HISQ_EVEN, HISQ_ODD = 0, 1
 HISQ_MAX_NRHS = 16
 HISQ_EINVAL, HISQ_ENOLINKS, HISQ_ENOWORKSPACE, HISQ_ECUDA = -1, -2, -3, -4
-HISQ_ENOCONV, HISQ_EBREAKDOWN, HISQ_EIO = -5, -6, -7
+HISQ_ENOCONV, HISQ_EBREAKDOWN, HISQ_EIO, HISQ_EPEER = -5, -6, -7, -8
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("HISQ_LIB", os.path.join(_HERE, "libhisq.so"))

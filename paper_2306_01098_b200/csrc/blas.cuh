@@ -149,8 +149,11 @@ template <typename T>
 __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict__ x, T* __restrict__ r, const T* __restrict__ p,
                                                                   const T* __restrict__ q, size_t nreal, CgState* st,
                                                                   double* partial, int defer = 0, PeerPush push = PeerPush(),
-                                                                  const double* red_pq = nullptr, Span sp = Span(), int fold_x = 0)
+                                                                  const double* red_pq = nullptr, Span sp = Span(), int fold_x = 0,
+                                                                  int trips = 1)
 {
+    // trips: consecutive 4 KB-per-array chunks one CTA works through (large fields: the reduction tail and the dependent
+    // loads of the scalars at the head of a CTA cost as much as streaming one chunk; measured 4.7 -> see DESIGN.md 7)
     // fold_x = 1: x is left alone here; alpha_k is handed to the next cg_update_p_kernel pass (st->alpha, st->xpend)
     // defer = 1 (partitioned lattice).  red_pq: <p,q> is not in st->pq yet but, rank by rank, in this slot of the
     // mailbox (every block adds them up itself); push: the last block hands the local ||r||^2 to all ranks.
@@ -174,37 +177,40 @@ __global__ void __launch_bounds__(kBlasBlock) cg_update_xr_kernel(T* __restrict_
     const V* pv = reinterpret_cast<const V*>(p + base);
     const V* qv = reinterpret_cast<const V*>(q + base);
     const bool live = st->active[k] != 0;  // frozen RHS: no traffic, but the block still joins the reduction
-    V xx[kBlasItems], rr[kBlasItems], pp[kBlasItems], qq[kBlasItems];
-#pragma unroll
-    for (int it = 0; it < kBlasItems; ++it) {
-        size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
-        if (live && i < nvec) {
-            const size_t j = span_map(sp, i);
-            rr[it] = rv[j]; qq[it] = qv[j];
-            if (!fold_x) { xx[it] = xv[j]; pp[it] = pv[j]; }
-        }
-    }
     double sum[1] = { 0.0 };
+    for (int tr = 0; tr < trips; ++tr) {
+        const size_t bx = (size_t)blockIdx.x * trips + tr;
+        V xx[kBlasItems], rr[kBlasItems], pp[kBlasItems], qq[kBlasItems];
 #pragma unroll
-    for (int it = 0; it < kBlasItems; ++it) {
-        size_t i = ((size_t)blockIdx.x * kBlasItems + it) * kBlasBlock + threadIdx.x;
-        if (live && i < nvec) {
-            T b[N], d[N];
-            unpack16<T>(rr[it], b); unpack16<T>(qq[it], d);
-#pragma unroll
-            for (int e = 0; e < N; ++e) {
-                b[e] = fma(-alpha, d[e], b[e]);
-                sum[0] += (double)b[e] * (double)b[e];
+        for (int it = 0; it < kBlasItems; ++it) {
+            size_t i = (bx * kBlasItems + it) * kBlasBlock + threadIdx.x;
+            if (live && i < nvec) {
+                const size_t j = span_map(sp, i);
+                rr[it] = rv[j]; qq[it] = qv[j];
+                if (!fold_x) { xx[it] = xv[j]; pp[it] = pv[j]; }
             }
-            const size_t j = span_map(sp, i);
-            if (!fold_x) {
-                T a[N], c[N];
-                unpack16<T>(xx[it], a); unpack16<T>(pp[it], c);
+        }
 #pragma unroll
-                for (int e = 0; e < N; ++e) a[e] = fma(alpha, c[e], a[e]);
-                xv[j] = pack16<T>(a);
+        for (int it = 0; it < kBlasItems; ++it) {
+            size_t i = (bx * kBlasItems + it) * kBlasBlock + threadIdx.x;
+            if (live && i < nvec) {
+                T b[N], d[N];
+                unpack16<T>(rr[it], b); unpack16<T>(qq[it], d);
+#pragma unroll
+                for (int e = 0; e < N; ++e) {
+                    b[e] = fma(-alpha, d[e], b[e]);
+                    sum[0] += (double)b[e] * (double)b[e];
+                }
+                const size_t j = span_map(sp, i);
+                if (!fold_x) {
+                    T a[N], c[N];
+                    unpack16<T>(xx[it], a); unpack16<T>(pp[it], c);
+#pragma unroll
+                    for (int e = 0; e < N; ++e) a[e] = fma(alpha, c[e], a[e]);
+                    xv[j] = pack16<T>(a);
+                }
+                rv[j] = pack16<T>(b);
             }
-            rv[j] = pack16<T>(b);
         }
     }
     __shared__ double totals[kMaxNrhs];
@@ -574,6 +580,23 @@ __global__ void __launch_bounds__(32) peer_reduce_send_kernel(const double* __re
     }
     __syncwarp();
     if (threadIdx.x == 0) atomicAdd_system(reinterpret_cast<unsigned*>(box + counter_off) + slot, 1u);
+}
+
+// Abort path of the mailbox protocol: a rank that leaves a multi-rank solve with an error raises every rank's abort word and
+// adds a poison value to all four arrival counters of every mailbox, so that every stream wait (">= expected") anywhere
+// passes at once and no peer's stream stays parked on a counter that will never arrive; the peers see the abort word at
+// their next status poll.  One thread per (mailbox, counter).
+constexpr unsigned kMboxPoison = 0x40000000u;
+constexpr int kMboxAbortWord = 15;
+__global__ void __launch_bounds__(64) peer_abort_kernel(PeerBoxes pb, int nranks)
+{
+    const int r = threadIdx.x / 4, c = threadIdx.x % 4;
+    if (r >= nranks || pb.box[r] == nullptr) return;
+    unsigned* counters = reinterpret_cast<unsigned*>(pb.box[r]);
+    const int idx[4] = { 0, 1, 8, 9 };   // halo slots 0, 1; reduce slots 0, 1
+    if (c == 0) atomicExch_system(counters + kMboxAbortWord, 1u);
+    __threadfence_system();
+    atomicAdd_system(counters + idx[c], kMboxPoison);
 }
 
 __global__ void __launch_bounds__(32) peer_reduce_sum_kernel(double* __restrict__ dst, const char* __restrict__ mybox, int nranks, int slot,

@@ -58,6 +58,8 @@ template <typename T> struct DslashArgs {
     // warp -> sites map of one (tile, t) slab: nseg runs of seg_len consecutive half-indices, wps warps each; a warp
     // covers one ALIGNED block of 32 half-indices (lanes outside the run idle: only when seg_len % 32 != 0)
     int nseg, seg_len, wps, merged;
+    int wide_dot;        // epilogue scalar products: 1 = every product widened to fp64, 0 = the 6 products of one site summed
+                         // in T and widened once (fp32 only matters: fp64 is the same either way)
     int t0, tn;          // this launch covers tn owned slices: blockIdx.y = j is slice g.t_lo + t0 + j, plus t_skip for
     PeerPush push;       // MODE_APPLY_A on a partitioned lattice: the last CTA also hands the sums to every rank's mailbox
     int t_skip_at, t_skip;  // j >= t_skip_at (two ranges in one launch: the first and last slices around an interior).
@@ -387,15 +389,18 @@ __global__ void __launch_bounds__(kDslashBlock, KernelShape<T, NR, MODE>::minb) 
                 }
                 const T m2 = (T)a.m2;
                 if (MODE == MODE_APPLY_A) {
-                    // the 6 products of one site are summed in T and widened once: fp32 -> fp64 conversions run at a
-                    // fraction of the FMA rate (12 per RHS and site cost ~25 % of the fp32 n = 4 kernel); sites add in fp64
+                    // a.wide_dot == 0: the 6 products of one site are summed in T and widened once: fp32 -> fp64 conversions
+                    // run at a fraction of the FMA rate (12 per RHS and site cost ~25 % of the fp32 n = 4 kernel); sites add
+                    // in fp64 either way.  The launcher widens every product where the kernel is DRAM-bound anyway (NR <= 2).
                     T part = T(0);
+                    double wide = 0.0;
 #pragma unroll
                     for (int i = 0; i < 6; ++i) {
                         o[i] = fma(m2, uu[i], -acc[k][i]);
-                        part = fma(uu[i], o[i], part);
+                        if (sizeof(T) == 4 && a.wide_dot) wide = fma((double)uu[i], (double)o[i], wide);
+                        else part = fma(uu[i], o[i], part);
                     }
-                    red[k] += (double)part;
+                    red[k] += (sizeof(T) == 4 && a.wide_dot) ? wide : (double)part;
                 } else {
                     T vv[6];
                     if (EARLY) {
@@ -405,12 +410,14 @@ __global__ void __launch_bounds__(kDslashBlock, KernelShape<T, NR, MODE>::minb) 
                         load_vec(a.v + (size_t)(chunk * NR + k) * rhs_stride, Vh, h, vv);
                     }
                     T part = T(0);
+                    double wide = 0.0;
 #pragma unroll
                     for (int i = 0; i < 6; ++i) {
                         o[i] = vv[i] - fma(m2, uu[i], -acc[k][i]);
-                        part = fma(o[i], o[i], part);
+                        if (sizeof(T) == 4 && a.wide_dot) wide = fma((double)o[i], (double)o[i], wide);
+                        else part = fma(o[i], o[i], part);
                     }
-                    red[k] += (double)part;
+                    red[k] += (sizeof(T) == 4 && a.wide_dot) ? wide : (double)part;
                 }
             }
 #pragma unroll

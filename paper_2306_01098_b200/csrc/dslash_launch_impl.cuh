@@ -74,6 +74,7 @@ int launch_dslash(DslashArgs<T> args, int mode, int nrhs, int inner_cap, bool c1
         if (args.v) a.v = args.v + (size_t)k * rhs_stride;
         a.k0 = k;
         a.nchunks = plan_cnt[i];
+        a.wide_dot = args.wide_dot < 0 ? (plan_nr[i] <= 2 ? 1 : 0) : args.wide_dot;   // -1: widen where it is free
         dim3 grid((unsigned)(a.slab_blocks * a.nchunks), (unsigned)a.tn, (unsigned)ntiles);
         cudaError_t e;
         switch (plan_nr[i]) {

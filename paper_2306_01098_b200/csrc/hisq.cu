@@ -40,6 +40,8 @@ struct hisq_ctx {
     int naik_compress;     // option: try to compress at the next hisq_set_links
     int fused_blas;        // option: cooperative fused x/r/p update for small fields
     void* cgp_x; int cgp_nrhs; double cgp_tol;   // phase-wise CG on partitioned lattices
+    int work_prec;         // precision the phase-wise / halo calls operate in: prec, except inside a HISQ_MIXED multi-rank
+                           // solve, which switches between the fp32 iteration and the fp64 reliable update
     // peer-memory halo transport (hisq_peer_attach): mailboxes of this rank and of its t-neighbours, exchange counters
     int part_rank, part_nranks;
     char *mbox, *mbox_up, *mbox_down;
@@ -51,10 +53,11 @@ struct hisq_ctx {
     size_t mbox_buf;       // bytes of one halo buffer inside a mailbox
     int mbox_nrhs;
     unsigned seq_send, seq_recv, red_send, red_recv;
+    cudaStream_t abort_stream;   // the abort kernel must not queue behind a stream that is itself waiting for a peer
     int num_sms;
     unsigned long long* bad_count;  // device counter used by the compression check
     // options
-    int max_iter, reliable_interval, check_interval, use_graph, nrhs_inner, tile_y, tile_z, overlap_opt;
+    int max_iter, reliable_interval, check_interval, use_graph, nrhs_inner, tile_y, tile_z, overlap_opt, dot_fp64;
     double window_mb;
     // info of the last solve
     int info_iters, info_reliable;
@@ -149,8 +152,10 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     h->use_graph = 1;
     h->nrhs_inner = 0;
     h->naik_c14 = false; h->naik_compress = 0; h->bad_count = nullptr;
-    h->fused_blas = 1; h->num_sms = 0; h->overlap_opt = -1;
+    h->fused_blas = 1; h->num_sms = 0; h->overlap_opt = -1; h->dot_fp64 = -1;
     h->cgp_x = nullptr; h->cgp_nrhs = 0; h->cgp_tol = 0.0;
+    h->work_prec = prec == HISQ_MIXED ? HISQ_FP64 : prec;
+    h->abort_stream = nullptr;
     { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev); }
     h->tile_y = 0; h->tile_z = 0;
     h->window_mb = 20.0;   // measured on C5 and C3: 10-20 MB windows are 2-3 % faster than 40, 10 % faster than none
@@ -203,6 +208,7 @@ extern "C" int hisq_destroy(hisq_ctx* h)
     if (h->host_state) cudaFreeHost(h->host_state);
     if (h->d_boxes) cudaFree(h->d_boxes);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    if (h->abort_stream) cudaStreamDestroy(h->abort_stream);
     for (int i = 0; i < 2; ++i) if (h->poll_ev[i]) cudaEventDestroy(h->poll_ev[i]);
     delete h;
     return HISQ_OK;
@@ -348,6 +354,7 @@ static int run_dslash(hisq_ctx* h, const T* links, T* out, const T* in, int pari
     a.par = parity;
     a.k0 = 0; a.nrhs_total = nrhs; a.nchunks = 1; a.slab_blocks = 0; a.total_blocks = 0;
     a.nseg = a.seg_len = a.wps = a.merged = 0;
+    a.wide_dot = h->dot_fp64;
     a.t0 = t_first; a.tn = t_count < 0 ? h->g.t_cnt - t_first : t_count;
     a.t_skip_at = t_skip_at; a.t_skip = t_skip;
     a.push = mode == MODE_APPLY_A ? h->fuse_push_pq : PeerPush();
@@ -513,7 +520,11 @@ static int enqueue_iteration(hisq_ctx* h, const T* links, T* x, T* r, T* p, T* q
     if (rc) return rc;
     if (keep == 0) {
         // x is not touched here: its update is folded into the next iteration's p pass (or cg_solve's flush)
-        cg_update_xr_kernel<T><<<gb, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial, 0, PeerPush(), nullptr, Span(), 1);
+        // large fields: several chunks per CTA (blas.cuh), as long as >= 16 CTAs per SM remain
+        int trips = (int)((size_t)gb.x * nrhs / ((size_t)h->num_sms * 16));
+        trips = trips < 1 ? 1 : (trips > 8 ? 8 : trips);
+        dim3 gt((gb.x + trips - 1) / trips, (unsigned)nrhs);
+        cg_update_xr_kernel<T><<<gt, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial, 0, PeerPush(), nullptr, Span(), 1, trips);
         CK(cudaGetLastError());
     } else {
         cudaError_t e = keep == 1 ? launch_fused<T, 1>(h, x, r, p, q, nreal, nrhs, do_p)
@@ -1052,6 +1063,7 @@ extern "C" int hisq_set_option(hisq_ctx* h, const char* key, double value)
     else if (!strcmp(key, "nrhs_inner")) { if (v < 0 || v > 8) return HISQ_EINVAL; h->nrhs_inner = v; }
     else if (!strcmp(key, "naik_compress")) h->naik_compress = v != 0;
     else if (!strcmp(key, "fused_blas")) h->fused_blas = v != 0;
+    else if (!strcmp(key, "dot_fp64")) { if (v < -1 || v > 1) return HISQ_EINVAL; h->dot_fp64 = v; }
     else if (!strcmp(key, "overlap")) { if (v < -1 || v > 1) return HISQ_EINVAL; h->overlap_opt = v; }
     else if (!strcmp(key, "tile_y")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[1] % v))) return HISQ_EINVAL; h->tile_y = v; }
     else if (!strcmp(key, "tile_z")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[2] % v))) return HISQ_EINVAL; h->tile_z = v; }
@@ -1141,7 +1153,11 @@ extern "C" int hisq_cg_host(hisq_ctx* h, void* x_host, const void* b_host, doubl
 struct CgpFields { void *r, *p, *q, *t; };
 static CgpFields cgp_fields(hisq_ctx* h)
 {
-    const size_t fb = field_bytes(h, h->ws_nrhs, elem_size(h->prec));
+    if (h->prec == HISQ_MIXED && h->work_prec == HISQ_FP64) {   // the fp64 pair of the reliable update: r_hi, t_hi
+        char* hi = h->fields + 5 * field_bytes(h, h->ws_nrhs, 4);
+        return { hi, nullptr, nullptr, hi + field_bytes(h, h->ws_nrhs, 8) };
+    }
+    const size_t fb = field_bytes(h, h->ws_nrhs, elem_size(h->work_prec));
     return { h->fields, h->fields + fb, h->fields + 2 * fb, h->fields + 3 * fb };
 }
 
@@ -1228,10 +1244,14 @@ extern "C" int hisq_cgp_begin(hisq_ctx* h, void* x, const void* b, double tol, i
     return h->prec == HISQ_FP32 ? cgp_begin<float>(h, (float*)x, (const float*)b, tol, nrhs)
                                 : cgp_begin<double>(h, (double*)x, (const double*)b, tol, nrhs);
 }
+static int cgp_phase_any(hisq_ctx* h, int phase, double mass)
+{
+    return h->work_prec == HISQ_FP32 ? cgp_phase<float>(h, h->links32, phase, mass) : cgp_phase<double>(h, h->links64, phase, mass);
+}
 extern "C" int hisq_cgp_phase(hisq_ctx* h, int phase, double mass)
 {
     if (!h || h->prec == HISQ_MIXED) return HISQ_EINVAL;
-    return h->prec == HISQ_FP32 ? cgp_phase<float>(h, h->links32, phase, mass) : cgp_phase<double>(h, h->links64, phase, mass);
+    return cgp_phase_any(h, phase, mass);
 }
 // which: 0 = p field, 1 = t field (halo exchange); 2 = rho, 3 = pq, 4 = sums (kMaxNrhs doubles each; all-reduce the first nrhs)
 extern "C" void* hisq_cgp_ptr(hisq_ctx* h, int which)
@@ -1277,7 +1297,7 @@ static int halo_move(hisq_ctx* h, void* field, void* lo, void* hi, int nrhs, uns
     unsigned grid = (unsigned)((total + 255) / 256);
     if (grid > 148 * 4) grid = 148 * 4;
     unsigned* ticket = &h->state->ticket[3];
-    if (h->prec == HISQ_FP32)
+    if (h->work_prec == HISQ_FP32)
         halo_kernel<float, PACK><<<grid, 256, 0, h->stream>>>((float*)field, (float*)lo, (float*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHopMax, nrhs, ticket, sig_a, sig_b);
     else
         halo_kernel<double, PACK><<<grid, 256, 0, h->stream>>>((double*)field, (double*)lo, (double*)hi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, kHopMax, nrhs, ticket, sig_a, sig_b);
@@ -1347,6 +1367,17 @@ extern "C" int hisq_peer_attach(hisq_ctx* h, void* const* boxes, int nboxes, int
     h->mbox_buf = align_up(hisq_halo_bytes(h, nrhs));
     h->mbox_nrhs = nrhs;
     h->seq_send = h->seq_recv = h->red_send = h->red_recv = 0;
+    {   // the protocol counts arrivals from zero: a mailbox that has been used (or poisoned by an abort) is refused
+        unsigned counters[16];
+        CK(cudaMemcpyAsync(counters, h->mbox, sizeof counters, cudaMemcpyDeviceToHost, h->stream));
+        CK(cudaStreamSynchronize(h->stream));
+        for (int i = 0; i < 16; ++i)
+            if (counters[i] != 0) {
+                h->mbox = nullptr;
+                h->last_error = "hisq_peer_attach: this rank's mailbox is not zeroed (used before, or aborted)";
+                return HISQ_EINVAL;
+            }
+    }
     if (!h->d_boxes) CK(cudaMalloc(&h->d_boxes, sizeof(PeerBoxes)));
     CK(cudaMemcpyAsync(h->d_boxes, &h->mbox_all, sizeof(PeerBoxes), cudaMemcpyHostToDevice, h->stream));
     CK(cudaStreamSynchronize(h->stream));
@@ -1464,17 +1495,75 @@ static int cgp_true_residual_t(hisq_ctx* h, const T* links, T* x, const T* b, do
 }
 static int cgp_true_residual(hisq_ctx* h, void* x, const void* b, double mass, int nrhs)
 {
-    return h->prec == HISQ_FP32 ? cgp_true_residual_t<float>(h, h->links32, (float*)x, (const float*)b, mass, nrhs)
+    return h->work_prec == HISQ_FP32 ? cgp_true_residual_t<float>(h, h->links32, (float*)x, (const float*)b, mass, nrhs)
                                 : cgp_true_residual_t<double>(h, h->links64, (double*)x, (const double*)b, mass, nrhs);
 }
 
 // hisq_cg on a partitioned context: the phase-wise iteration with every cross-rank step done through the mailboxes, all
 // on the stream -- the host only polls the state every check_interval iterations.  The all-reduce gives every rank the
 // same bits, so all ranks take the same decisions (stop, breakdown, iteration count) and issue the same calls.
+// Tell every rank that this one is leaving the solve with an error (peer_abort_kernel): on a stream of its own, because
+// the context's stream may itself be waiting for a peer.
+static void peer_abort(hisq_ctx* h)
+{
+    if (!h->mbox) return;
+    if (!h->abort_stream && cudaStreamCreateWithFlags(&h->abort_stream, cudaStreamNonBlocking) != cudaSuccess) return;
+    peer_abort_kernel<<<1, 64, 0, h->abort_stream>>>(h->mbox_all, h->part_nranks);
+    cudaStreamSynchronize(h->abort_stream);
+    cudaStreamSynchronize(h->stream);   // poisoned counters release this rank's own waits too
+}
+// state + this rank's abort word; HISQ_EPEER if a peer has aborted
+static int poll_state_peer(hisq_ctx* h)
+{
+    int rc = poll_state(h);
+    if (rc) return rc;
+    unsigned flag = 0;
+    CK(cudaMemcpyAsync(&flag, h->mbox + kMboxAbortWord * sizeof(unsigned), sizeof flag, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    if (flag) { h->last_error = "a peer rank aborted the solve"; return HISQ_EPEER; }
+    return HISQ_OK;
+}
+// All ranks must run the same sequence of exchanges: compare what decides it (nrhs, max_iter, check_interval, overlap, tol,
+// mass) across the ranks before the first iteration, through one round of the reduce mailbox.
+static int cgp_check_options(hisq_ctx* h, double mass, double tol, int nrhs, bool split)
+{
+    double mine[6] = { (double)nrhs, (double)h->max_iter, (double)h->check_interval, split ? 1.0 : 0.0, tol, mass };
+    CK(cudaMemcpyAsync(h->state->sums, mine, sizeof mine, cudaMemcpyHostToDevice, h->stream));
+    int rc = hisq_peer_reduce_send(h, 4, 6);
+    if (rc) return rc;
+    const double* slot = reduce_wait(h, rc);
+    if (rc) return rc;
+    double all[kMaxRanks * kMaxNrhs];
+    unsigned flag = 0;
+    CK(cudaMemcpyAsync(all, slot, sizeof all, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaMemcpyAsync(&flag, h->mbox + kMboxAbortWord * sizeof(unsigned), sizeof flag, cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    if (flag) { h->last_error = "a peer rank aborted the solve"; return HISQ_EPEER; }   // the wait was released by its poison
+    for (int r = 0; r < h->part_nranks; ++r)
+        for (int i = 0; i < 6; ++i)
+            if (all[r * kMaxNrhs + i] != mine[i]) {
+                h->last_error = "hisq_cg on a partitioned lattice: rank " + std::to_string(r) + " was called with different arguments or options";
+                return HISQ_EINVAL;
+            }
+    return HISQ_OK;
+}
+
+static int cgp_solve_impl(hisq_ctx* h, void* x, const void* b, double mass, double tol, int nrhs);
 static int cgp_solve(hisq_ctx* h, void* x, const void* b, double mass, double tol, int nrhs)
 {
+    const int rc = cgp_solve_impl(h, x, b, mass, tol, nrhs);
+    // HISQ_ENOCONV / HISQ_EBREAKDOWN are decided from all-reduced numbers: every rank returns them together.  Anything else
+    // is this rank's own failure: release the others (they return HISQ_EPEER at their next poll)
+    if (rc != HISQ_OK && rc != HISQ_ENOCONV && rc != HISQ_EBREAKDOWN && rc != HISQ_EPEER) peer_abort(h);
+    return rc;
+}
+static int cgp_solve_impl(hisq_ctx* h, void* x, const void* b, double mass, double tol, int nrhs)
+{
     if (h->prec == HISQ_MIXED || !h->mbox || nrhs > h->mbox_nrhs) return HISQ_EINVAL;
-    int rc = hisq_cgp_begin(h, x, b, tol, nrhs);
+    const bool split_opt = h->overlap_opt < 0 ? h->g.t_cnt >= 4 * kHopMax : h->overlap_opt != 0;
+    int rc = cgp_check_options(h, mass, tol, nrhs, split_opt);
+    if (rc) return rc;
+    rc = hisq_cgp_begin(h, x, b, tol, nrhs);
     if (rc) return rc;
     if ((rc = hisq_peer_reduce_send(h, 2, nrhs)) || (rc = hisq_peer_reduce_recv(h, 2, nrhs)) || (rc = hisq_cgp_phase(h, 0, mass))) return rc;
     void* p = hisq_cgp_ptr(h, 0);
@@ -1483,10 +1572,10 @@ static int cgp_solve(hisq_ctx* h, void* x, const void* b, double mass, double to
     FuseGuard guard{ h };
     // splitting a Dslash costs a launch tail and some L2 reuse: do it when at least half of the owned
     // slices can run under the transfer, or when asked to (option "overlap": -1 auto, 0 never, 1 always)
-    const bool split = h->overlap_opt < 0 ? h->g.t_cnt >= 4 * kHopMax : h->overlap_opt != 0;
+    const bool split = split_opt;
     int confirms = 0;
     for (;;) {
-        if ((rc = poll_state(h))) return rc;
+        if ((rc = poll_state_peer(h))) return rc;
         CgState s = *h->host_state;
         if (s.done && !s.breakdown && s.iter < h->max_iter) {
             if (confirms >= 8) {   // the recursive residual keeps converging, the true one does not: below the attainable accuracy
@@ -1499,7 +1588,7 @@ static int cgp_solve(hisq_ctx* h, void* x, const void* b, double mass, double to
             // iteration resumes from the true residual (the single-GPU rule, a7)
             ++confirms;
             h->fuse_push_pq = h->fuse_push_sums = PeerPush(); h->fuse_red_pq = h->fuse_red_sums = nullptr;
-            if ((rc = cgp_true_residual(h, x, b, mass, nrhs)) || (rc = poll_state(h))) return rc;
+            if ((rc = cgp_true_residual(h, x, b, mass, nrhs)) || (rc = poll_state_peer(h))) return rc;
             s = *h->host_state;
             h->info_reliable = confirms;
         }
@@ -1551,6 +1640,7 @@ extern "C" const char* hisq_strerror(int code)
     case HISQ_ENOCONV: return "CG did not converge within max_iter";
     case HISQ_EBREAKDOWN: return "breakdown (CG: <p,Ap> <= 0 or non-finite scalar; smearing: singular link)";
     case HISQ_EIO: return "file cannot be read / written or fails its checksum";
+    case HISQ_EPEER: return "multi-rank solve aborted by another rank (its error, or options that differ between ranks)";
     default: return "unknown error code";
     }
 }

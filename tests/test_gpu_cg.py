@@ -162,3 +162,39 @@ def test_cg_on_a_side_stream_and_varying_nrhs():
     ref = oracle.dslash_parity(L, X, W, b4_full, 1)
     assert rel_l2(to_full(ctx, L, t, 1), ref) <= 1e-14
     ctx.close()
+
+
+def test_fp32_in_site_partial_sums_do_not_cost_iterations():
+    """DESIGN.md reading R27: in the fp32 operator the 6 products of one site's <p,Ap> are summed in fp32 and widened to
+    fp64 once (SURVEY a6 says "sums in fp64"; the deviation saves 25 % of the n = 4 kernel).  Pin that it costs nothing: a
+    C4-shaped mixed-precision solve (m = 0.002, tol 1e-9, 4 RHS, reduced volume) needs the same number of iterations,
+    to 2 %, with every product widened (option dot_fp64 = 1) and both reach the tolerance (oracle operator)."""
+    L, m, tol, n = (16, 16, 16, 8), 0.002, 1e-9, 4
+    its = {}
+    for wide in (0, 1):
+        ctx, X, W = make_ctx(L, "mixed", n, 5)
+        ctx.set_option("dot_fp64", wide)
+        b_dev, b_full = make_field(ctx, L, 6, n, 0)
+        x_dev, info = ctx.cg(b_dev, m, tol)
+        its[wide] = info["iterations"]
+        assert max(_true_relres(L, X, W, m, to_full(ctx, L, x_dev, 0), b_full)) <= tol
+        ctx.close()
+    assert abs(its[0] - its[1]) <= 0.02 * its[1] + 10, its
+
+
+def test_reliable_updates_keep_their_cadence_after_an_unconfirmed_convergence():
+    """after the first convergence claimed by the fp32 recursion and refused by the fp64 true residual the solve
+    resumes from an iteration count that is no multiple of the batch; the reliable-update schedule must keep firing every
+    `reliable_interval` iterations from there (it used to be tied to iter % R and never fired again, leaving a pure fp32
+    recursion).  A tolerance far below fp32 accuracy with a short interval forces several refused convergences."""
+    L, m, tol, R = (8, 8, 8, 8), 0.3, 1e-13, 10
+    ctx, X, W = make_ctx(L, "mixed", 1, 2)
+    ctx.set_option("reliable_interval", R)
+    ctx.set_option("check_interval", 10)
+    b_dev, b_full = make_field(ctx, L, 3, 1, 0)
+    x_dev, info = ctx.cg(b_dev, m, tol, strict=False)
+    assert info["status"] == 0, info
+    assert _true_relres(L, X, W, m, to_full(ctx, L, x_dev, 0), b_full)[0] <= tol
+    # one true residual per R iterations at least, whatever happened on the way
+    assert info["reliable_updates"] >= info["iterations"] // R, info
+    ctx.close()

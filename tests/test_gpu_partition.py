@@ -442,3 +442,62 @@ def test_partitioned_cg_two_processes_gloo_on_one_gpu(transport):
     b = oracle_field(L, seed + 1, 1, parity=0)
     r = b - oracle.apply_A(L, X, W, m, x)
     assert np.linalg.norm(r) / np.linalg.norm(b) <= 1.05 * tol
+
+
+def _abort_worker(rank, world, port, L, q, case):
+    import os
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import torch.distributed as dist
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    dev = torch.device("cuda:0")
+    ctx = binding.Hisq(L, "fp64", 2, dev, part=(rank, world))
+    fat, naik = partition.make_links_part(L, 3, rank, world, dev)
+    ctx.set_links(fat, naik)
+    peer = partition.PeerHalo(ctx, rank, world, 1, dist)            # mailboxes sized for ONE right-hand side
+    n = 2 if (case == "badcall" and rank == 1) else 1                # rank 1 asks for more than the mailboxes hold
+    if case == "options" and rank == 1:
+        ctx.set_option("max_iter", 77)                               # the ranks would run different numbers of exchanges
+    b = ctx.pack(partition.make_sources_part(L, 4, n, 0, rank, world, dev))
+    code = 0
+    try:
+        ctx.cg(b, 0.2, 1e-8)
+    except binding.HisqError as e:
+        code = e.code
+    reattach = 0
+    try:
+        ctx.peer_attach(ctx._mailboxes, 1)                           # a mailbox that has been used / poisoned is refused
+    except binding.HisqError as e:
+        reattach = e.code
+    q.put((rank, code, reattach))
+    dist.barrier()
+    ctx.close()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("case", ["badcall", "options"])
+def test_multi_rank_solve_fails_on_every_rank_instead_of_hanging(case):
+    """an early error return on one rank used to leave the other rank's stream parked in a stream wait for ever.
+    badcall: rank 1's hisq_cg fails its argument check (HISQ_EINVAL) -> it poisons the counters, rank 0 returns HISQ_EPEER.
+    options: the ranks were given different max_iter -> both see it in the option exchange and return HISQ_EINVAL."""
+    import torch.multiprocessing as mp
+    L, world = (4, 4, 4, 16), 2
+    ctxmp = mp.get_context("spawn")
+    q = ctxmp.Queue()
+    port = 35600 + __import__("os").getpid() % 2000 + (0 if case == "badcall" else 13)
+    ps = [ctxmp.Process(target=_abort_worker, args=(r, world, port, L, q, case)) for r in range(world)]
+    for p in ps:
+        p.start()
+    try:
+        res = dict((r, (c, ra)) for r, c, ra in (q.get(timeout=120) for _ in range(world)))
+        for p in ps:
+            p.join(timeout=60)
+            assert p.exitcode == 0
+    finally:
+        for p in ps:
+            if p.is_alive():
+                p.kill()
+    if case == "badcall":
+        assert res[1][0] == binding.HISQ_EINVAL and res[0][0] == binding.HISQ_EPEER
+    else:
+        assert res[0][0] == binding.HISQ_EINVAL and res[1][0] == binding.HISQ_EINVAL
+    assert res[0][1] == binding.HISQ_EINVAL and res[1][1] == binding.HISQ_EINVAL
