@@ -33,12 +33,19 @@ template <> __device__ __forceinline__ float4 pack16<float>(const float* e) { re
 // Partitioned lattices: the per-iteration updates touch the OWNED slices only.  A field is 3 planes (colour) per RHS,
 // the owned part of a plane is one contiguous run: vector i' of the 3*seg owned vectors is vector
 // (i'/seg)*plane + off + i'%seg of the field.  seg == 0: the whole field, i' = i.
-struct Span { size_t seg, plane, off; };
+// With a z cut as well the owned part of a time slice is itself a run (sub vectors) inside the slice (sub_stride vectors):
+// seg = t_cnt * sub.
+struct Span { size_t seg, plane, off, sub, sub_stride; };
 __device__ __forceinline__ size_t span_map(const Span& sp, size_t i)
 {
     if (sp.seg == 0) return i;
     const size_t c = i / sp.seg;
-    return c * sp.plane + sp.off + (i - c * sp.seg);
+    size_t j = i - c * sp.seg;
+    if (sp.sub) {
+        const size_t tt = j / sp.sub;
+        j = tt * sp.sub_stride + (j - tt * sp.sub);
+    }
+    return c * sp.plane + sp.off + j;
 }
 
 inline int blas_grid_x(size_t nreal, int vec_n) {
@@ -437,19 +444,23 @@ __global__ void cgp_finalize_xr_kernel(CgState* st, int n, const double* red_sum
     if (!any || it >= st->max_iter || st->breakdown) st->done = 1;
 }
 
-// zero the halo slices of a native field, so that sums over the whole extended array are sums over the interior
+// zero everything outside the owned box (t and, with a z cut, z) of a native field, so that sums over the whole extended
+// array are sums over the owned sites.  S = complex per time slice, HLy = complex per z plane.
 template <typename T>
-__global__ void __launch_bounds__(256) zero_halo_kernel(T* __restrict__ field, int S, int Lt_ext, int t_lo, int t_cnt, int nrhs)
+__global__ void __launch_bounds__(256) zero_halo_kernel(T* __restrict__ field, int S, int Lt_ext, int t_lo, int t_cnt, int nrhs,
+                                                        int HLy = 0, int z_lo = 0, int z_cnt = 0)
 {
     using C = typename Vec<T>::c1;
     C* f = reinterpret_cast<C*>(field);
-    const size_t per_plane = (size_t)(Lt_ext - t_cnt) * S, total = (size_t)nrhs * 3 * per_plane;
+    const size_t total = (size_t)nrhs * 3 * Lt_ext * S;
     for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < total; i += (size_t)gridDim.x * 256) {
-        const size_t kc = i / per_plane;
-        size_t j = i % per_plane;
-        if (j >= (size_t)t_lo * S) j += (size_t)t_cnt * S;     // skip the interior
-        C z; z.x = 0; z.y = 0;
-        f[kc * (size_t)Lt_ext * S + j] = z;
+        const int t = (int)((i / S) % Lt_ext);
+        bool out = t < t_lo || t >= t_lo + t_cnt;
+        if (HLy > 0) {
+            const int z = (int)((i % S) / HLy);
+            out = out || z < z_lo || z >= z_lo + z_cnt;
+        }
+        if (out) { C zero; zero.x = 0; zero.y = 0; f[i] = zero; }
     }
 }
 
@@ -566,6 +577,46 @@ __global__ void __launch_bounds__(256) halo_kernel(T* __restrict__ field, T* __r
     }
 }
 
+// ---- z-halo pack / unpack (second cut): H = 3 planes of HLy complex on each side, for the OWNED time slices only (the
+// stencil is axis-aligned: a site reads its z-neighbours at its own t).  Buffers are [k][c][t_cnt][H*HLy] complex; the H
+// planes of one slice are one contiguous run.  Signalling as in halo_kernel.
+template <typename T, bool PACK>
+__global__ void __launch_bounds__(256) zhalo_kernel(T* __restrict__ field, T* __restrict__ lo, T* __restrict__ hi, int HLy, int S,
+                                                    int Lt_ext, int t_lo, int t_cnt, int z_lo, int z_cnt, int H, int nrhs,
+                                                    unsigned* ticket, unsigned* sig_a, unsigned* sig_b)
+{
+    using C = typename Vec<T>::c1;
+    C* f = reinterpret_cast<C*>(field);
+    C* l = reinterpret_cast<C*>(lo);
+    C* u = reinterpret_cast<C*>(hi);
+    const size_t chunk = (size_t)H * HLy, per_kc = (size_t)t_cnt * chunk, total = (size_t)nrhs * 3 * per_kc;
+    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < total; i += (size_t)gridDim.x * 256) {
+        const size_t kc = i / per_kc, rem = i % per_kc;
+        const size_t tt = rem / chunk, j = rem % chunk;
+        const size_t base = (kc * Lt_ext + t_lo + tt) * (size_t)S;
+        if (PACK) {
+            l[i] = f[base + (size_t)z_lo * HLy + j];
+            u[i] = f[base + (size_t)(z_lo + z_cnt - H) * HLy + j];
+        } else {
+            f[base + (size_t)(z_lo - H) * HLy + j] = l[i];
+            f[base + (size_t)(z_lo + z_cnt) * HLy + j] = u[i];
+        }
+    }
+    if (PACK && sig_a != nullptr) {
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence_system();
+            const unsigned done = atomicAdd(ticket, 1u);
+            if (done == gridDim.x - 1) {
+                *ticket = 0;
+                __threadfence_system();
+                atomicAdd_system(sig_a, 1u);
+                atomicAdd_system(sig_b, 1u);
+            }
+        }
+    }
+}
+
 // ---- all-reduce of nrhs doubles through peer-mapped mailboxes (row f3): every rank stores its local sums into EVERY
 // rank's mailbox (slot, source rank) and bumps that mailbox's arrival counter; after a stream wait on its own counter
 // each rank adds the contributions in rank order -- the same order everywhere, so all ranks hold the same bits.
@@ -588,12 +639,12 @@ __global__ void __launch_bounds__(32) peer_reduce_send_kernel(const double* __re
 // their next status poll.  One thread per (mailbox, counter).
 constexpr unsigned kMboxPoison = 0x40000000u;
 constexpr int kMboxAbortWord = 15;
-__global__ void __launch_bounds__(64) peer_abort_kernel(PeerBoxes pb, int nranks)
+__global__ void __launch_bounds__(96) peer_abort_kernel(PeerBoxes pb, int nranks)
 {
-    const int r = threadIdx.x / 4, c = threadIdx.x % 4;
+    const int r = threadIdx.x / 6, c = threadIdx.x % 6;
     if (r >= nranks || pb.box[r] == nullptr) return;
     unsigned* counters = reinterpret_cast<unsigned*>(pb.box[r]);
-    const int idx[4] = { 0, 1, 8, 9 };   // halo slots 0, 1; reduce slots 0, 1
+    const int idx[6] = { 0, 1, 8, 9, 2, 3 };   // t-halo slots 0, 1; reduce slots 0, 1; z-halo slots 0, 1
     if (c == 0) atomicExch_system(counters + kMboxAbortWord, 1u);
     __threadfence_system();
     atomicAdd_system(counters + idx[c], kMboxPoison);
@@ -623,6 +674,38 @@ __device__ __forceinline__ double ms_zeta_next(double zeta, double zeta_prev, do
 {
     const double den = alpha_old * zeta_prev * (1.0 + delta * alpha) + alpha * beta_old * (zeta_prev - zeta);
     return zeta * zeta_prev * alpha_old / den;
+}
+
+// One thread: with rn = ||r||^2 of the new residual, advance every scalar recurrence of the multi-shift iteration
+// (alpha from the state as ms_update_xr_kernel formed it: rho and pq are still those of this iteration).
+__device__ __forceinline__ void ms_advance(CgState* st, double rn, int nshift)
+{
+    const double pq = st->pq[0];
+    const bool ok = pq > 0.0 && isfinite(pq);
+    const double alpha = ok ? st->rho[0] / pq : 0.0;
+    const double alpha_old = st->ms_alpha_old, beta_old = st->ms_beta_old;
+    if (!ok || !isfinite(rn)) st->breakdown = 1;
+    const double beta = rn / st->rho[0];
+    int any = 0;
+    for (int s = 0; s < nshift; ++s) {
+        if (!st->active[s]) continue;
+        const double z = st->ms_zeta[s];
+        const double zn = ms_zeta_next(z, st->ms_zeta_prev[s], alpha, alpha_old, beta_old, st->ms_delta[s]);
+        st->ms_beta_k[s] = beta * (zn / z) * (zn / z);
+        st->ms_zeta_prev[s] = z;
+        st->ms_zeta[s] = zn;
+        if (!isfinite(zn)) st->breakdown = 1;
+        // ||r_s|| = |zeta_s| ||r||; stop at half the requested tolerance (recursion drift margin)
+        if (zn * zn * rn <= 0.25 * st->tol2 * st->bnorm2[0]) st->active[s] = 0;
+        any |= st->active[s];
+    }
+    st->rho_prev[0] = st->rho[0];
+    st->rho[0] = rn;
+    st->ms_alpha_old = alpha;
+    st->ms_beta_old = beta;
+    const int it = st->iter + 1;
+    st->iter = it;
+    if (!any || it >= st->max_iter || st->breakdown) st->done = 1;
 }
 
 // start: r = b, x_k = 0 and p_k = 0 are memset by the host; rho = ||b||^2
@@ -687,7 +770,8 @@ __global__ void __launch_bounds__(kBlasBlock) ms_update_p_kernel(T* __restrict__
 // blockIdx.y == nshift: r -= alpha q, rho' = ||r||^2; the last block advances every scalar recurrence
 template <typename T>
 __global__ void __launch_bounds__(kBlasBlock) ms_update_xr_kernel(T* __restrict__ x, T* __restrict__ r, const T* __restrict__ p,
-                                                                  const T* __restrict__ q, size_t nreal, CgState* st, double* partial)
+                                                                  const T* __restrict__ q, size_t nreal, CgState* st, double* partial,
+                                                                  int defer = 0)
 {
     if (st->done) return;
     using V = typename V16<T>::type;
@@ -743,31 +827,26 @@ __global__ void __launch_bounds__(kBlasBlock) ms_update_xr_kernel(T* __restrict_
     if (grid_reduce<1, kBlasBlock>(sum, k < nshift ? 1 : 0, partial, gridDim.x, blockIdx.x, &st->ticket[1], gridDim.x * gridDim.y,
                                    1, totals)) {
         if (threadIdx.x == 0) {
-            const double rn = totals[0];
-            if (!ok || !isfinite(rn)) st->breakdown = 1;
-            const double beta = rn / st->rho[0];
-            int any = 0;
-            for (int s = 0; s < nshift; ++s) {
-                if (!st->active[s]) continue;
-                const double z = st->ms_zeta[s];
-                const double zn = ms_zeta_next(z, st->ms_zeta_prev[s], alpha, alpha_old, beta_old, st->ms_delta[s]);
-                st->ms_beta_k[s] = beta * (zn / z) * (zn / z);
-                st->ms_zeta_prev[s] = z;
-                st->ms_zeta[s] = zn;
-                if (!isfinite(zn)) st->breakdown = 1;
-                // ||r_s|| = |zeta_s| ||r||; stop at half the requested tolerance (recursion drift margin)
-                if (zn * zn * rn <= 0.25 * st->tol2 * st->bnorm2[0]) st->active[s] = 0;
-                any |= st->active[s];
-            }
-            st->rho_prev[0] = st->rho[0];
-            st->rho[0] = rn;
-            st->ms_alpha_old = alpha;
-            st->ms_beta_old = beta;
-            const int it = st->iter + 1;
-            st->iter = it;
-            if (!any || it >= st->max_iter || st->breakdown) st->done = 1;
+            if (defer) st->sums[0] = totals[0];   // partitioned lattice: the LOCAL sum; ms_finalize_kernel after the all-reduce
+            else ms_advance(st, totals[0], nshift);
         }
     }
+}
+
+// partitioned lattice: the scalar recurrences once ||r||^2 (st->sums[0]) has been all-reduced
+__global__ void ms_finalize_kernel(CgState* st, int nshift)
+{
+    if (st->done) return;
+    ms_advance(st, st->sums[0], nshift);
+}
+
+// partitioned lattice: state from the all-reduced ||b||^2 (st->rho[0]) after ms_init_kernel ran on the local part
+__global__ void ms_finalize_init_kernel(CgState* st, int nshift)
+{
+    const double bb = st->rho[0];
+    st->rho_prev[0] = bb; st->bnorm2[0] = bb;
+    for (int k = 0; k < nshift; ++k) { st->active[k] = bb > 0.0 ? 1 : 0; st->bnorm2[k] = bb; }
+    st->done = bb > 0.0 ? 0 : 1;
 }
 
 }  // namespace hisq

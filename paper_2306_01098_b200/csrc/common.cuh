@@ -42,6 +42,9 @@ struct Geom {
     int part;       // 0: ordinary periodic lattice (t_lo = 0, t_cnt = L[3])
     int t_lo, t_cnt;
     int flip_lo, flip_hi;  // this rank owns the lower / upper global t boundary
+    // second cut, along z (a rank grid nz x nt): the context holds z_cnt planes of the global lattice at local planes
+    // [z_lo, z_lo + z_cnt) of L[2] = z_cnt + 2*z_lo; z-hops never wrap locally (z is periodic: no sign).  zpart = 0: z whole.
+    int zpart, z_lo, z_cnt;
 };
 
 // ---- device-side state of one CG solve (all scalars stay on the GPU) -------------

@@ -286,7 +286,7 @@ __global__ void __launch_bounds__(kDslashBlock, KernelShape<T, NR, MODE>::minb) 
     const int seg = wslab / a.wps, wseg = wslab - seg * a.wps;
     const bool wvalid = seg < a.nseg;
     const int y0 = (tile % g.nty) * g.ty;
-    const int z0 = (tile / g.nty) * g.tz + (a.merged ? 0 : seg);
+    const int z0 = g.z_lo + (tile / g.nty) * g.tz + (a.merged ? 0 : seg);
     const int hseg = H * (y0 + g.L[1] * (z0 + g.L[2] * t));
     const int hb = (hseg >> 5) + wseg;
     const bool valid = wvalid && hb * 32 + lane >= hseg && hb * 32 + lane < hseg + a.seg_len;
@@ -336,6 +336,8 @@ __global__ void __launch_bounds__(kDslashBlock, KernelShape<T, NR, MODE>::minb) 
                 if (mu == 3 && g.part) {   // partitioned in t: read the halo slices, sign only at the global boundary
                     wp = g.flip_hi && cp >= g.t_lo + g.t_cnt;
                     wm = g.flip_lo && cm < g.t_lo;
+                } else if (mu == 2 && g.zpart) {   // partitioned in z: read the halo planes (periodic direction: no sign)
+                    wp = wm = false;
                 } else {
                     cp -= wp ? Lmu : 0;
                     cm += wm ? Lmu : 0;

@@ -43,8 +43,9 @@ struct hisq_ctx {
     int work_prec;         // precision the phase-wise / halo calls operate in: prec, except inside a HISQ_MIXED multi-rank
                            // solve, which switches between the fp32 iteration and the fp64 reliable update
     // peer-memory halo transport (hisq_peer_attach): mailboxes of this rank and of its t-neighbours, exchange counters
-    int part_rank, part_nranks;
-    char *mbox, *mbox_up, *mbox_down;
+    int part_rank, part_nranks, part_nz, part_nt;
+    char *mbox, *mbox_up, *mbox_down, *mbox_zup, *mbox_zdown;
+    size_t mbox_zbuf;      // bytes of one z-halo buffer inside a mailbox
     PeerBoxes mbox_all;    // every rank's mailbox (all-reduce)
     PeerBoxes* d_boxes;    // the same table in device memory (kernels that push their sums themselves)
     // set by cgp_solve around the phases whose kernels push / read the cross-rank sums themselves; all null otherwise
@@ -101,25 +102,26 @@ static int cuda_fail(hisq_ctx* h, cudaError_t e, const char* where)
 static void choose_tiles(hisq_ctx* h, int nrhs, size_t w)
 {
     Geom& g = h->g;
-    int ty = g.L[1], tz = g.L[2];
+    const int Lz = g.z_cnt;   // the owned z planes (all of them unless the lattice is cut along z)
+    int ty = g.L[1], tz = Lz;
     if (h->tile_y > 0 && g.L[1] % h->tile_y == 0) ty = h->tile_y;
-    if (h->tile_z > 0 && g.L[2] % h->tile_z == 0) tz = h->tile_z;
+    if (h->tile_z > 0 && Lz % h->tile_z == 0) tz = h->tile_z;
     if (h->tile_y <= 0 && h->tile_z <= 0) {
         const double target = h->window_mb * 1e6;
         const double per_site = 6.0 * nrhs * (double)w;
         double best_cost = 1e300;
         for (int cy = 4; cy <= g.L[1]; ++cy) {
             if (g.L[1] % cy) continue;
-            for (int cz = 4; cz <= g.L[2]; ++cz) {
-                if (g.L[2] % cz) continue;
+            for (int cz = 4; cz <= Lz; ++cz) {
+                if (Lz % cz) continue;
                 const double window = 7.0 * g.H * cy * cz * per_site;
-                const double halo = (cy == g.L[1] ? 1.0 : (cy + 6.0) / cy) * (cz == g.L[2] ? 1.0 : (cz + 6.0) / cz);
+                const double halo = (cy == g.L[1] ? 1.0 : (cy + 6.0) / cy) * (cz == Lz ? 1.0 : (cz + 6.0) / cz);
                 double cost = halo + (window > target ? 100.0 * window / target : 0.0) - 1e-9 * cy * cz;
                 if (cost < best_cost) { best_cost = cost; ty = cy; tz = cz; }
             }
         }
     }
-    g.ty = ty; g.tz = tz; g.nty = g.L[1] / ty; g.ntz = g.L[2] / tz;
+    g.ty = ty; g.tz = tz; g.nty = g.L[1] / ty; g.ntz = Lz / tz;
 }
 
 extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int prec)
@@ -141,6 +143,7 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
     h->g.stride[0] = 1; h->g.stride[1] = h->g.sy; h->g.stride[2] = h->g.sz; h->g.stride[3] = h->g.st;
     h->g.ty = Ly; h->g.tz = Lz; h->g.nty = 1; h->g.ntz = 1;
     h->g.part = 0; h->g.t_lo = 0; h->g.t_cnt = Lt; h->g.flip_lo = 1; h->g.flip_hi = 1;
+    h->g.zpart = 0; h->g.z_lo = 0; h->g.z_cnt = Lz;
     h->prec = prec;
     h->stream = 0;
     h->cap_stream = nullptr;
@@ -179,18 +182,27 @@ extern "C" int hisq_create(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt, int p
 // Eq. (6)/(7) :467-488).  The context lives on the EXTENDED local lattice Lx x Ly x Lz x (Lt/nranks + 2*kHaloT).
 static const int kHopMax = 3;  // reach of the stencil in one direction (Naik term)
 static const int kHaloT = 4;   // halo slices on each side: 3 are needed (Naik reach), 4 keeps site parity = global parity
-extern "C" int hisq_create_part(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt_global, int prec, int rank, int nranks)
+// rank = rz + nz * rt on an nz x nt grid of ranks: the lattice is cut into nz parts along z and nt along t.  nz = 1 leaves z
+// whole (periodic on every rank, no z halo); the t direction always carries halos (nt = 1: the ring closes on the rank).
+extern "C" int hisq_create_part2(hisq_ctx** out, int Lx, int Ly, int Lz_global, int Lt_global, int prec, int rank, int nz, int nt)
 {
-    if (!out || nranks < 1 || rank < 0 || rank >= nranks || Lt_global % nranks) return HISQ_EINVAL;
-    const int Lt_loc = Lt_global / nranks;
+    if (!out || nz < 1 || nt < 1 || nz * nt > kMaxRanks || rank < 0 || rank >= nz * nt || Lt_global % nt || Lz_global % nz) return HISQ_EINVAL;
+    const int Lt_loc = Lt_global / nt, Lz_loc = Lz_global / nz;
     if (Lt_loc < 4 || (Lt_loc & 1)) return HISQ_EINVAL;   // even (parity) and >= 3 (halo comes from the nearest rank only)
-    int rc = hisq_create(out, Lx, Ly, Lz, Lt_loc + 2 * kHaloT, prec);
+    if (nz > 1 && (Lz_loc < 4 || (Lz_loc & 1))) return HISQ_EINVAL;
+    int rc = hisq_create(out, Lx, Ly, Lz_loc + (nz > 1 ? 2 * kHaloT : 0), Lt_loc + 2 * kHaloT, prec);
     if (rc != HISQ_OK) return rc;
     Geom& g = (*out)->g;
+    const int rz = rank % nz, rt = rank / nz;
     g.part = 1; g.t_lo = kHaloT; g.t_cnt = Lt_loc;
-    g.flip_lo = rank == 0; g.flip_hi = rank == nranks - 1;
-    (*out)->part_rank = rank; (*out)->part_nranks = nranks;
+    g.flip_lo = rt == 0; g.flip_hi = rt == nt - 1;
+    if (nz > 1) { g.zpart = 1; g.z_lo = kHaloT; g.z_cnt = Lz_loc; }
+    (*out)->part_rank = rank; (*out)->part_nranks = nz * nt; (*out)->part_nz = nz; (*out)->part_nt = nt;
     return HISQ_OK;
+}
+extern "C" int hisq_create_part(hisq_ctx** out, int Lx, int Ly, int Lz, int Lt_global, int prec, int rank, int nranks)
+{
+    return hisq_create_part2(out, Lx, Ly, Lz, Lt_global, prec, rank, 1, nranks);
 }
 
 static void drop_graphs(hisq_ctx* h)
@@ -447,10 +459,16 @@ extern "C" int hisq_apply_A(hisq_ctx* h, void* out, const void* in, double mass,
 //   p = r + beta p ; t = D_oe p ; q = m^2 p - D_eo t , <p,q> ; x += alpha p , r -= alpha q , rho' = ||r||^2
 static Span owned_span(const hisq_ctx* h, int vec_n)
 {
-    Span sp = { 0, 0, 0 };
+    Span sp = { 0, 0, 0, 0, 0 };
     if (h->g.part) {   // vectors of vec_n reals; a plane is [Lt_ext][S] complex, the owned run starts at slice t_lo
         const size_t S = (size_t)h->g.Vh / h->g.L[3];
         sp.seg = 2 * S * h->g.t_cnt / vec_n; sp.plane = 2 * S * h->g.L[3] / vec_n; sp.off = 2 * S * h->g.t_lo / vec_n;
+        if (h->g.zpart) {   // ... and inside every owned slice only the planes [z_lo, z_lo + z_cnt) are owned
+            const size_t HLy = (size_t)h->g.H * h->g.L[1];
+            sp.sub = 2 * HLy * h->g.z_cnt / vec_n; sp.sub_stride = 2 * S / vec_n;
+            sp.seg = sp.sub * h->g.t_cnt;
+            sp.off += 2 * HLy * h->g.z_lo / vec_n;
+        }
     }
     return sp;
 }
@@ -838,24 +856,26 @@ static int ms_solve(hisq_ctx* h, const T* links, T* x, const T* b, double mass, 
     return status;
 }
 
+static int cgp_ms_solve(hisq_ctx* h, void* x, const void* b, double mass, const double* shifts, int nshift, double tol);
+
 extern "C" int hisq_cg_multishift(hisq_ctx* h, void* x, const void* b, double mass, const double* shifts, int nshift, double tol)
 {
     if (!h || !x || !b || !shifts || nshift < 1 || nshift > HISQ_MAX_NRHS || !(tol > 0.0) || !std::isfinite(mass)) return HISQ_EINVAL;
     if (((uintptr_t)x & 15) || ((uintptr_t)b & 15)) return HISQ_EINVAL;
     for (int k = 0; k < nshift; ++k)
         if (!(shifts[k] >= 0.0) || !std::isfinite(shifts[k])) return HISQ_EINVAL;
-    if (h->prec == HISQ_MIXED || h->g.part) return HISQ_EINVAL;   // fp64 or fp32 contexts only, not partitioned
+    if (h->prec == HISQ_MIXED) return HISQ_EINVAL;   // fp64 or fp32 contexts only
     if (!h->ws) return HISQ_ENOWORKSPACE;
     if (nshift > h->ws_nrhs) return HISQ_ENOWORKSPACE;
     if (!h->have_links) return HISQ_ENOLINKS;
     const size_t bytes = (size_t)6 * h->g.Vh * elem_size(h->prec);
     if ((const char*)x < (const char*)b + bytes && (const char*)b < (const char*)x + bytes * nshift) return HISQ_EINVAL;
+    if (h->g.part) return cgp_ms_solve(h, x, b, mass, shifts, nshift, tol);   // across ranks: needs the peer mailboxes
     if (h->prec == HISQ_FP32) return ms_solve<float>(h, h->links32, (float*)x, (const float*)b, mass, shifts, nshift, tol);
     return ms_solve<double>(h, h->links64, (double*)x, (const double*)b, mass, shifts, nshift, tol);
 }
 
 static int cgp_solve(hisq_ctx* h, void* x, const void* b, double mass, double tol, int nrhs);
-
 extern "C" int hisq_cg(hisq_ctx* h, void* x, const void* b, double mass, double tol, int nrhs)
 {
     if (!h || !x || !b || nrhs < 1 || nrhs > HISQ_MAX_NRHS || !(tol > 0.0) || !std::isfinite(mass)) return HISQ_EINVAL;
@@ -1066,7 +1086,7 @@ extern "C" int hisq_set_option(hisq_ctx* h, const char* key, double value)
     else if (!strcmp(key, "dot_fp64")) { if (v < -1 || v > 1) return HISQ_EINVAL; h->dot_fp64 = v; }
     else if (!strcmp(key, "overlap")) { if (v < -1 || v > 1) return HISQ_EINVAL; h->overlap_opt = v; }
     else if (!strcmp(key, "tile_y")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[1] % v))) return HISQ_EINVAL; h->tile_y = v; }
-    else if (!strcmp(key, "tile_z")) { if (v < 0 || (v > 0 && (v < 4 || h->g.L[2] % v))) return HISQ_EINVAL; h->tile_z = v; }
+    else if (!strcmp(key, "tile_z")) { if (v < 0 || (v > 0 && (v < 4 || h->g.z_cnt % v))) return HISQ_EINVAL; h->tile_z = v; }
     else if (!strcmp(key, "window_mb")) { if (!(value > 0)) return HISQ_EINVAL; h->window_mb = value; }
     else return HISQ_EINVAL;
     return HISQ_OK;
@@ -1173,7 +1193,7 @@ static int cgp_begin(hisq_ctx* h, T* x, const T* b, double tol, int nrhs)
     const int S = h->g.Vh / h->g.L[3];
     // r = b, then r's halo := 0 so that ||r||^2 over the extended array is the interior sum; LOCAL ||b||^2 -> state.rho
     cudaMemcpyAsync(f.r, b, total * sizeof(T), cudaMemcpyDeviceToDevice, h->stream);
-    zero_halo_kernel<T><<<148 * 4, 256, 0, h->stream>>>((T*)f.r, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, nrhs);
+    zero_halo_kernel<T><<<148 * 4, 256, 0, h->stream>>>((T*)f.r, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, nrhs, h->g.zpart ? h->g.H * h->g.L[1] : 0, h->g.z_lo, h->g.z_cnt);
     dim3 gi((unsigned)init_grid_x(nreal), (unsigned)nrhs);
     cg_init_kernel<T, T><<<gi, kBlasBlock, 0, h->stream>>>((const T*)f.r, (T*)f.r, nreal, h->state, h->partial, tol, h->max_iter);
     h->stats.launches += 2;
@@ -1314,6 +1334,40 @@ extern "C" int hisq_halo_unpack(hisq_ctx* h, void* field, const void* recv_lo, c
     return halo_move<false>(h, field, const_cast<void*>(recv_lo), const_cast<void*>(recv_hi), nrhs);
 }
 
+// the same for the z cut: 3 planes on each side of the owned z range, owned time slices only
+extern "C" size_t hisq_zhalo_bytes(const hisq_ctx* h, int nrhs)
+{
+    if (!h || !h->g.zpart || nrhs < 1 || nrhs > HISQ_MAX_NRHS) return 0;
+    return (size_t)nrhs * 3 * h->g.t_cnt * kHopMax * h->g.H * h->g.L[1] * 2 * elem_size(h->prec);
+}
+template <bool PACK>
+static int zhalo_move(hisq_ctx* h, void* field, void* lo, void* hi, int nrhs, unsigned* sig_a = nullptr, unsigned* sig_b = nullptr)
+{
+    if (!h || !field || !lo || !hi || nrhs < 1 || nrhs > HISQ_MAX_NRHS || !h->g.zpart) return HISQ_EINVAL;
+    if (!h->ws) return HISQ_ENOWORKSPACE;
+    const Geom& g = h->g;
+    const int S = g.Vh / g.L[3], HLy = g.H * g.L[1];
+    const size_t total = (size_t)nrhs * 3 * g.t_cnt * kHopMax * HLy;
+    unsigned grid = (unsigned)((total + 255) / 256);
+    if (grid > 148 * 4) grid = 148 * 4;
+    unsigned* ticket = &h->state->ticket[3];
+    if (h->work_prec == HISQ_FP32)
+        zhalo_kernel<float, PACK><<<grid, 256, 0, h->stream>>>((float*)field, (float*)lo, (float*)hi, HLy, S, g.L[3], g.t_lo, g.t_cnt, g.z_lo, g.z_cnt, kHopMax, nrhs, ticket, sig_a, sig_b);
+    else
+        zhalo_kernel<double, PACK><<<grid, 256, 0, h->stream>>>((double*)field, (double*)lo, (double*)hi, HLy, S, g.L[3], g.t_lo, g.t_cnt, g.z_lo, g.z_cnt, kHopMax, nrhs, ticket, sig_a, sig_b);
+    h->stats.launches++;
+    CK(cudaGetLastError());
+    return HISQ_OK;
+}
+extern "C" int hisq_zhalo_pack(hisq_ctx* h, void* send_lo, void* send_hi, const void* field, int nrhs)
+{
+    return zhalo_move<true>(h, const_cast<void*>(field), send_lo, send_hi, nrhs);
+}
+extern "C" int hisq_zhalo_unpack(hisq_ctx* h, void* field, const void* recv_lo, const void* recv_hi, int nrhs)
+{
+    return zhalo_move<false>(h, field, const_cast<void*>(recv_lo), const_cast<void*>(recv_hi), nrhs);
+}
+
 // ---- halo transport through peer-mapped memory (no library collective) ----------------------------------------
 // Mailbox = [16 counters (u32), 256 B][reduce data: [2 slots][16 ranks][16] doubles][slot 0: lo, hi][slot 1: lo, hi].
 // Counters 0, 1: halo arrivals of the two slots (each exchange adds 2: one per neighbour); 8, 9: reduce arrivals (each
@@ -1347,11 +1401,14 @@ static CUresult stream_wait_geq(hisq_ctx* h, const void* counter, unsigned value
 }
 static char* mbox_buffer(char* box, size_t buf, int slot, int hi) { return box + kMboxFlags + kMboxReduce + (size_t)(2 * slot + hi) * buf; }
 static unsigned* mbox_counter(char* box, int slot) { return reinterpret_cast<unsigned*>(box) + slot; }
+// the z-halo buffers follow the four t-halo buffers; their arrival counters are 2, 3
+static char* mbox_zbuffer(char* box, size_t tbuf, size_t zbuf, int slot, int hi) { return box + kMboxFlags + kMboxReduce + 4 * tbuf + (size_t)(2 * slot + hi) * zbuf; }
+static unsigned* mbox_zcounter(char* box, int slot) { return reinterpret_cast<unsigned*>(box) + 2 + slot; }
 
 extern "C" size_t hisq_peer_bytes(const hisq_ctx* h, int nrhs)
 {
     const size_t b = hisq_halo_bytes(h, nrhs);
-    return b ? kMboxFlags + kMboxReduce + 4 * align_up(b) : 0;
+    return b ? kMboxFlags + kMboxReduce + 4 * align_up(b) + 4 * align_up(hisq_zhalo_bytes(h, nrhs)) : 0;
 }
 extern "C" int hisq_peer_attach(hisq_ctx* h, void* const* boxes, int nboxes, int nrhs)
 {
@@ -1362,9 +1419,15 @@ extern "C" int hisq_peer_attach(hisq_ctx* h, void* const* boxes, int nboxes, int
     if (!load_memops()) { h->last_error = "stream memory operations (cuStreamWaitValue32) are not available"; return HISQ_ECUDA; }
     for (int r = 0; r < kMaxRanks; ++r) h->mbox_all.box[r] = r < nboxes ? (char*)boxes[r] : nullptr;
     h->mbox = (char*)boxes[h->part_rank];
-    h->mbox_up = (char*)boxes[(h->part_rank + 1) % nboxes];
-    h->mbox_down = (char*)boxes[(h->part_rank + nboxes - 1) % nboxes];
+    {   // neighbours on the nz x nt grid of ranks (rank = rz + nz * rt), periodic in both directions
+        const int nz = h->part_nz, nt = h->part_nt, rz = h->part_rank % nz, rt = h->part_rank / nz;
+        h->mbox_up = (char*)boxes[rz + nz * ((rt + 1) % nt)];
+        h->mbox_down = (char*)boxes[rz + nz * ((rt + nt - 1) % nt)];
+        h->mbox_zup = (char*)boxes[(rz + 1) % nz + nz * rt];
+        h->mbox_zdown = (char*)boxes[(rz + nz - 1) % nz + nz * rt];
+    }
     h->mbox_buf = align_up(hisq_halo_bytes(h, nrhs));
+    h->mbox_zbuf = align_up(hisq_zhalo_bytes(h, nrhs));
     h->mbox_nrhs = nrhs;
     h->seq_send = h->seq_recv = h->red_send = h->red_recv = 0;
     {   // the protocol counts arrivals from zero: a mailbox that has been used (or poisoned by an abort) is refused
@@ -1399,6 +1462,12 @@ extern "C" int hisq_halo_send(hisq_ctx* h, const void* field, int nrhs)
                              mbox_buffer(h->mbox_up, h->mbox_buf, s, 0), nrhs, mbox_counter(h->mbox_down, s),
                              mbox_counter(h->mbox_up, s));
     if (rc) return rc;
+    if (h->g.zpart) {   // my lowest planes -> the z-previous rank's UPPER z-halo buffer, my highest -> the z-next rank's LOWER
+        rc = zhalo_move<true>(h, const_cast<void*>(field), mbox_zbuffer(h->mbox_zdown, h->mbox_buf, h->mbox_zbuf, s, 1),
+                              mbox_zbuffer(h->mbox_zup, h->mbox_buf, h->mbox_zbuf, s, 0), nrhs, mbox_zcounter(h->mbox_zdown, s),
+                              mbox_zcounter(h->mbox_zup, s));
+        if (rc) return rc;
+    }
     h->seq_send = e;
     return HISQ_OK;
 }
@@ -1412,6 +1481,12 @@ extern "C" int hisq_halo_recv(hisq_ctx* h, void* field, int nrhs)
     CKU(stream_wait_geq(h, mbox_counter(h->mbox, s), 2u * uses));
     int rc = halo_move<false>(h, field, mbox_buffer(h->mbox, h->mbox_buf, s, 0), mbox_buffer(h->mbox, h->mbox_buf, s, 1), nrhs);
     if (rc) return rc;
+    if (h->g.zpart) {
+        CKU(stream_wait_geq(h, mbox_zcounter(h->mbox, s), 2u * uses));
+        rc = zhalo_move<false>(h, field, mbox_zbuffer(h->mbox, h->mbox_buf, h->mbox_zbuf, s, 0),
+                               mbox_zbuffer(h->mbox, h->mbox_buf, h->mbox_zbuf, s, 1), nrhs);
+        if (rc) return rc;
+    }
     h->seq_recv = e;
     return HISQ_OK;
 }
@@ -1508,7 +1583,7 @@ static void peer_abort(hisq_ctx* h)
 {
     if (!h->mbox) return;
     if (!h->abort_stream && cudaStreamCreateWithFlags(&h->abort_stream, cudaStreamNonBlocking) != cudaSuccess) return;
-    peer_abort_kernel<<<1, 64, 0, h->abort_stream>>>(h->mbox_all, h->part_nranks);
+    peer_abort_kernel<<<1, 96, 0, h->abort_stream>>>(h->mbox_all, h->part_nranks);
     cudaStreamSynchronize(h->abort_stream);
     cudaStreamSynchronize(h->stream);   // poisoned counters release this rank's own waits too
 }
@@ -1557,72 +1632,237 @@ static int cgp_solve(hisq_ctx* h, void* x, const void* b, double mass, double to
     if (rc != HISQ_OK && rc != HISQ_ENOCONV && rc != HISQ_EBREAKDOWN && rc != HISQ_EPEER) peer_abort(h);
     return rc;
 }
+// start of a HISQ_MIXED multi-rank solve: fp64 interface (x, b), fp32 iteration fields r p q t x_lo, fp64 pair r_hi t_hi
+static int cgp_begin_mixed(hisq_ctx* h, double* x, const double* b, double tol, int nrhs)
+{
+    const size_t nreal = (size_t)6 * h->g.Vh, total = nreal * nrhs;
+    const size_t fb32 = field_bytes(h, h->ws_nrhs, 4), fb64 = field_bytes(h, h->ws_nrhs, 8);
+    float* r = (float*)h->fields;
+    float* xlo = (float*)(h->fields + 4 * fb32);
+    double* rhi = (double*)(h->fields + 5 * fb32);
+    double* thi = (double*)(h->fields + 5 * fb32 + fb64);
+    CK(cudaMemsetAsync(x, 0, total * 8, h->stream));
+    CK(cudaMemsetAsync(h->fields + fb32, 0, 4 * fb32, h->stream));   // p, q, t, x_lo
+    CK(cudaMemsetAsync(thi, 0, total * 8, h->stream));
+    // r_hi = b with zeroed halo slices (sums over the extended arrays are then interior sums); r = (float) r_hi;
+    // LOCAL ||b||^2 in fp64 -> state.rho
+    CK(cudaMemcpyAsync(rhi, b, total * 8, cudaMemcpyDeviceToDevice, h->stream));
+    const int S = h->g.Vh / h->g.L[3];
+    zero_halo_kernel<double><<<148 * 4, 256, 0, h->stream>>>(rhi, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, nrhs, h->g.zpart ? h->g.H * h->g.L[1] : 0, h->g.z_lo, h->g.z_cnt);
+    dim3 gi((unsigned)init_grid_x(nreal), (unsigned)nrhs);
+    cg_init_kernel<double, float><<<gi, kBlasBlock, 0, h->stream>>>(rhi, r, nreal, h->state, h->partial, tol, h->max_iter);
+    h->stats.launches += 2;
+    CK(cudaGetLastError());
+    h->cgp_x = xlo; h->cgp_nrhs = nrhs; h->cgp_tol = tol;
+    return HISQ_OK;
+}
+
+struct WorkPrecGuard {   // the working precision never outlives the solve
+    hisq_ctx* h;
+    ~WorkPrecGuard() { h->work_prec = h->prec == HISQ_MIXED ? HISQ_FP64 : h->prec; }
+};
+
 static int cgp_solve_impl(hisq_ctx* h, void* x, const void* b, double mass, double tol, int nrhs)
 {
-    if (h->prec == HISQ_MIXED || !h->mbox || nrhs > h->mbox_nrhs) return HISQ_EINVAL;
-    const bool split_opt = h->overlap_opt < 0 ? h->g.t_cnt >= 4 * kHopMax : h->overlap_opt != 0;
+    if (!h->mbox || nrhs > h->mbox_nrhs) return HISQ_EINVAL;
+    const bool mixed = h->prec == HISQ_MIXED;
+    // with a z cut every time slice reads the z halo: the interior / edge split by time slices does not apply
+    const bool split_opt = !h->g.zpart && (h->overlap_opt < 0 ? h->g.t_cnt >= 4 * kHopMax : h->overlap_opt != 0);
     int rc = cgp_check_options(h, mass, tol, nrhs, split_opt);
     if (rc) return rc;
-    rc = hisq_cgp_begin(h, x, b, tol, nrhs);
+    WorkPrecGuard wguard{ h };
+    h->work_prec = mixed ? HISQ_FP32 : h->prec;     // the iteration's precision (phases, halos, fields)
+    rc = mixed ? cgp_begin_mixed(h, (double*)x, (const double*)b, tol, nrhs) : hisq_cgp_begin(h, x, b, tol, nrhs);
     if (rc) return rc;
-    if ((rc = hisq_peer_reduce_send(h, 2, nrhs)) || (rc = hisq_peer_reduce_recv(h, 2, nrhs)) || (rc = hisq_cgp_phase(h, 0, mass))) return rc;
-    void* p = hisq_cgp_ptr(h, 0);
-    void* t = hisq_cgp_ptr(h, 1);
+    if ((rc = hisq_peer_reduce_send(h, 2, nrhs)) || (rc = hisq_peer_reduce_recv(h, 2, nrhs)) || (rc = cgp_phase_any(h, 0, mass))) return rc;
+    const CgpFields fl = cgp_fields(h);
+    void* p = fl.p;
+    void* t = fl.t;
+    const size_t total = (size_t)6 * h->g.Vh * nrhs;
     h->info_reliable = 0;
     FuseGuard guard{ h };
     // splitting a Dslash costs a launch tail and some L2 reuse: do it when at least half of the owned
     // slices can run under the transfer, or when asked to (option "overlap": -1 auto, 0 never, 1 always)
     const bool split = split_opt;
-    int confirms = 0;
+    // HISQ_MIXED: every R iterations (counted from the last one) x_hi += x_lo and r is replaced by the fp64 true residual
+    // over all ranks, as on one GPU (a8); batches divide R so that a poll falls on every boundary
+    const int R = mixed ? h->reliable_interval : 0;
+    int batch = h->check_interval > 0 ? h->check_interval : 32;
+    if (R > 0) {
+        int best = 1;
+        for (int d = 1; d <= R && d <= batch; ++d)
+            if (R % d == 0) best = d;
+        batch = best;
+    }
+    int confirms = 0, rel_base = 0;
+    bool have_true = false;
     for (;;) {
         if ((rc = poll_state_peer(h))) return rc;
         CgState s = *h->host_state;
-        if (s.done && !s.breakdown && s.iter < h->max_iter) {
-            if (confirms >= 8) {   // the recursive residual keeps converging, the true one does not: below the attainable accuracy
+        const bool claimed = s.done && !s.breakdown && s.iter < h->max_iter;
+        const bool due = R > 0 && !s.done && s.iter > rel_base && (s.iter - rel_base) % R == 0;
+        if (claimed || due) {
+            if (claimed && confirms >= 8) {   // the recursive residual keeps converging, the true one does not: below the attainable accuracy
                 h->info_iters = s.iter;
                 for (int k = 0; k < nrhs; ++k) h->info_relres[k] = s.bnorm2[k] > 0.0 ? std::sqrt(((const double*)((const char*)h->host_state + sizeof(CgState)))[k] / s.bnorm2[k]) : 0.0;
                 return HISQ_ENOCONV;
             }
-            // converged by the recursive residual: confirm with r = b - A x across the ranks (halo of x, of D_oe x, one
-            // all-reduce); the bookkeeping kernel re-activates the systems whose true residual is above tol and the
-            // iteration resumes from the true residual (the single-GPU rule, a7)
-            ++confirms;
+            // converged by the recursive residual (or a reliable update is due): r = b - A x across the ranks (halo of x,
+            // of D_oe x, one all-reduce); the bookkeeping kernel re-activates the systems whose true residual is above tol
+            // and the iteration resumes from the true residual (the single-GPU rule, a7 / a8)
+            if (claimed) ++confirms;
             h->fuse_push_pq = h->fuse_push_sums = PeerPush(); h->fuse_red_pq = h->fuse_red_sums = nullptr;
-            if ((rc = cgp_true_residual(h, x, b, mass, nrhs)) || (rc = poll_state_peer(h))) return rc;
+            if (mixed) {
+                acc_xhi_kernel<<<(unsigned)((total / 4 + kBlasBlock - 1) / kBlasBlock + 1), kBlasBlock, 0, h->stream>>>((double*)x, (float*)h->cgp_x, total);
+                h->stats.launches++;
+                h->work_prec = HISQ_FP64;
+                rc = cgp_true_residual_t<double>(h, h->links64, (double*)x, (const double*)b, mass, nrhs);
+                const CgpFields hi = cgp_fields(h);
+                h->work_prec = HISQ_FP32;
+                if (rc) return rc;
+                convert_kernel<double, float><<<1184, kBlasBlock, 0, h->stream>>>((const double*)hi.r, (float*)fl.r, total);
+                h->stats.launches++;
+                CK(cudaGetLastError());
+            } else if ((rc = cgp_true_residual(h, x, b, mass, nrhs))) return rc;
+            if ((rc = poll_state_peer(h))) return rc;
             s = *h->host_state;
-            h->info_reliable = confirms;
+            rel_base = s.iter;
+            have_true = true;
+            h->info_reliable++;
         }
         if (s.done || s.breakdown || s.iter >= h->max_iter) {
+            if (mixed && !(claimed || due)) {   // stopped by max_iter or a breakdown: hand out what has been accumulated
+                acc_xhi_kernel<<<(unsigned)((total / 4 + kBlasBlock - 1) / kBlasBlock + 1), kBlasBlock, 0, h->stream>>>((double*)x, (float*)h->cgp_x, total);
+                h->stats.launches++;
+                CK(cudaStreamSynchronize(h->stream));
+            }
             h->info_iters = s.iter;
+            (void)have_true;
             for (int k = 0; k < nrhs; ++k) h->info_relres[k] = s.bnorm2[k] > 0.0 ? std::sqrt(s.rho[k] / s.bnorm2[k]) : 0.0;
             if (s.breakdown) return HISQ_EBREAKDOWN;
             int any = 0;      // done is also raised at max_iter: converged = no system left active
             for (int k = 0; k < nrhs; ++k) any |= s.active[k];
             return any ? HISQ_ENOCONV : HISQ_OK;
         }
-        for (int i = 0; i < h->check_interval; ++i) {
-            if ((rc = hisq_cgp_phase(h, 1, mass))) return rc;
+        for (int i = 0; i < batch; ++i) {
+            if ((rc = cgp_phase_any(h, 1, mass))) return rc;
             // the kernels that produce <p,q> and ||r||^2 push them to all ranks themselves, those that consume them add up
             // the mailbox entries themselves: no reduction kernel, one stream wait per all-reduce
             h->fuse_push_pq = reduce_next_push(h);
             if (split) {   // interior slices while the halo is in flight, edge slices once it has arrived
-                if ((rc = hisq_halo_send(h, p, nrhs)) || (rc = hisq_cgp_phase(h, 20, mass))) return rc;
-                if ((rc = hisq_halo_recv(h, p, nrhs)) || (rc = hisq_cgp_phase(h, 21, mass))) return rc;
-                if ((rc = hisq_halo_send(h, t, nrhs)) || (rc = hisq_cgp_phase(h, 30, mass))) return rc;
-                if ((rc = hisq_halo_recv(h, t, nrhs)) || (rc = hisq_cgp_phase(h, 31, mass))) return rc;
+                if ((rc = hisq_halo_send(h, p, nrhs)) || (rc = cgp_phase_any(h, 20, mass))) return rc;
+                if ((rc = hisq_halo_recv(h, p, nrhs)) || (rc = cgp_phase_any(h, 21, mass))) return rc;
+                if ((rc = hisq_halo_send(h, t, nrhs)) || (rc = cgp_phase_any(h, 30, mass))) return rc;
+                if ((rc = hisq_halo_recv(h, t, nrhs)) || (rc = cgp_phase_any(h, 31, mass))) return rc;
             } else {
-                if ((rc = hisq_halo_send(h, p, nrhs)) || (rc = hisq_halo_recv(h, p, nrhs)) || (rc = hisq_cgp_phase(h, 2, mass))) return rc;
-                if ((rc = hisq_halo_send(h, t, nrhs)) || (rc = hisq_halo_recv(h, t, nrhs)) || (rc = hisq_cgp_phase(h, 3, mass))) return rc;
+                if ((rc = hisq_halo_send(h, p, nrhs)) || (rc = hisq_halo_recv(h, p, nrhs)) || (rc = cgp_phase_any(h, 2, mass))) return rc;
+                if ((rc = hisq_halo_send(h, t, nrhs)) || (rc = hisq_halo_recv(h, t, nrhs)) || (rc = cgp_phase_any(h, 3, mass))) return rc;
             }
             h->fuse_red_pq = reduce_wait(h, rc);            // <p,q> of all ranks have arrived
             if (rc) return rc;
             h->fuse_push_sums = reduce_next_push(h);
-            if ((rc = hisq_cgp_phase(h, 4, mass))) return rc;
+            if ((rc = cgp_phase_any(h, 4, mass))) return rc;
             h->fuse_red_sums = reduce_wait(h, rc);          // ||r||^2 of all ranks have arrived
             if (rc) return rc;
-            if ((rc = hisq_cgp_phase(h, 5, mass))) return rc;
+            if ((rc = cgp_phase_any(h, 5, mass))) return rc;
         }
     }
+}
+
+// Multi-shift CG across the ranks of a partitioned lattice (PAPER.md:141 on top of :187-191): the single-GPU iteration
+// (ms_solve) with the two halo exchanges of the base direction and the two all-reduces (<p,q>, ||r||^2: one double each)
+// put where the cross-rank steps are due; the other shifts cost AXPYs only, as on one GPU.
+template <typename T>
+static int cgp_ms_solve_t(hisq_ctx* h, const T* links, T* x, const T* b, double mass, const double* shifts, int nshift, double tol)
+{
+    if (!h->mbox || h->mbox_nrhs < 1) return HISQ_EINVAL;
+    double shift_sum = 0.0;
+    for (int k = 0; k < nshift; ++k) shift_sum += shifts[k] * (k + 1);
+    int rc = cgp_check_options(h, mass + shift_sum, tol, nshift, false);
+    if (rc) return rc;
+    const size_t nreal = (size_t)6 * h->g.Vh;
+    const size_t fb = field_bytes(h, h->ws_nrhs, sizeof(T));
+    T* r = (T*)(h->fields);
+    T* p = (T*)(h->fields + fb);
+    T* q = (T*)(h->fields + 2 * fb);
+    T* t = (T*)(h->fields + 3 * fb);
+    int kmin = 0;
+    for (int k = 1; k < nshift; ++k)
+        if (shifts[k] < shifts[kmin]) kmin = k;
+    const double m2_base = mass * mass + shifts[kmin];
+    h->info_iters = 0; h->info_reliable = 0;
+    CK(cudaMemsetAsync(x, 0, nreal * nshift * sizeof(T), h->stream));
+    CK(cudaMemsetAsync(p, 0, nreal * nshift * sizeof(T), h->stream));
+    CK(cudaMemsetAsync(q, 0, nreal * sizeof(T), h->stream));
+    CK(cudaMemsetAsync(t, 0, nreal * sizeof(T), h->stream));
+    // r = b with zeroed halo slices, LOCAL ||b||^2 -> rho, all-reduce, then the state from the global value
+    CK(cudaMemcpyAsync(r, b, nreal * sizeof(T), cudaMemcpyDeviceToDevice, h->stream));
+    const int S = h->g.Vh / h->g.L[3];
+    zero_halo_kernel<T><<<148 * 4, 256, 0, h->stream>>>(r, S, h->g.L[3], h->g.t_lo, h->g.t_cnt, 1, h->g.zpart ? h->g.H * h->g.L[1] : 0, h->g.z_lo, h->g.z_cnt);
+    ms_init_kernel<T><<<(unsigned)init_grid_x(nreal), kBlasBlock, 0, h->stream>>>(r, r, nreal, h->state, h->partial, tol, h->max_iter, nshift);
+    h->stats.launches += 2;
+    double delta[kMaxNrhs];
+    for (int k = 0; k < nshift; ++k) delta[k] = shifts[k] - shifts[kmin];
+    CK(cudaMemcpyAsync(h->state->ms_delta, delta, nshift * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));   // `delta` is a stack array
+    if ((rc = hisq_peer_reduce_send(h, 2, 1)) || (rc = hisq_peer_reduce_recv(h, 2, 1))) return rc;
+    ms_finalize_init_kernel<<<1, 1, 0, h->stream>>>(h->state, nshift);
+    h->stats.launches++;
+    const unsigned gx = (unsigned)blas_grid_x(nreal, V16<T>::n);
+    T* pb = p + (size_t)kmin * nreal;   // the base direction: the smallest shift has zeta = 1
+    int status = HISQ_OK;
+    for (;;) {
+        if ((rc = poll_state_peer(h))) return rc;
+        const CgState s = *h->host_state;
+        if (s.done || s.breakdown || s.iter >= h->max_iter) {
+            h->info_iters = s.iter;
+            if (s.breakdown) status = HISQ_EBREAKDOWN;
+            else
+                for (int k = 0; k < nshift; ++k)
+                    if (s.active[k]) status = HISQ_ENOCONV;
+            break;
+        }
+        for (int i = 0; i < h->check_interval; ++i) {
+            ms_update_p_kernel<T><<<dim3(gx, (unsigned)nshift), kBlasBlock, 0, h->stream>>>(p, r, nreal, h->state);
+            h->stats.launches++;
+            if ((rc = hisq_halo_send(h, pb, 1)) || (rc = hisq_halo_recv(h, pb, 1))) return rc;
+            if ((rc = run_dslash<T>(h, links, t, pb, HISQ_ODD, 1, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, &h->state->done, 2))) return rc;
+            if ((rc = hisq_halo_send(h, t, 1)) || (rc = hisq_halo_recv(h, t, 1))) return rc;
+            if ((rc = run_dslash<T>(h, links, q, t, HISQ_EVEN, 1, MODE_APPLY_A, pb, nullptr, m2_base, h->state->pq, &h->state->done, 2))) return rc;
+            if ((rc = hisq_peer_reduce_send(h, 3, 1)) || (rc = hisq_peer_reduce_recv(h, 3, 1))) return rc;
+            ms_update_xr_kernel<T><<<dim3(gx, (unsigned)nshift + 1), kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial, 1);
+            h->stats.launches++;
+            if ((rc = hisq_peer_reduce_send(h, 4, 1)) || (rc = hisq_peer_reduce_recv(h, 4, 1))) return rc;
+            ms_finalize_kernel<<<1, 1, 0, h->stream>>>(h->state, nshift);
+            h->stats.launches++;
+            CK(cudaGetLastError());
+        }
+    }
+    // true residuals ||b - (A + sigma_k) x_k|| / ||b|| per shift over all ranks (q and t are free now)
+    for (int k = 0; k < nshift; ++k) {
+        const double m2k = mass * mass + shifts[k];
+        T* xk = x + (size_t)k * nreal;
+        if ((rc = hisq_halo_send(h, xk, 1)) || (rc = hisq_halo_recv(h, xk, 1))) return rc;
+        if ((rc = run_dslash<T>(h, links, t, xk, HISQ_ODD, 1, MODE_PLAIN, nullptr, nullptr, 0.0, nullptr, nullptr, 2))) return rc;
+        if ((rc = hisq_halo_send(h, t, 1)) || (rc = hisq_halo_recv(h, t, 1))) return rc;
+        if ((rc = run_dslash<T>(h, links, q, t, HISQ_EVEN, 1, MODE_RESID, xk, b, m2k, h->state->sums + k, nullptr, 2))) return rc;
+    }
+    if ((rc = hisq_peer_reduce_send(h, 4, nshift)) || (rc = hisq_peer_reduce_recv(h, 4, nshift))) return rc;
+    if ((rc = poll_state_peer(h)) != HISQ_OK) return rc;
+    const CgState& s = *h->host_state;
+    for (int k = 0; k < nshift; ++k) {
+        h->info_relres[k] = s.bnorm2[0] > 0.0 ? std::sqrt(s.sums[k] / s.bnorm2[0]) : 0.0;
+        if (status == HISQ_OK && !(h->info_relres[k] <= tol)) status = HISQ_ENOCONV;
+    }
+    return status;
+}
+
+static int cgp_ms_solve(hisq_ctx* h, void* x, const void* b, double mass, const double* shifts, int nshift, double tol)
+{
+    const int rc = h->prec == HISQ_FP32 ? cgp_ms_solve_t<float>(h, h->links32, (float*)x, (const float*)b, mass, shifts, nshift, tol)
+                                        : cgp_ms_solve_t<double>(h, h->links64, (double*)x, (const double*)b, mass, shifts, nshift, tol);
+    if (rc != HISQ_OK && rc != HISQ_ENOCONV && rc != HISQ_EBREAKDOWN && rc != HISQ_EPEER) peer_abort(h);
+    return rc;
 }
 
 extern "C" int hisq_naik_compressed(const hisq_ctx* h) { return h && h->naik_c14 ? 1 : 0; }

@@ -501,3 +501,112 @@ def test_multi_rank_solve_fails_on_every_rank_instead_of_hanging(case):
     else:
         assert res[0][0] == binding.HISQ_EINVAL and res[1][0] == binding.HISQ_EINVAL
     assert res[0][1] == binding.HISQ_EINVAL and res[1][1] == binding.HISQ_EINVAL
+
+
+def _interior(ctx, L, world, field, n):
+    Le = partition.extended_lattice(L, world)
+    S = ctx.Vh // Le[3]
+    return ctx.unpack(field).view(n, Le[3], S, 3)[:, partition.HALO_T:Le[3] - partition.HALO_T].reshape(n, -1, 3)
+
+
+def test_mixed_precision_and_multishift_on_a_single_rank_ring():
+    """PAPER.md:135 / :141 on partitioned contexts: HISQ_MIXED hisq_cg and hisq_cg_multishift with the
+    mailboxes attached (one rank, the ring closes on itself), against the same calls on the plain lattice and the oracle
+    operator."""
+    L, m, seed = (4, 4, 6, 12), 0.05, 21
+    dev = torch.device("cuda:0")
+    X, W = oracle_links(L, seed)
+    # mixed precision, 2 right-hand sides, reliable updates every 20 iterations
+    n, tol = 2, 1e-10
+    ctx = binding.Hisq(L, "mixed", n, dev, part=(0, 1))
+    ctx.set_links(*partition.make_links_part(L, seed, 0, 1, dev))
+    ctx.set_option("reliable_interval", 20)
+    b = ctx.pack(partition.make_sources_part(L, seed + 1, n, 0, 0, 1, dev))
+    peer = partition.PeerHalo(ctx, 0, 1, n)
+    x, info = ctx.cg(b, m, tol)
+    assert info["reliable_updates"] >= info["iterations"] // 20 and max(info["true_rel_resid"]) <= tol
+    xf = oracle.half_to_full(L, _interior(ctx, L, 1, x, n).cpu().numpy(), 0)
+    bf = oracle_field(L, seed + 1, n, parity=0)
+    r = bf - oracle.apply_A(L, X, W, m, xf)
+    for k in range(n):
+        assert np.linalg.norm(r[k]) / np.linalg.norm(bf[k]) <= tol
+    peer.close(); ctx.close()
+    # multi-shift, 4 shifts
+    shifts, tol = [0.0, 0.01, 0.3, 2.0], 1e-9
+    ctx = binding.Hisq(L, "fp64", len(shifts), dev, part=(0, 1))
+    ctx.set_links(*partition.make_links_part(L, seed, 0, 1, dev))
+    b = ctx.pack(partition.make_sources_part(L, seed + 2, 1, 0, 0, 1, dev))
+    peer = partition.PeerHalo(ctx, 0, 1, 1)
+    xs, info = ctx.cg_multishift(b, m, shifts, tol)
+    assert max(info["true_rel_resid"]) <= tol
+    xf = oracle.half_to_full(L, _interior(ctx, L, 1, xs, len(shifts)).cpu().numpy(), 0)
+    bf = oracle_field(L, seed + 2, 1, parity=0)
+    for k, sg in enumerate(shifts):
+        rk = bf[0] - oracle.apply_A(L, X, W, float(np.sqrt(m * m + sg)), xf[k:k + 1])[0]
+        assert np.linalg.norm(rk) / np.linalg.norm(bf[0]) <= tol
+    peer.close(); ctx.close()
+
+
+def _mp_worker2(rank, world, port, L, m, tol, seed, q, mode, shifts):
+    import os
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import torch.distributed as dist
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    dev = torch.device("cuda:0")
+    nx = len(shifts) if mode == "multishift" else 1
+    ctx = binding.Hisq(L, "mixed" if mode == "mixed" else "fp64", nx, dev, part=(rank, world))
+    ctx.set_links(*partition.make_links_part(L, seed, rank, world, dev))
+    if mode == "mixed":
+        ctx.set_option("reliable_interval", 25)
+    b = ctx.pack(partition.make_sources_part(L, seed + 1, 1, 0, rank, world, dev))
+    peer = partition.PeerHalo(ctx, rank, world, 1, dist)
+    if mode == "mixed":
+        x, info = ctx.cg(b, m, tol)
+    else:
+        x, info = ctx.cg_multishift(b, m, shifts, tol)
+    peer.close()
+    xr = torch.view_as_real(_interior(ctx, L, world, x, nx).cpu()).contiguous()
+    parts = [torch.empty_like(xr) for _ in range(world)] if rank == 0 else None
+    dist.gather(xr, parts, dst=0)
+    if rank == 0:
+        q.put((info, [torch.view_as_complex(p).numpy() for p in parts]))
+    dist.barrier()
+    ctx.close()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("mode", ["mixed", "multishift"])
+def test_mixed_and_multishift_two_processes_on_one_gpu(mode):
+    """Two PROCESSES, mailboxes mapped through CUDA IPC, hisq_cg (HISQ_MIXED) and hisq_cg_multishift driving the iteration
+    from C across the two ranks; judged by the oracle operator on the reassembled solution."""
+    import torch.multiprocessing as mp
+    L, m, tol, seed, world = (4, 4, 6, 16), 0.1, 1e-9, 11, 2
+    shifts = [0.0, 0.02, 0.5]
+    ctxmp = mp.get_context("spawn")
+    q = ctxmp.Queue()
+    port = 36700 + __import__("os").getpid() % 2000 + (0 if mode == "mixed" else 19)
+    ps = [ctxmp.Process(target=_mp_worker2, args=(r, world, port, L, m, tol, seed, q, mode, shifts)) for r in range(world)]
+    for p in ps:
+        p.start()
+    try:
+        info, parts = q.get(timeout=150)
+        for p in ps:
+            p.join(timeout=120)
+            assert p.exitcode == 0
+    finally:
+        for p in ps:
+            if p.is_alive():
+                p.kill()
+    assert info["status"] == 0
+    xh = np.concatenate(parts, axis=1).astype(np.complex128)
+    X, W = oracle_links(L, seed)
+    b = oracle_field(L, seed + 1, 1, parity=0)
+    if mode == "mixed":
+        assert info["reliable_updates"] >= info["iterations"] // 25
+        r = b - oracle.apply_A(L, X, W, m, oracle.half_to_full(L, xh, 0))
+        assert np.linalg.norm(r) / np.linalg.norm(b) <= 1.05 * tol
+    else:
+        xf = oracle.half_to_full(L, xh, 0)
+        for k, sg in enumerate(shifts):
+            rk = b[0] - oracle.apply_A(L, X, W, float(np.sqrt(m * m + sg)), xf[k:k + 1])[0]
+            assert np.linalg.norm(rk) / np.linalg.norm(b[0]) <= 1.05 * tol
