@@ -223,8 +223,26 @@ int hisq_cg_host(hisq_ctx *h, void *x_host, const void *b_host, double mass, dou
  * mailboxes are attached (hisq_peer_attach, below; HISQ_EINVAL before): every rank calls it with its slab of b and
  * gets its slab of x (halo slices of x are overwritten); same arithmetic and stopping rule as on one GPU, including
  * the true-residual confirmation b - A x (over all ranks) and the resume if it fails; hisq_get_info reports the
- * global true residuals, identical on every rank.  hisq_cg_multishift and HISQ_MIXED: HISQ_EINVAL. */
+ * global true residuals, identical on every rank.  HISQ_MIXED contexts run the fp32 iteration across the ranks with the
+ * fp64 reliable update (halos of x and D_oe x in fp64, one all-reduce) every `reliable_interval` iterations;
+ * hisq_cg_multishift (fp32 / fp64 contexts) runs the base system's two halo exchanges and two one-number all-reduces per
+ * iteration, every rank getting its slab of all nshift solutions; mailboxes sized for nrhs >= 1 suffice for it.
+ * A rank that fails releases the others: they return HISQ_EPEER instead of waiting for ever; every rank must be called
+ * with the same arguments and options (checked at the start of the solve, HISQ_EINVAL on all ranks if not). */
 int hisq_create_part(hisq_ctx **h, int Lx, int Ly, int Lz, int Lt_global, int prec, int rank, int nranks);
+/* A second cut, along z: an nz x nt grid of ranks, rank = rz + nz * rt (the paper's sub-lattices are 4-dimensional,
+ * PAPER.md:187-191; two cuts are what lets the 8 GPUs of a node share BASELINE's C5, whose Lt = 24 admits at most 6 ranks
+ * along t).  With nz > 1 the extended local lattice is Lx x Ly x (Lz/nz + 8) x (Lt/nt + 8): local plane 4 + j is global
+ * plane rz*Lz_loc + j, the 4 planes on each side are halos (3 are read; periodic direction, no sign).  The stencil is
+ * axis-aligned, so the two halos are independent: z planes are exchanged for the owned time slices only, no corners.
+ * Lz/nz and Lt/nt must be even and >= 4, nz * nt <= 16.  nz = 1 is hisq_create_part.  Everything said there holds;
+ * hisq_halo_send / recv move both halos; hisq_cg does not split its Dslashes around the exchange on such a context (every
+ * time slice reads the z halo).  hisq_zhalo_bytes / pack / unpack are the z counterparts of hisq_halo_bytes / pack /
+ * unpack: buffers [k][c][Lt_loc][3 * (Lx/2) * Ly] complex; 0 / HISQ_EINVAL on a context without a z cut. */
+int hisq_create_part2(hisq_ctx **h, int Lx, int Ly, int Lz_global, int Lt_global, int prec, int rank, int nz, int nt);
+size_t hisq_zhalo_bytes(const hisq_ctx *h, int nrhs);
+int hisq_zhalo_pack(hisq_ctx *h, void *send_lo, void *send_hi, const void *field, int nrhs);
+int hisq_zhalo_unpack(hisq_ctx *h, void *field, const void *recv_lo, const void *recv_hi, int nrhs);
 /* hisq_dslash restricted to the OWNED time slices [t_first, t_first + t_count) (0 <= t_first, t_first + t_count <= the
  * number of owned slices: Lt_loc on a partitioned context, Lt otherwise); all other slices of `out` are left untouched.
  * The slices [3, Lt_loc - 3) read no halo slice (the stencil reaches 3 sites), so the caller can compute

@@ -30,6 +30,7 @@ EXPORTS = [
     "hisq_cgp_begin", "hisq_cgp_phase", "hisq_cgp_ptr", "hisq_cgp_status", "hisq_strerror",
     "hisq_last_error", "hisq_debug_dslash_regs", "hisq_debug_tiles",
     "hisq_cfg_info", "hisq_cfg_read", "hisq_cfg_write",
+    "hisq_create_part2", "hisq_zhalo_bytes", "hisq_zhalo_pack", "hisq_zhalo_unpack",
 ]
 
 _lib = None
@@ -82,8 +83,13 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_cg_host.argtypes = [vp, vp, vp, d, d, i]
     lib.hisq_naik_compressed.argtypes = [vp]
     lib.hisq_create_part.argtypes = [ctypes.POINTER(vp), i, i, i, i, i, i, i]
+    lib.hisq_create_part2.argtypes = [ctypes.POINTER(vp), i, i, i, i, i, i, i, i]
     lib.hisq_halo_bytes.argtypes = [vp, i]
     lib.hisq_halo_bytes.restype = sz
+    lib.hisq_zhalo_bytes.argtypes = [vp, i]
+    lib.hisq_zhalo_bytes.restype = sz
+    lib.hisq_zhalo_pack.argtypes = [vp, vp, vp, vp, i]
+    lib.hisq_zhalo_unpack.argtypes = [vp, vp, vp, vp, i]
     lib.hisq_peer_bytes.argtypes = [vp, i]
     lib.hisq_peer_bytes.restype = sz
     lib.hisq_peer_attach.argtypes = [vp, ctypes.POINTER(vp), i, i]
@@ -114,8 +120,19 @@ _PREC = {"fp32": HISQ_FP32, "fp64": HISQ_FP64, "mixed": HISQ_MIXED}
 
 
 def rank_grid(L: Sequence[int], nranks: int):
-    """(nz, nt): how hisq_create_part cuts the lattice over nranks ranks (rank = rz + nz * rt)."""
-    return (1, int(nranks))
+    """(nz, nt): how the lattice is cut over nranks ranks (hisq_create_part2; rank = rz + nz * rt).  The cut along t alone
+    is preferred (contiguous halos); a z cut is added when Lt / nranks is not an even number >= 4 (C5's Lt = 24 on 8
+    ranks: 2 x 4).  Raises ValueError if no admissible grid exists."""
+    ok = lambda ext, n: ext % n == 0 and (ext // n) % 2 == 0 and ext // n >= 4
+    for nz in range(1, int(nranks) + 1):
+        if nranks % nz == 0 and ok(L[3], nranks // nz) and (nz == 1 or ok(L[2], nz)):
+            return (nz, int(nranks) // nz)
+    raise ValueError(f"no (nz, nt) grid of {nranks} ranks fits the lattice {tuple(L)}: local extents must be even and >= 4")
+
+
+def _grid_of(part):
+    """part = (rank, nranks) [t cut only] or (rank, nz, nt) -> (rank, nz, nt)."""
+    return (int(part[0]), 1, int(part[1])) if len(part) == 2 else (int(part[0]), int(part[1]), int(part[2]))
 
 
 class Hisq:
@@ -128,16 +145,21 @@ class Hisq:
 
     def __init__(self, L: Sequence[int], prec: str = "fp64", nrhs_max: int = 1, device: Optional[torch.device] = None,
                  part: Optional[tuple] = None):
-        """part = (rank, nranks): this context is rank's share of the lattice L partitioned along t (hisq_create_part);
-        self.L then is the EXTENDED local lattice (Lt/nranks + 8 slices) that every layout refers to."""
+        """part = (rank, nranks): this context is rank's share of the lattice L partitioned along t (hisq_create_part), or
+        part = (rank, nz, nt): cut nz times along z and nt times along t (hisq_create_part2, rank = rz + nz * rt);
+        self.L then is the EXTENDED local lattice (Lt/nt + 8 slices, and Lz/nz + 8 planes if nz > 1) that every layout
+        refers to."""
         layout.check_extents(L)
         self.part = part
         self.L_global = tuple(int(v) for v in L)
         if part is not None:
-            rank, nranks = part
-            if L[3] % nranks or (L[3] // nranks) % 2 or L[3] // nranks < 4:
-                raise ValueError("Lt / nranks must be even and >= 4")
-            L = (L[0], L[1], L[2], L[3] // nranks + 8)
+            rank, nz, nt = _grid_of(part)
+            if L[3] % nt or (L[3] // nt) % 2 or L[3] // nt < 4:
+                raise ValueError("Lt / nt must be even and >= 4")
+            if nz > 1 and (L[2] % nz or (L[2] // nz) % 2 or L[2] // nz < 4):
+                raise ValueError("Lz / nz must be even and >= 4")
+            self.grid = (nz, nt)
+            L = (L[0], L[1], L[2] // nz + (8 if nz > 1 else 0), L[3] // nt + 8)
         if not torch.cuda.is_available():
             raise RuntimeError("libhisq needs a CUDA device (no CPU fallback)")
         self.lib = load_library()
@@ -153,7 +175,7 @@ class Hisq:
             if part is None:
                 self._check(self.lib.hisq_create(ctypes.byref(self._h), *self.L, _PREC[prec]))
             else:
-                self._check(self.lib.hisq_create_part(ctypes.byref(self._h), *self.L_global, _PREC[prec], part[0], part[1]))
+                self._check(self.lib.hisq_create_part2(ctypes.byref(self._h), *self.L_global, _PREC[prec], *_grid_of(part)))
             self._check(self.lib.hisq_set_stream(self._h, ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)))
             nbytes = self.lib.hisq_workspace_bytes(self._h, self.nrhs_max)
             if nbytes == 0:
@@ -335,6 +357,21 @@ class Hisq:
 
     def halo_unpack(self, field: torch.Tensor, lo: torch.Tensor, hi: torch.Tensor):
         self._check(self.lib.hisq_halo_unpack(self._h, self._ptr(field), self._ptr(lo), self._ptr(hi), field.shape[0]))
+
+    # the same for the z cut (contexts created with nz > 1): 3 planes on each side, owned time slices only
+    def zhalo_buffers(self, nrhs: int):
+        nb = self.lib.hisq_zhalo_bytes(self._h, nrhs)
+        if nb == 0:
+            raise HisqError(-1, "not a z-partitioned context")
+        n = nb // (nrhs * 3 * (8 if self.prec == "fp32" else 16))
+        mk = lambda: torch.empty((nrhs, 3, n), dtype=self.cdtype, device=self.device)
+        return mk(), mk()
+
+    def zhalo_pack(self, field: torch.Tensor, lo: torch.Tensor, hi: torch.Tensor):
+        self._check(self.lib.hisq_zhalo_pack(self._h, self._ptr(lo), self._ptr(hi), self._ptr(field), field.shape[0]))
+
+    def zhalo_unpack(self, field: torch.Tensor, lo: torch.Tensor, hi: torch.Tensor):
+        self._check(self.lib.hisq_zhalo_unpack(self._h, self._ptr(field), self._ptr(lo), self._ptr(hi), field.shape[0]))
 
     # -- halo transport through peer-mapped mailboxes ------------------------------------------------
     def peer_mailbox(self, nrhs: int) -> torch.Tensor:

@@ -15,13 +15,27 @@ HALO_T = 4
 HOP_MAX = 3   # reach of the stencil along one direction (Naik term)
 
 
-def extended_lattice(L: Sequence[int], nranks: int):
-    return (int(L[0]), int(L[1]), int(L[2]), int(L[3]) // nranks + 2 * HALO_T)
+def grid_of(nranks):
+    """nranks = an int (cut along t only) or a pair (nz, nt) (cut along z and t; rank = rz + nz * rt) -> (nz, nt)."""
+    return (1, int(nranks)) if isinstance(nranks, int) else (int(nranks[0]), int(nranks[1]))
 
 
-def global_sites_of_rank(L: Sequence[int], rank: int, nranks: int, device="cpu") -> torch.Tensor:
+def extended_lattice(L: Sequence[int], nranks):
+    nz, nt = grid_of(nranks)
+    return (int(L[0]), int(L[1]), int(L[2]) // nz + (2 * HALO_T if nz > 1 else 0), int(L[3]) // nt + 2 * HALO_T)
+
+
+def owned_box(L: Sequence[int], nranks):
+    """(z_lo, z_cnt, t_lo, t_cnt): the owned planes / slices inside the extended local lattice."""
+    nz, nt = grid_of(nranks)
+    return (HALO_T if nz > 1 else 0, int(L[2]) // nz, HALO_T, int(L[3]) // nt)
+
+
+def global_sites_of_rank(L: Sequence[int], rank: int, nranks, device="cpu") -> torch.Tensor:
     """For every memory index eo of rank's EXTENDED lattice (Eq. 4 on that lattice), the GLOBAL lexicographic site
-    it is a copy of (halo slices wrap around the global lattice)."""
+    it is a copy of (halo slices / planes wrap around the global lattice)."""
+    nz, nt = grid_of(nranks)
+    rz, rt = rank % nz, rank // nz
     Le = extended_lattice(L, nranks)
     lex = layout.lex_of_eo(Le, device=device)
     x = lex % Le[0]
@@ -30,11 +44,21 @@ def global_sites_of_rank(L: Sequence[int], rank: int, nranks: int, device="cpu")
     r = r // Le[1]
     z = r % Le[2]
     t = r // Le[2]
-    tg = (rank * (L[3] // nranks) + t - HALO_T) % L[3]
-    return x + L[0] * (y + L[1] * (z + L[2] * tg))
+    tg = (rt * (L[3] // nt) + t - HALO_T) % L[3]
+    zg = (rz * (L[2] // nz) + z - HALO_T) % L[2] if nz > 1 else z
+    return x + L[0] * (y + L[1] * (zg + L[2] * tg))
 
 
-def make_links_part(L, seed: int, rank: int, nranks: int, device, cdtype=torch.complex128, gen_device=None):
+def interior(ctx, L: Sequence[int], nranks, canonical: torch.Tensor) -> torch.Tensor:
+    """The owned sites of a CANONICAL half-lattice field [n, Vh_ext, 3] of a partitioned context, as [n, t_cnt, z_cnt, H*Ly, 3]."""
+    Le = extended_lattice(L, nranks)
+    z_lo, z_cnt, t_lo, t_cnt = owned_box(L, nranks)
+    HLy = Le[0] // 2 * Le[1]
+    v = canonical.view(canonical.shape[0], Le[3], Le[2], HLy, 3)
+    return v[:, t_lo:t_lo + t_cnt, z_lo:z_lo + z_cnt]
+
+
+def make_links_part(L, seed: int, rank: int, nranks, device, cdtype=torch.complex128, gen_device=None):
     """(fat, naik) canonical on rank's extended lattice: [4, V_ext, 3, 3]."""
     g = torch.device(gen_device) if gen_device is not None else torch.device("cpu")
     sites = global_sites_of_rank(L, rank, nranks, device=g)
@@ -43,7 +67,7 @@ def make_links_part(L, seed: int, rank: int, nranks: int, device, cdtype=torch.c
     return fat, naik
 
 
-def make_sources_part(L, seed: int, nrhs: int, parity: int, rank: int, nranks: int, device, cdtype=torch.complex128,
+def make_sources_part(L, seed: int, nrhs: int, parity: int, rank: int, nranks, device, cdtype=torch.complex128,
                       gen_device=None, fill_halo: bool = False):
     """Gaussian sources on one parity of rank's extended lattice, canonical [nrhs, Vh_ext, 3]; halo slices are zero
     unless fill_halo (they are what the exchange must deliver)."""
@@ -53,10 +77,12 @@ def make_sources_part(L, seed: int, nrhs: int, parity: int, rank: int, nranks: i
     sites = global_sites_of_rank(L, rank, nranks, device=g)[parity * Vh:(parity + 1) * Vh]
     src = inputs.sources(L, seed, sites, nrhs).to(cdtype)
     if not fill_halo:
-        S = Vh // Le[3]
-        v = src.view(nrhs, Le[3], S, 3)
-        v[:, :HALO_T] = 0
-        v[:, Le[3] - HALO_T:] = 0
+        z_lo, z_cnt, t_lo, t_cnt = owned_box(L, nranks)
+        v = src.view(nrhs, Le[3], Le[2], -1, 3)
+        v[:, :t_lo] = 0
+        v[:, t_lo + t_cnt:] = 0
+        v[:, :, :z_lo] = 0
+        v[:, :, z_lo + z_cnt:] = 0
     return src.contiguous().to(device)
 
 
@@ -195,9 +221,12 @@ class PeerHalo:
 
 
 class PartitionedCG:
-    """One rank's side of the multi-RHS CG on a t-partitioned lattice (include/hisq.h, hisq_cgp_*): every kernel is the
-    library's; this class only sequences the phases and performs the two cross-rank steps between them -- halo
-    exchange of a field and all-reduce of nrhs doubles -- through `dist` (torch.distributed: NCCL between GPUs)."""
+    """TEST SCAFFOLD, not the product path: one rank's side of the multi-RHS CG on a t-partitioned lattice sequenced from
+    Python over the phase-wise calls (include/hisq.h, hisq_cgp_*), so that the phases can be checked one by one and ranks
+    can be emulated in lockstep inside one process.  The product is hisq_cg on a partitioned context, which drives the
+    same phases from C with every cross-rank step on the stream (hisq.cu, cgp_solve).  Every kernel is the library's;
+    this class only sequences the phases and performs the two cross-rank steps between them -- halo exchange of a field
+    and all-reduce of nrhs doubles -- through `dist` (torch.distributed: NCCL between GPUs).  t cut only."""
 
     def __init__(self, ctx, rank: int, nranks: int, dist=None, peer: "PeerHalo | None" = None):
         """peer: move the halos AND the all-reduces of the scalar products through peer-mapped mailboxes (PeerHalo)
