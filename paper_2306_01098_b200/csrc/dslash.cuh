@@ -187,7 +187,7 @@ template <typename T, int NR, int MODE = 0> struct KernelShape {
     static constexpr bool f32 = sizeof(T) == 4;
     static constexpr int vb = NR >= 6 ? 4 : NR;   // gathered vectors in flight per stencil term
     static constexpr int minb = NR >= 6 ? (f32 ? 4 : 1)
-                              : NR >= 3 ? (f32 ? (MODE == 0 ? 6 : 4) : 3)
+                              : NR >= 3 ? (f32 ? (MODE == 0 ? 5 : 4) : 3)
                               : NR == 2 ? (f32 ? 8 : 5) : (f32 ? 3 : 4);
     static constexpr bool early = MODE != MODE_PLAIN && NR <= 4;   // fetch the epilogue operands before the stencil
 };
