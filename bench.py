@@ -217,23 +217,30 @@ def oracle_block(cfg):
     return tuple(L)
 
 
-def oracle_sample(cfg, seed: int, budget_s: float):
-    """Time the oracle on a bounded sample of the step: `iters` CG iterations of ONE right-hand side on oracle_block."""
+def oracle_inputs(cfg, seed: int):
+    """The oracle's inputs on oracle_block(cfg), generated once: (L, X, W, b, mass)."""
     import oracle
     from paper_2306_01098_b200 import inputs
     L = oracle_block(cfg)
-    V = inputs.volume(L)
-    s = torch.arange(V, dtype=torch.int64)
+    s = torch.arange(inputs.volume(L), dtype=torch.int64)
     X = inputs.fat_links(L, seed, s).numpy()
     W = inputs.naik_links(L, seed, s).numpy()
     b = inputs.sources(L, seed, s, 1).numpy()
-    par = oracle.site_parity(L)
-    b[:, par == 1, :] = 0
-    mass = cfg["mass"] if cfg["mass"] is not None else 0.1
-    t0 = time.perf_counter()
-    oracle.cg(L, X, W, mass, 1e-30, b, max_iter=1)
-    t1 = time.perf_counter() - t0
-    iters = max(2, min(2000, int(budget_s / max(t1 / 2, 1e-3))))   # 1 iteration = 2 A-applies incl. the final check
+    b[:, oracle.site_parity(L) == 1, :] = 0
+    return L, X, W, b, (cfg["mass"] if cfg["mass"] is not None else 0.1)
+
+
+def oracle_sample(cfg, seed: int, budget_s: float, prepared=None, iters=None):
+    """Time the oracle on a bounded sample of the step: `iters` CG iterations of ONE right-hand side on oracle_block
+    (iters chosen from a one-iteration probe to fill budget_s unless given)."""
+    import oracle
+    L, X, W, b, mass = prepared if prepared is not None else oracle_inputs(cfg, seed)
+    V = L[0] * L[1] * L[2] * L[3]
+    if iters is None:
+        t0 = time.perf_counter()
+        oracle.cg(L, X, W, mass, 1e-30, b, max_iter=1)
+        t1 = time.perf_counter() - t0
+        iters = max(2, min(2000, int(budget_s / max(t1 / 2, 1e-3))))   # 1 iteration = 2 A-applies incl. the final check
     t0 = time.perf_counter()
     oracle.cg(L, X, W, mass, 1e-30, b, max_iter=iters)
     dt = time.perf_counter() - t0
@@ -242,15 +249,19 @@ def oracle_sample(cfg, seed: int, budget_s: float):
     sample = (f"{iters} CG iterations (2 Dslash each, + 1 final residual) of 1 of the {cfg['nrhs']} right-hand sides on a "
               f"{L[0]}x{L[1]}x{L[2]}x{L[3]} " + ("lattice (the config's own)" if tuple(L) == tuple(cfg["L"]) else
                                                 f"block of the {'x'.join(map(str, cfg['L']))} lattice (same generators)") + f", {dt:.1f} s")
-    return gflops, dt, sample, oracle.threads()
+    return gflops, dt, sample, oracle.threads(), iters
 
 
 def run_reference(args, cfg, rank):
+    """This tier's reference arm: the oracle as it stands on the host cores, rank 0 only.  Inputs are generated once; every
+    step is the same bounded sample, sized so that the whole --steps K --warmup W run ends within a few minutes."""
     if rank != 0:
         return
-    vals, dts = [], []
+    prepared = oracle_inputs(cfg, 0)
+    budget = max(1.5, min(args.ref_budget, 150.0 / max(args.steps + args.warmup, 1)))
+    vals, dts, iters, sample, cores = [], [], None, "", 0
     for i in range(args.warmup + args.steps):
-        g, dt, sample, cores = oracle_sample(cfg, 0, args.ref_budget)
+        g, dt, sample, cores, iters = oracle_sample(cfg, 0, budget, prepared, iters)
         if i >= args.warmup:
             vals.append(g)
             dts.append(dt)
@@ -540,7 +551,7 @@ def main():
     if rank == 0 and not args.no_extras:
         out["extras_c2"] = extras_c2(dev, peak, ctxpk)
     if rank == 0 and not args.no_cpu_baseline:
-        g, dt, sample, cores = oracle_sample(cfg, 0, args.cpu_budget)
+        g, dt, sample, cores, _ = oracle_sample(cfg, 0, args.cpu_budget)
         out["cpu_baseline"] = {"value": g, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample}
     if rank == 0:
         print(json.dumps(out))
