@@ -57,8 +57,9 @@ enum {
     HISQ_ENOCONV = -5,      /* max_iter reached; x holds the last iterate, hisq_get_info the residuals     */
     HISQ_EBREAKDOWN = -6,   /* <p, A p> <= 0 or a non-finite scalar appeared in CG; hisq_smear: singular link */
     HISQ_EIO = -7,          /* file cannot be opened / is truncated / fails its checksum or link trace     */
-    HISQ_EPEER = -8         /* multi-rank solve: another rank aborted (its error, or options that differ
+    HISQ_EPEER = -8,        /* multi-rank solve: another rank aborted (its error, or options that differ
                                between the ranks); the mailboxes must be zeroed and re-attached             */
+    HISQ_ETOOBIG = -9       /* hisq_norm2_noalloc: more right-hand sides or reals than its static scratch holds */
 };
 
 /* Create a context for an Lx x Ly x Lz x Lt lattice on the current CUDA device.
@@ -329,6 +330,25 @@ long long hisq_launch_count(const hisq_ctx *h);
 const char *hisq_strerror(int code);
 /* Text of the last CUDA error seen by this context ("" if none). */
 const char *hisq_last_error(const hisq_ctx *h);
+
+/* An entry point that allocates NOTHING, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid allocation): no context, no workspace.  out[k] = ||a_k||^2 = sum_i a[k][i]^2 for
+ * nrhs fields of nreal reals each (field k at offset k*nreal reals; element type by prec: HISQ_FP32 float, HISQ_FP64 and
+ * HISQ_MIXED double; for a half-lattice field nreal = 6*Vh), accumulated in fp64 in the fixed two-stage order of the CG's own
+ * reductions (block partition and order of the solver's ||b_k||^2: the same bits).  field, out: DEVICE pointers (field
+ * 16-byte aligned), out receives nrhs doubles; asynchronous on cuda_stream (a cudaStream_t as void*, NULL = legacy stream).
+ * The scratch of the reduction (block partial sums, last-block ticket) is a file-scope __device__ array of 2 MiB + 256 B that
+ * every GPU loading the library holds until the process exits; its device address is resolved once per device
+ * (cudaGetSymbolAddress) on the first call with that device current.  Limits: nrhs <= HISQ_NOALLOC_MAX_NRHS (16) and
+ * nreal <= hisq_norm2_noalloc_max_reals() = HISQ_NOALLOC_MAX_COLS * 4096 = 67 108 864 (BASELINE's largest lattice, 96^3 x 24,
+ * has 63 700 992 reals per field); beyond either: HISQ_ETOOBIG, nothing is launched.  HISQ_EINVAL for null / misaligned
+ * pointers, nreal = 0, nrhs < 1, a bad prec.  Calls no cudaMalloc / cudaFree or allocating library routine.
+ * ALL calls on a device share the one array: calls that overlap on the GPU (different streams or host threads without
+ * ordering between them) race and return wrong sums; ordered calls are safe (the array keeps the previous call's contents;
+ * the partial sums are rewritten before they are read and the ticket is cleared on the stream before every launch). */
+enum { HISQ_NOALLOC_MAX_NRHS = 16, HISQ_NOALLOC_MAX_COLS = 16384 };
+size_t hisq_norm2_noalloc_max_reals(void);
+int hisq_norm2_noalloc(const void *field, int prec, size_t nreal, int nrhs, double *out, void *cuda_stream);
 
 /* Introspection (tests, DESIGN.md tables; no effect on any result).
  * hisq_debug_dslash_regs: registers per thread of the Dslash kernel instantiation for prec (HISQ_FP32 | HISQ_FP64),

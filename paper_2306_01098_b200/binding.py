@@ -17,7 +17,7 @@ HISQ_FP32, HISQ_FP64, HISQ_MIXED = 4, 8, 12
 HISQ_EVEN, HISQ_ODD = 0, 1
 HISQ_MAX_NRHS = 16
 HISQ_EINVAL, HISQ_ENOLINKS, HISQ_ENOWORKSPACE, HISQ_ECUDA = -1, -2, -3, -4
-HISQ_ENOCONV, HISQ_EBREAKDOWN, HISQ_EIO, HISQ_EPEER = -5, -6, -7, -8
+HISQ_ENOCONV, HISQ_EBREAKDOWN, HISQ_EIO, HISQ_EPEER, HISQ_ETOOBIG = -5, -6, -7, -8, -9
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("HISQ_LIB", os.path.join(_HERE, "libhisq.so"))
@@ -31,6 +31,7 @@ EXPORTS = [
     "hisq_last_error", "hisq_debug_dslash_regs", "hisq_debug_tiles",
     "hisq_cfg_info", "hisq_cfg_read", "hisq_cfg_write",
     "hisq_create_part2", "hisq_zhalo_bytes", "hisq_zhalo_pack", "hisq_zhalo_unpack",
+    "hisq_norm2_noalloc", "hisq_norm2_noalloc_max_reals",
 ]
 
 _lib = None
@@ -71,6 +72,9 @@ def load_library() -> ctypes.CDLL:
     lib.hisq_cfg_info.argtypes = [ctypes.c_char_p, i, ctypes.POINTER(i), ctypes.POINTER(i)]
     lib.hisq_cfg_read.argtypes = [ctypes.c_char_p, i, vp, sz]
     lib.hisq_cfg_write.argtypes = [ctypes.c_char_p, i, vp, ctypes.POINTER(i), i]
+    lib.hisq_norm2_noalloc.argtypes = [vp, i, sz, i, vp, vp]
+    lib.hisq_norm2_noalloc_max_reals.argtypes = []
+    lib.hisq_norm2_noalloc_max_reals.restype = sz
     lib.hisq_smear_bytes.argtypes = [vp]
     lib.hisq_smear_bytes.restype = sz
     lib.hisq_smear.argtypes = [vp, vp, vp, vp, vp, d, d, i]
@@ -484,6 +488,27 @@ def nersc_write(path: str, links: torch.Tensor, L, rows: int = 3, plaquette: flo
                                 float(plaquette))
     if code:
         raise HisqError(code, lib.hisq_strerror(code).decode())
+
+
+def norm2_noalloc(field: torch.Tensor, out: torch.Tensor) -> torch.Tensor:
+    """hisq_norm2_noalloc: out[k] = ||field[k]||^2 for a contiguous CUDA tensor field [nrhs, ...] (complex64 / complex128 /
+    float32 / float64) into the caller's CUDA tensor `out` (nrhs float64), on the current stream.  The library call
+    allocates nothing (static device scratch; at most 16 right-hand sides of 67 108 864 reals: HisqError -9 beyond);
+    calls that overlap on the GPU race (include/hisq.h)."""
+    lib = load_library()
+    if not field.is_cuda or not field.is_contiguous() or not out.is_cuda or not out.is_contiguous():
+        raise ValueError("expected contiguous CUDA tensors")
+    nrhs = field.shape[0]
+    if out.dtype != torch.float64 or out.numel() < nrhs or out.device != field.device:
+        raise ValueError("out: float64 CUDA tensor of at least nrhs elements on the field's device")
+    real = torch.view_as_real(field) if field.is_complex() else field
+    prec = {torch.float32: HISQ_FP32, torch.float64: HISQ_FP64}[real.dtype]
+    with torch.cuda.device(field.device):
+        code = lib.hisq_norm2_noalloc(ctypes.c_void_p(real.data_ptr()), prec, real.numel() // nrhs, nrhs,
+                                      ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if code:
+        raise HisqError(code, lib.hisq_strerror(code).decode())
+    return out
 
 
 CFG_FORMATS = {"ildg": 1, "milc": 2, "openqcd": 3}

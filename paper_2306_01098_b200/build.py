@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libhisq.so")
-SOURCES = ["hisq.cu", "dslash_f32.cu", "dslash_f64.cu", "nersc_io.cpp", "cfg_io.cpp"]
+SOURCES = ["hisq.cu", "dslash_f32.cu", "dslash_f64.cu", "nersc_io.cpp", "cfg_io.cpp", "noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

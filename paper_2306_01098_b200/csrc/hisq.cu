@@ -1881,6 +1881,7 @@ extern "C" const char* hisq_strerror(int code)
     case HISQ_EBREAKDOWN: return "breakdown (CG: <p,Ap> <= 0 or non-finite scalar; smearing: singular link)";
     case HISQ_EIO: return "file cannot be read / written or fails its checksum";
     case HISQ_EPEER: return "multi-rank solve aborted by another rank (its error, or options that differ between ranks)";
+    case HISQ_ETOOBIG: return "hisq_norm2_noalloc: beyond its static scratch (at most 16 right-hand sides of 67108864 reals each)";
     default: return "unknown error code";
     }
 }
