@@ -538,8 +538,10 @@ static int enqueue_iteration(hisq_ctx* h, const T* links, T* x, T* r, T* p, T* q
     if (rc) return rc;
     if (keep == 0) {
         // x is not touched here: its update is folded into the next iteration's p pass (or cg_solve's flush)
-        // large fields: several chunks per CTA (blas.cuh), as long as >= 16 CTAs per SM remain
-        int trips = (int)((size_t)gb.x * nrhs / ((size_t)h->num_sms * 16));
+        // several chunks per CTA (blas.cuh: the dependent scalar loads at the head of a CTA and its reduction tail cost as
+        // much as streaming one chunk), as long as >= 2 CTAs per SM remain; up to 8.  Measured on C4 (48^3 x 12, mixed,
+        // n = 4): 57.8 us at one chunk per CTA, iteration 0.432 -> 0.412 ms with this rule (>= 16 CTAs per SM: no change there)
+        int trips = (int)((size_t)gb.x * nrhs / ((size_t)h->num_sms * 2));
         trips = trips < 1 ? 1 : (trips > 8 ? 8 : trips);
         dim3 gt((gb.x + trips - 1) / trips, (unsigned)nrhs);
         cg_update_xr_kernel<T><<<gt, kBlasBlock, 0, h->stream>>>(x, r, p, q, nreal, h->state, h->partial, 0, PeerPush(), nullptr, Span(), 1, trips);
