@@ -14,10 +14,7 @@
 namespace hisq {
 
 constexpr int kBlasBlock = 256;
-#ifndef HISQ_BLAS_ITEMS
-#define HISQ_BLAS_ITEMS 4
-#endif
-constexpr int kBlasItems = HISQ_BLAS_ITEMS;  // 16-byte vectors per thread
+constexpr int kBlasItems = 4;  // 16-byte vectors per thread
 
 template <typename T> struct V16;
 template <> struct V16<double> { using type = double2; static constexpr int n = 2; };

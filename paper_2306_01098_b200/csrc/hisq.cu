@@ -1394,12 +1394,7 @@ static bool load_memops()
 }
 static CUresult stream_wait_geq(hisq_ctx* h, const void* counter, unsigned value)
 {
-#ifdef HISQ_DEBUG_NOWAIT   // timing experiment only (single rank: stream order already guarantees the arrival)
-    (void)h; (void)counter; (void)value;
-    return CUDA_SUCCESS;
-#else
     return g_wait32((CUstream)h->stream, (CUdeviceptr)(uintptr_t)counter, value, CU_STREAM_WAIT_VALUE_GEQ);
-#endif
 }
 static char* mbox_buffer(char* box, size_t buf, int slot, int hi) { return box + kMboxFlags + kMboxReduce + (size_t)(2 * slot + hi) * buf; }
 static unsigned* mbox_counter(char* box, int slot) { return reinterpret_cast<unsigned*>(box) + slot; }

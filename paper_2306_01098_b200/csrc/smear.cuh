@@ -127,11 +127,9 @@ __global__ void __launch_bounds__(128) smear_init_kernel(T* __restrict__ out, co
 // with Lu = a_up (+ b), Ld = a_dn (+ b); acc(x) += coef (up + dn); up / dn are stored to out_up / out_dn if given (their
 // sum if both point to the same array).  U: the 4V links being smeared; a_*, b, out_*, acc: V matrices of direction mu.
 // All structure-of-arrays (V matrices per block).
-#ifndef HISQ_STAPLE_MINB
-#define HISQ_STAPLE_MINB 4   // CTAs per SM the staple kernel is compiled for (128 registers; measured best of 1, 4, 5, 6)
-#endif
+constexpr int kStapleMinBlocks = 4;   // CTAs per SM the staple kernel is compiled for (128 registers; measured best of 1, 4, 5, 6)
 template <typename T>
-__global__ void __launch_bounds__(128, HISQ_STAPLE_MINB) staple_kernel(const Geom g, const T* __restrict__ U, const T* __restrict__ a_up,
+__global__ void __launch_bounds__(128, kStapleMinBlocks) staple_kernel(const Geom g, const T* __restrict__ U, const T* __restrict__ a_up,
                                                      const T* __restrict__ a_dn, const T* __restrict__ b, T* out_up, T* out_dn,
                                                      T* __restrict__ acc, int mu, int nu, T coef)
 {
