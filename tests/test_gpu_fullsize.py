@@ -88,6 +88,31 @@ def test_c3_64x64x64x16_fp32_nrhs8_sampled(parity):
     assert tiles != (64, 64)            # the nRHS = 8 launch really runs the tiled sweep order
 
 
+def test_c3_64x64x64x16_fp32_nrhs8_full_field():
+    """one oracle application on the WHOLE field for all 8 right-hand sides of the nRHS = 8 launch (the tiled
+    launch shape bench.py times), the oracle on the same fp32-rounded inputs widened to double."""
+    from paper_2306_01098_b200 import layout
+    L, n, parity = (64, 64, 64, 16), 8, 1
+    dev = torch.device("cuda:0")
+    ctx = binding.Hisq(L, "fp32", n, dev)
+    fat, naik = binding.make_links(L, 0, dev, ctx.cdtype, gen_device=dev)
+    ctx.set_links(fat, naik)
+    eo = layout.eo_of_lex(L)
+    X = fat.cpu().permute(1, 0, 2, 3)[eo].contiguous().numpy().astype(np.complex128)     # the fp32 values, widened
+    W = naik.cpu().permute(1, 0, 2, 3)[eo].contiguous().numpy().astype(np.complex128)
+    del fat, naik
+    src = binding.make_sources(L, 2, n, 1 - parity, dev, ctx.cdtype, gen_device=dev)
+    out = ctx.unpack(ctx.dslash(ctx.pack(src), parity))
+    assert ctx.tiles(n) != (64, 64)
+    got = oracle.half_to_full(L, out.cpu().numpy().astype(np.complex128), parity)
+    ref = oracle.dslash_parity(L, X, W, oracle.half_to_full(L, src.cpu().numpy().astype(np.complex128), 1 - parity), parity)
+    ctx.close()
+    for k in range(n):
+        assert rel_l2(got[k], ref[k]) <= 1e-6
+        scale = np.sqrt(np.mean(np.abs(ref[k]) ** 2)) * np.sqrt(2.0)      # RMS over the output parity (the other half is zero)
+        assert np.abs(got[k] - ref[k]).max() / scale <= 2e-5
+
+
 def test_c5_96x96x96x24_fp64_nrhs8_sampled():
     import gc
     gc.collect()
