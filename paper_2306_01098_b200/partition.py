@@ -101,38 +101,49 @@ class HaloExchange:
         self.works, self.staged = [], None
 
 
+def grid_neighbours(rank: int, nranks):
+    """Neighbours of `rank` on the nz x nt grid (rank = rz + nz * rt), periodic in both directions."""
+    nz, nt = grid_of(nranks)
+    rz, rt = rank % nz, rank // nz
+    return {"t_down": rz + nz * ((rt - 1) % nt), "t_up": rz + nz * ((rt + 1) % nt),
+            "z_down": (rz - 1) % nz + nz * rt, "z_up": (rz + 1) % nz + nz * rt}
+
+
 def begin_exchange(send_lo: torch.Tensor, send_hi: torch.Tensor, recv_lo: torch.Tensor, recv_hi: torch.Tensor,
-                   rank: int, nranks: int, dist=None) -> HaloExchange:
-    """Periodic ring in t: my send_hi goes to rank+1's recv_lo, my send_lo to rank-1's recv_hi.
+                   rank: int, nranks: int, dist=None, up=None, down=None, tag_base: int = 0) -> HaloExchange:
+    """One direction of the halo exchange over a periodic ring: my send_hi goes to `up`'s recv_lo, my send_lo to `down`'s
+    recv_hi.  up / down default to the ring of `nranks` ranks along t (rank +- 1); pass grid_neighbours(...) for a rank grid
+    (tag_base keeps the messages of the two directions apart).
     dist = torch.distributed (initialised) or None for a single rank (own halos: periodic wrap onto itself).
     With NCCL the transfers are enqueued behind what the current stream holds so far (the pack kernel) and run on
     NCCL's own stream: kernels launched between begin_exchange and finish() overlap them.  Other backends (gloo: CPU
-    tests, or two processes sharing one GPU) go through the host and complete inside this call."""
-    if nranks == 1 or dist is None:
+    tests, or processes sharing one GPU) go through the host and complete inside this call."""
+    if up is None:
+        up, down = (rank + 1) % nranks, (rank - 1) % nranks
+    if dist is None or (up == rank and down == rank):
         recv_lo.copy_(send_hi)
         recv_hi.copy_(send_lo)
         return HaloExchange()
-    up, down = (rank + 1) % nranks, (rank - 1) % nranks
     stage = send_lo.is_cuda and dist.get_backend() != "nccl"
     # communicate as real arrays (not every backend knows complex dtypes)
     real = lambda t: torch.view_as_real(t) if t.is_complex() else t
     s_lo, s_hi = (real(send_lo.cpu()), real(send_hi.cpu())) if stage else (real(send_lo), real(send_hi))
     r_lo, r_hi = (torch.empty_like(s_lo), torch.empty_like(s_hi)) if stage else (real(recv_lo), real(recv_hi))
     staged = [(real(recv_lo), r_lo), (real(recv_hi), r_hi)] if stage else None
-    if nranks == 2 and dist.get_backend() != "nccl":
+    if up == down and dist.get_backend() != "nccl":
         # both neighbours are the same peer: two tagged exchanges, lower rank sends first (no reliance on message order)
-        for tag, (snd, rcv) in enumerate(((s_hi, r_lo), (s_lo, r_hi))):
-            if rank == 0:
-                dist.send(snd, up, tag=tag)
-                dist.recv(rcv, up, tag=tag)
+        for i, (snd, rcv) in enumerate(((s_hi, r_lo), (s_lo, r_hi))):
+            if rank < up:
+                dist.send(snd, up, tag=tag_base + i)
+                dist.recv(rcv, up, tag=tag_base + i)
             else:
-                dist.recv(rcv, up, tag=tag)
-                dist.send(snd, up, tag=tag)
+                dist.recv(rcv, up, tag=tag_base + i)
+                dist.send(snd, up, tag=tag_base + i)
         return HaloExchange(staged=staged)
     # one grouped call: NCCL matches sends and receives between a pair of ranks in issue order, the same on both sides
-    # (hi -> lo first, then lo -> hi), which also covers nranks == 2 where up == down
-    ops = [dist.P2POp(dist.isend, s_hi, up), dist.P2POp(dist.irecv, r_lo, down),
-           dist.P2POp(dist.isend, s_lo, down), dist.P2POp(dist.irecv, r_hi, up)]
+    # (hi -> lo first, then lo -> hi), which also covers up == down
+    ops = [dist.P2POp(dist.isend, s_hi, up, tag=tag_base), dist.P2POp(dist.irecv, r_lo, down, tag=tag_base),
+           dist.P2POp(dist.isend, s_lo, down, tag=tag_base + 1), dist.P2POp(dist.irecv, r_hi, up, tag=tag_base + 1)]
     return HaloExchange(dist.batch_isend_irecv(ops), staged)
 
 
@@ -140,31 +151,42 @@ def exchange_halos(send_lo, send_hi, recv_lo, recv_hi, rank: int, nranks: int, d
     begin_exchange(send_lo, send_hi, recv_lo, recv_hi, rank, nranks, dist).finish()
 
 
-def dslash_partitioned(ctx, field_in: torch.Tensor, parity: int, rank: int, nranks: int, dist=None, out=None,
+def dslash_partitioned(ctx, field_in: torch.Tensor, parity: int, rank: int, nranks, dist=None, out=None,
                        overlap: bool = True, peer=None):
-    """What one rank does per Dslash application: pack the halo of `field_in`, exchange it, compute.  overlap: the owned
-    slices that read no halo are computed while the exchange is in flight, the first and last 3 afterwards
-    (hisq_dslash_slices; PAPER.md:340-348 'communication hidden behind computation')."""
+    """What one rank does per Dslash application: pack the halos of `field_in`, exchange them, compute.  nranks: an int (cut
+    along t) or (nz, nt).  overlap (t cut only): the owned slices that read no halo are computed while the exchange is in
+    flight, the first and last 3 afterwards (hisq_dslash_slices; PAPER.md:340-348 'communication hidden behind computation')."""
     n = field_in.shape[0]
-    if peer is not None:             # PeerHalo: the pack kernel writes into the neighbours' mailboxes
+    nz, nt = grid_of(nranks)
+    if peer is not None:             # PeerHalo: the pack kernels write into the neighbours' mailboxes (both directions)
         peer.send(field_in)
         arrive = lambda: peer.recv(field_in)
     else:
+        nb = grid_neighbours(rank, nranks)
         slo, shi = ctx.halo_buffers(n)
         rlo, rhi = ctx.halo_buffers(n)
         ctx.halo_pack(field_in, slo, shi)
-        ex = begin_exchange(slo, shi, rlo, rhi, rank, nranks, dist)
+        ex = begin_exchange(slo, shi, rlo, rhi, rank, nt, dist, up=nb["t_up"], down=nb["t_down"])
+        exz = None
+        if nz > 1:
+            zslo, zshi = ctx.zhalo_buffers(n)
+            zrlo, zrhi = ctx.zhalo_buffers(n)
+            ctx.zhalo_pack(field_in, zslo, zshi)
+            exz = begin_exchange(zslo, zshi, zrlo, zrhi, rank, nz, dist, up=nb["z_up"], down=nb["z_down"], tag_base=2)
 
         def arrive():
             ex.finish()
             ctx.halo_unpack(field_in, rlo, rhi)
-    nt = ctx.L[3] - 2 * HALO_T
-    if not overlap or nt <= 2 * HOP_MAX:
+            if exz is not None:
+                exz.finish()
+                ctx.zhalo_unpack(field_in, zrlo, zrhi)
+    t_cnt = ctx.L[3] - 2 * HALO_T
+    if not overlap or nz > 1 or t_cnt <= 2 * HOP_MAX:
         arrive()
         return ctx.dslash(field_in, parity, out=out)
     if out is None:
         out = ctx.new_field(n)
-    ctx.dslash_slices(field_in, parity, out, HOP_MAX, nt - 2 * HOP_MAX)
+    ctx.dslash_slices(field_in, parity, out, HOP_MAX, t_cnt - 2 * HOP_MAX)
     arrive()
     ctx.dslash_edges(field_in, parity, out, HOP_MAX)
     return out

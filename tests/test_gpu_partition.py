@@ -747,3 +747,58 @@ def test_zt_partitioned_cg_processes_on_one_gpu(grid, prec):
     r = b - oracle.apply_A(L, X, W, m, oracle.half_to_full(L, xh.reshape(2, -1, 3), 0))
     for k in range(2):
         assert np.linalg.norm(r[k]) / np.linalg.norm(b[k]) <= 1.05 * tol
+
+
+def _mp_worker_grid_dslash(rank, grid, port, L, seed, q):
+    import os
+    world = grid[0] * grid[1]
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import torch.distributed as dist
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    dev = torch.device("cuda:0")
+    ctx = binding.Hisq(L, "fp64", 2, dev, part=(rank, grid[0], grid[1]))
+    ctx.set_links(*partition.make_links_part(L, seed, rank, grid, dev))
+    f = ctx.pack(partition.make_sources_part(L, seed + 1, 2, 0, rank, grid, dev))
+    # no mailboxes: both halos travel through torch.distributed (gloo here, staged through the host; NCCL between GPUs)
+    out = partition.dslash_partitioned(ctx, f, 1, rank, grid, dist)
+    xr = torch.view_as_real(partition.interior(ctx, L, grid, ctx.unpack(out)).contiguous().cpu()).contiguous()
+    parts = [torch.empty_like(xr) for _ in range(world)] if rank == 0 else None
+    dist.gather(xr, parts, dst=0)
+    if rank == 0:
+        q.put([torch.view_as_complex(p).numpy() for p in parts])
+    dist.barrier()
+    ctx.close()
+    dist.destroy_process_group()
+
+
+def test_zt_partitioned_dslash_through_torch_distributed_four_processes():
+    """partition.dslash_partitioned on a 2 x 2 grid of ranks with the torch.distributed transport for both halo directions
+    (grid_neighbours + begin_exchange): four processes on the one GPU, the reassembled output bit-equal to the single lattice."""
+    import torch.multiprocessing as mp
+    L, seed, grid = (4, 4, 16, 8), 17, (2, 2)
+    nz, nt = grid
+    ctxmp = mp.get_context("spawn")
+    q = ctxmp.Queue()
+    port = 38900 + __import__("os").getpid() % 2000
+    ps = [ctxmp.Process(target=_mp_worker_grid_dslash, args=(r, grid, port, L, seed, q)) for r in range(nz * nt)]
+    for p in ps:
+        p.start()
+    try:
+        parts = q.get(timeout=200)
+        for p in ps:
+            p.join(timeout=120)
+            assert p.exitcode == 0
+    finally:
+        for p in ps:
+            if p.is_alive():
+                p.kill()
+    Lz_loc, Lt_loc, HLy = L[2] // nz, L[3] // nt, L[0] // 2 * L[1]
+    got = np.zeros((2, L[3], L[2], HLy, 3), dtype=np.complex128)
+    for r, part in enumerate(parts):
+        rz, rt = r % nz, r // nz
+        got[:, rt * Lt_loc:(rt + 1) * Lt_loc, rz * Lz_loc:(rz + 1) * Lz_loc] = part
+    ctx = binding.Hisq(L, "fp64", 2)
+    ctx.set_links(*binding.make_links(L, seed, ctx.device))
+    one = ctx.unpack(ctx.dslash(ctx.pack(binding.make_sources(L, seed + 1, 2, 0, ctx.device)), 1)).cpu().numpy()
+    ctx.close()
+    assert np.array_equal(got.reshape(2, -1, 3), one)

@@ -106,3 +106,48 @@ def test_global_sites_of_rank_cover_the_lattice_once():
         gpar = (x + y + z + t) & 1
         assert torch.all(gpar[: Ve // 2] == 0) and torch.all(gpar[Ve // 2:] == 1)
     assert torch.all(count == 1)
+
+
+# ---- a 2 x 2 grid of ranks (cut along z and t): both directions of the exchange, gloo, CPU tensors ----
+def _grid_worker(rank, grid, port, q):
+    world = grid[0] * grid[1]
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    from paper_2306_01098_b200 import partition
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    nb = partition.grid_neighbours(rank, grid)
+    got = {}
+    for d, (nr, base) in {"t": (grid[1], 0), "z": (grid[0], 2)}.items():
+        code = 100.0 * rank + (10.0 if d == "z" else 0.0)
+        slo = torch.full((1, 3, 4), code + 1, dtype=torch.complex128)      # my lowest owned slices / planes
+        shi = torch.full((1, 3, 4), code + 2, dtype=torch.complex128)      # my highest
+        rlo, rhi = torch.zeros_like(slo), torch.zeros_like(slo)
+        partition.begin_exchange(slo, shi, rlo, rhi, rank, nr, dist, up=nb[d + "_up"], down=nb[d + "_down"], tag_base=base).finish()
+        got[d] = (rlo[0, 0, 0].real.item(), rhi[0, 0, 0].real.item())
+    q.put((rank, nb, got))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("grid", [(2, 2), (2, 1)])
+def test_halo_exchange_grid_routing(grid):
+    nz, nt = grid
+    world = nz * nt
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 32500 + os.getpid() % 2000 + 3 * world
+    ps = [ctx.Process(target=_grid_worker, args=(r, grid, port, q)) for r in range(world)]
+    for p in ps:
+        p.start()
+    res = {r: (nb, got) for r, nb, got in (q.get(timeout=120) for _ in ps)}
+    for p in ps:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for r in range(world):
+        rz, rt = r % nz, r // nz
+        nb, got = res[r]
+        assert nb == {"t_down": rz + nz * ((rt - 1) % nt), "t_up": rz + nz * ((rt + 1) % nt),
+                      "z_down": (rz - 1) % nz + nz * rt, "z_up": (rz + 1) % nz + nz * rt}
+        # lower halo <- the "down" neighbour's highest slices, upper halo <- the "up" neighbour's lowest
+        assert got["t"] == (100.0 * nb["t_down"] + 2, 100.0 * nb["t_up"] + 1)
+        assert got["z"] == (100.0 * nb["z_down"] + 12, 100.0 * nb["z_up"] + 11)
